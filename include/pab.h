@@ -1,0 +1,164 @@
+/*
+ * pab.h -- C ABI of libpab.so: linear-array photoacoustic image reconstruction by order-k
+ * delay-multiply-and-sum (DMAS-k, k = 1..5) beamforming in its O(N)-per-pixel form, for one
+ * NVIDIA B200 (sm_100a).  Method: arXiv 2203.14906, "Higher-order correlation based real-time
+ * beamforming in photoacoustic imaging".  Citations are PAPER.md:<line> (the paper's text) and
+ * DESIGN.md reading numbers A1..A19.
+ *
+ * What the library computes, per pixel (x_j, z_m) and frame:
+ *   delay      idx_i = fs * sqrt((x_j - xe_i)^2 + z_m^2) / c            (eq. 1's Delta_i; A5)
+ *   sample     s_i   = (1-a) rf_i[i0] + a rf_i[i0+1], i0 = floor(idx_i), a = idx_i - i0,
+ *                      0 when i0 < 0 or i0+1 > n_samp-1                 (eq. 1; A4, A6)
+ *   root       u_i   = sgn(s_i) |s_i|^(1/k)                             (A3)
+ *   power sums p_m   = sum_i u_i^m, m = 1..k   (p_k = sum s_i or sum |s_i|)
+ *   output     e_k(u_1..u_N) from p_1..p_k by Newton's identities       (eqs. 1, 3, 7, 8, 9: PAPER.md:29, :45,
+ *                                                                        :66, :69, :71-82 with repair A1)
+ *   optional   axial band-pass FIR -> Hilbert-FIR envelope -> log compression   (A8-A12)
+ *
+ * All pointers named *_dev are CUDA device pointers, *_host are host pointers.  No torch types, no
+ * exceptions, no global state.  Every function returns PAB_OK (0) or a negative error code; on an argument
+ * error nothing is written and nothing is launched.  There is no CPU fallback: without a usable sm_100
+ * device pab_create fails with PAB_ERR_DEVICE.
+ */
+#ifndef PAB_H_
+#define PAB_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PAB_OK            0
+#define PAB_ERR_INVALID  (-1)   /* null pointer, non-positive size, order outside 1..5, misaligned pointer        */
+#define PAB_ERR_DEVICE   (-2)   /* no CUDA device, or the current device is not compute capability 10.x           */
+#define PAB_ERR_ALLOC    (-3)   /* device or pinned-host allocation failed                                        */
+#define PAB_ERR_CUDA     (-4)   /* a CUDA call or kernel launch failed (see pab_last_cuda_error)                  */
+
+/* input sample type (pab_set_input) */
+#define PAB_F32 0
+#define PAB_I16 1
+
+/* post-processing mode (pab_set_post): what `out` holds */
+#define PAB_RAW      0   /* the beamformed image e_k (pre-band-pass); default                                     */
+#define PAB_BANDPASS 1   /* after the axial band-pass FIR                                                         */
+#define PAB_ENVELOPE 2   /* after band-pass and Hilbert-FIR envelope                                              */
+#define PAB_LOG      3   /* after band-pass, envelope and log compression, dB <= 0                                */
+
+/* beamforming kernel variant (pab_set_variant) */
+#define PAB_VARIANT_AUTO   0   /* staged when its shared-memory plan fits, else direct                            */
+#define PAB_VARIANT_DIRECT 1   /* per-thread gathers through L1/L2 from the staged RF copy, no shared memory      */
+#define PAB_VARIANT_STAGED 2   /* per-tile RF windows bulk-copied (TMA 1-D) into shared memory, mbarrier pipeline */
+
+typedef struct pab_ctx pab_ctx;     /* opaque; created by pab_create, owned by the library, freed by pab_destroy  */
+
+/* Pixel grid (A5).  Pixel (m, j), row m in depth and column j laterally, has its centre at
+ * (x, z) = (x0 + j*dx, z0 + m*dz), metres.  The array lies on z = 0, centred on x = 0. */
+typedef struct {
+    int   nx, nz;            /* columns (lateral), rows (depth); both >= 1                                        */
+    float x0, dx, z0, dz;    /* metres; dx > 0, dz > 0, z0 >= 0                                                    */
+} pab_grid;
+
+/* The plan the library derives from a geometry (host logic only; see pab_plan). */
+typedef struct {
+    int   tile_z, tile_x;        /* pixel tile of one thread block of the staged kernel (rows, columns)            */
+    int   window_samples;        /* upper bound of the per-channel RF window a tile needs, samples (mult. of 4)    */
+    int   chunk_channels;        /* channels staged per pipeline stage                                             */
+    int   stages;                /* pipeline depth                                                                 */
+    int   smem_bytes;            /* dynamic shared memory per block, bytes; 0 when the staged kernel does not fit  */
+    int   frames_per_thread;     /* frames each thread carries in registers when n_frames >= 4 (4 or 8)            */
+    int   batch_frames;          /* internal frame batch per pass (ingest -> beamform -> post)                     */
+    double zs_per_row;           /* dz * fs / c : delay samples per pixel row                                      */
+    double xs_per_col;           /* dx * fs / c : delay samples per pixel column at grazing incidence              */
+} pab_plan_info;
+
+/*
+ * pab_create -- build a context for one array + grid (N-element linear array,
+ * pitch, sampling frequency fs, speed of sound c; one-way time of flight, record starts at t = 0: A5).
+ *   out       receives the handle (host pointer, written only on success)
+ *   n_elem    N >= 1, element i at x = (i - (N-1)/2) * pitch_m, z = 0
+ *   n_samp    S >= 2 samples per channel per frame
+ *   fs_hz, c_m_s, pitch_m   > 0
+ *   grid      host pointer, copied
+ * Uploads the per-row / per-column / per-element delay tables (computed in fp64 on the host, stored as
+ * fp32 hi+lo pairs in sample units) and allocates scratch.  Uses the CUDA device current at the call.
+ * Errors: PAB_ERR_INVALID, PAB_ERR_DEVICE, PAB_ERR_ALLOC, PAB_ERR_CUDA.
+ */
+int pab_create(pab_ctx** out, int n_elem, int n_samp, float fs_hz, float c_m_s, float pitch_m,
+               const pab_grid* grid);
+
+/* pab_set_input -- RF sample type and scale: sample value = scale * stored value (A15).  Default PAB_F32, 1.0.
+ * int16 ADC counts are converted to fp32 exactly while the frames are staged (BASELINE.json config C5). */
+int pab_set_input(pab_ctx* ctx, int dtype, float scale);
+
+/*
+ * pab_set_post -- post chain after the combination (A8-A13).  Default PAB_RAW.
+ *   mode             PAB_RAW | PAB_BANDPASS | PAB_ENVELOPE | PAB_LOG
+ *   f_center_hz, f_halfwidth_hz   pass band [f_c - f_hw, f_c + f_hw] of the Hamming-windowed-sinc band-pass, in Hz
+ *                    of the axial sampling rate fs_z = c / dz (one row per c/dz seconds of one-way flight)
+ *   n_taps_bp        T, 2..256:  y[m] = sum_{t<T} h[t] x[m + T/2 - t], x = 0 outside the image (A12)
+ *   n_taps_hilbert   2L+1, odd, 3..255: q[m] = sum_{|t|<=L} g[t] y[m-t], g[t] = 2/(pi t) * Hamming for odd t, 0 for
+ *                    even t; env = sqrt(y^2 + q^2) (A9)
+ *   dyn_range_db     DR > 0: out = max(20 log10(env / max_frame env), -DR); env = 0 or max = 0 gives -DR (A10)
+ */
+int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz, int n_taps_bp,
+                 int n_taps_hilbert, float dyn_range_db);
+
+/* pab_set_variant -- force a beamforming kernel variant (testing / benchmarking).  PAB_ERR_INVALID when the
+ * staged variant is requested but its plan does not fit in shared memory. */
+int pab_set_variant(pab_ctx* ctx, int variant);
+
+/*
+ * pab_beamform -- enqueue the whole hot path for n_frames frames on `cuda_stream` and return (never
+ * synchronises).
+ *   rf_dev     device pointer, [n_frames][n_elem][n_samp], sample index fastest, fp32 or int16 per
+ *              pab_set_input; aligned to its element size; read only; caller keeps it alive until the
+ *              stream work finishes
+ *   n_frames   >= 1; frames are independent; the library batches them internally
+ *   order      k = 1..5 (1 = DAS eq. 1, 2 = DMAS eq. 3, 3..5 = eqs. 7, 8, 9)
+ *   out_dev    device pointer, [n_frames][nz][nx], x fastest, fp32, 4-byte aligned; fully overwritten
+ *   cuda_stream a cudaStream_t passed as void*; NULL = the legacy default stream
+ * One context must not be used from two streams at once (shared scratch).
+ * Errors: PAB_ERR_INVALID (nothing launched), PAB_ERR_CUDA.
+ */
+int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int order, float* out_dev, void* cuda_stream);
+
+/*
+ * pab_beamform_host -- the same path from HOST buffers: copies rf_host to the device in frame batches
+ * through pinned staging buffers (copies overlapped with compute on two internal streams), runs the
+ * kernels, copies the images back to out_host, and returns after everything has finished.
+ *   rf_host   host pointer, same layout and type as rf_dev above (pageable or pinned)
+ *   out_host  host pointer, [n_frames][nz][nx] fp32
+ */
+int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host);
+
+/* pab_destroy -- free the context and everything it owns.  NULL is a no-op.  Synchronises the device. */
+void pab_destroy(pab_ctx* ctx);
+
+/* pab_plan -- host-only: the tiling / staging plan for a geometry (no GPU needed; pab_create uses the
+ * same routine).  smem_limit_bytes <= 0 means the sm_100 opt-in limit (232448).  Returns PAB_ERR_INVALID
+ * on bad arguments. */
+int pab_plan(int n_elem, int n_samp, float fs_hz, float c_m_s, float pitch_m, const pab_grid* grid,
+             int smem_limit_bytes, pab_plan_info* plan_out);
+
+/* pab_get_plan -- the plan a context is using. */
+int pab_get_plan(const pab_ctx* ctx, pab_plan_info* plan_out);
+
+/* pab_design_bandpass / pab_design_hilbert -- host-only: the FIR taps pab_set_post uploads (fp64 design,
+ * rounded to fp32).  h_host[T]; g_host[2L+1] with g_host[t + L] = g[t].  f_lo, f_hi in cycles per row. */
+int pab_design_bandpass(int n_taps, double f_lo, double f_hi, float* h_host);
+int pab_design_hilbert(int half_len, float* g_host);
+
+/* pab_launch_count -- number of kernels this context has launched since it was created. */
+long long pab_launch_count(const pab_ctx* ctx);
+
+/* pab_strerror -- static string for an error code.  pab_last_cuda_error -- the last cudaError_t string seen
+ * by this context ("" if none). */
+const char* pab_strerror(int code);
+const char* pab_last_cuda_error(const pab_ctx* ctx);
+
+/* pab_version -- "pab <major>.<minor> sm_100a". */
+const char* pab_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAB_H_ */

@@ -1,0 +1,109 @@
+// pab_math.cuh -- per-item arithmetic of the DMAS-k hot path (steps a2..a6 of DESIGN.md).
+//
+// Everything here is fp32 on the plain ALUs: FMA/ALU pipes plus the XU (MUFU) pipe for the roots.
+// Explicit approximate PTX intrinsics are used instead of a fast-math flag:
+//   lg2.approx.ftz / ex2.approx.ftz for the cube and fifth root, sqrt.approx.ftz for order 2,
+//   rsqrt.approx.ftz twice for the fourth root, rcp.approx.ftz + sqrt.approx.ftz for the delay.
+// lg2(0) = -inf and ex2(-inf) = +0, rsqrt(0) = +inf and rsqrt(+inf) = +0, so the root of zero is zero
+// without a branch; a negative argument never reaches a root (|s| is taken first, the sign copied back:
+// PAPER.md:41, :62, reading A3).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pab {
+
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// copysign(|r|, s) as one LOP3: (r & 0x7fffffff) | (s & 0x80000000)
+__device__ __forceinline__ float copy_sign(float r, float s) {
+    return __uint_as_float((__float_as_uint(r) & 0x7fffffffu) | (__float_as_uint(s) & 0x80000000u));
+}
+
+// Step a4 + a5: signed k-th root u = sgn(s)|s|^(1/k) and the running power sums p_m += u^m, m = 1..k,
+// with p_k += s (odd k) or |s| (even k), which needs no root (Table I :86-95).
+template <int K>
+__device__ __forceinline__ void accumulate(float s, float (&p)[K]) {
+    if constexpr (K == 1) {
+        p[0] += s;                                            // eq. (1)
+    } else if constexpr (K == 2) {
+        const float u = copy_sign(sqrt_approx(fabsf(s)), s);  // eq. (3)
+        p[0] += u;
+        p[1] += fabsf(s);
+    } else if constexpr (K == 3) {
+        const float r = ex2_approx(lg2_approx(fabsf(s)) * (1.0f / 3.0f));
+        const float u = copy_sign(r, s);                      // eq. (7): real cube root (A3)
+        p[0] += u;
+        p[1] = fmaf(u, u, p[1]);
+        p[2] += s;
+    } else if constexpr (K == 4) {
+        const float r = rsqrt_approx(rsqrt_approx(fabsf(s))); // |s|^(1/4); 0 -> inf -> 0
+        const float u = copy_sign(r, s);                      // eq. (8): signed fourth root
+        const float u2 = r * r;
+        p[0] += u;
+        p[1] += u2;
+        p[2] = fmaf(u2, u, p[2]);
+        p[3] += fabsf(s);
+    } else {
+        static_assert(K == 5, "orders 1..5");
+        const float r = ex2_approx(lg2_approx(fabsf(s)) * 0.2f);
+        const float u = copy_sign(r, s);                      // eq. (9): real fifth root (A3)
+        const float u2 = r * r;
+        p[0] += u;
+        p[1] += u2;
+        p[2] = fmaf(u2, u, p[2]);
+        p[3] = fmaf(u2, u2, p[3]);
+        p[4] += s;
+    }
+}
+
+// Step a6: e_k from p_1..p_k by Newton's identities, m e_m = sum_{i=1..m} (-1)^(i-1) e_{m-i} p_i.
+// Expanded, these are the paper's eqs. (3), (7), (8), (9) (eq. 9 with the lost square restored, reading A1).
+template <int K>
+__device__ __forceinline__ float combine(const float (&p)[K]) {
+    const float e1 = p[0];
+    if constexpr (K == 1) return e1;
+    else {
+        const float e2 = 0.5f * fmaf(e1, p[0], -p[1]);
+        if constexpr (K == 2) return e2;
+        else {
+            const float e3 = (1.0f / 3.0f) * (fmaf(e2, p[0], -e1 * p[1]) + p[2]);
+            if constexpr (K == 3) return e3;
+            else {
+                const float e4 = 0.25f * ((fmaf(e3, p[0], -e2 * p[1]) + e1 * p[2]) - p[3]);
+                if constexpr (K == 4) return e4;
+                else return 0.2f * (((fmaf(e4, p[0], -e3 * p[1]) + e2 * p[2]) - e1 * p[3]) + p[4]);
+            }
+        }
+    }
+}
+
+// Step a2 + the index half of a3, once per (pixel, element), shared by every frame a thread carries.
+//   xs   lateral offset pixel - element in samples;  row: (zs, zs^2, zf - 1/2, zi) with zs = z fs / c = zi + zf
+//   idx = zs + xs^2 / (sqrt(xs^2 + zs^2) + zs)   (== fs sqrt(dx^2 + z^2) / c, without the
+//   cancellation and without one float carrying a 12-bit integer part: DESIGN.md "Delay index precision")
+// Returns i0 = floor(idx) clamped into [0, S-2]; wa, wb = interpolation weights of rf[i0+1], rf[i0]
+// (both 0 when the delayed sample falls outside the record: reading A6).
+struct Tap { int i0; float wa, wb; };
+
+__device__ __forceinline__ Tap delay_tap(float xs, const float4 row, int S) {
+    const float xs2 = xs * xs;
+    const float d = sqrt_approx(fmaf(xs, xs, row.y));
+    const float delta = fminf(xs2 * rcp_approx(fmaxf(d + row.x, 1e-30f)), 2097152.0f);
+    const float w = row.z + delta;                              // idx - zi - 1/2  >= -1/2
+    const float t = w + 12582912.0f;                            // round to nearest integer: floor(idx - zi)
+    const float fl = t - 12582912.0f;
+    int i0 = __float_as_int(row.w) + (__float_as_int(t) - 0x4B400000);
+    float a = (w - fl) + 0.5f;
+    const bool ok = (i0 >= 0) && (i0 <= S - 2);
+    Tap r;
+    r.i0 = ok ? i0 : 0;
+    r.wa = ok ? a : 0.0f;
+    r.wb = ok ? 1.0f - a : 0.0f;
+    return r;
+}
+
+}  // namespace pab
