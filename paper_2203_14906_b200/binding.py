@@ -1,0 +1,208 @@
+"""Thin ctypes binding of libpab.so (include/pab.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device memory and
+streams (torch tensors in, torch tensors out).  There is no CPU fallback: `load()` raises if libpab.so is
+missing, and `Beamformer` raises if the library reports an error.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpab.so")
+
+OK, ERR_INVALID, ERR_DEVICE, ERR_ALLOC, ERR_CUDA = 0, -1, -2, -3, -4
+F32, I16 = 0, 1
+RAW, BANDPASS, ENVELOPE, LOG = 0, 1, 2, 3
+VARIANT_AUTO, VARIANT_DIRECT, VARIANT_STAGED = 0, 1, 2
+_MODES = {"raw": RAW, "bandpass": BANDPASS, "envelope": ENVELOPE, "log": LOG}
+_VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_STAGED}
+
+# every symbol include/pab.h declares
+SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_beamform", "pab_beamform_host",
+           "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
+           "pab_launch_count", "pab_strerror", "pab_last_cuda_error", "pab_version"]
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("nz", C.c_int), ("x0", C.c_float), ("dx", C.c_float),
+                ("z0", C.c_float), ("dz", C.c_float)]
+
+
+class PlanInfo(C.Structure):
+    _fields_ = [("tile_z", C.c_int), ("tile_x", C.c_int), ("window_samples", C.c_int), ("chunk_channels", C.c_int),
+                ("stages", C.c_int), ("smem_bytes", C.c_int), ("frames_per_thread", C.c_int),
+                ("batch_frames", C.c_int), ("zs_per_row", C.c_double), ("xs_per_col", C.c_double)]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class PabError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load(build_if_missing: bool = False):
+    """dlopen libpab.so and declare the prototypes.  Fails loudly when the library is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        from . import build as _b
+        _b.build_lib()
+    if not os.path.exists(LIB_PATH):
+        raise PabError(f"{LIB_PATH} is missing: build it with `python -m paper_2203_14906_b200.build` "
+                       "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, ip, fp = C.c_void_p, C.c_int, C.c_float
+    L.pab_create.argtypes = [C.POINTER(vp), ip, ip, fp, fp, fp, C.POINTER(Grid)]
+    L.pab_set_input.argtypes = [vp, ip, fp]
+    L.pab_set_post.argtypes = [vp, ip, fp, fp, ip, ip, fp]
+    L.pab_set_variant.argtypes = [vp, ip]
+    L.pab_beamform.argtypes = [vp, vp, ip, ip, vp, vp]
+    L.pab_beamform_host.argtypes = [vp, vp, ip, ip, vp]
+    L.pab_destroy.argtypes = [vp]
+    L.pab_destroy.restype = None
+    L.pab_plan.argtypes = [ip, ip, fp, fp, fp, C.POINTER(Grid), ip, C.POINTER(PlanInfo)]
+    L.pab_get_plan.argtypes = [vp, C.POINTER(PlanInfo)]
+    L.pab_design_bandpass.argtypes = [ip, C.c_double, C.c_double, C.POINTER(C.c_float)]
+    L.pab_design_hilbert.argtypes = [ip, C.POINTER(C.c_float)]
+    L.pab_launch_count.argtypes = [vp]
+    L.pab_launch_count.restype = C.c_longlong
+    L.pab_strerror.argtypes = [ip]
+    L.pab_strerror.restype = C.c_char_p
+    L.pab_last_cuda_error.argtypes = [vp]
+    L.pab_last_cuda_error.restype = C.c_char_p
+    L.pab_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _grid(g) -> Grid:
+    return Grid(int(g.nx), int(g.nz), float(g.x0), float(g.dx), float(g.z0), float(g.dz))
+
+
+def plan(g, smem_limit: int = 0) -> dict:
+    """pab_plan: the tiling / staging plan for a geometry (host-only, no GPU needed)."""
+    info = PlanInfo()
+    gr = _grid(g)
+    rc = load().pab_plan(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, C.byref(gr), smem_limit, C.byref(info))
+    if rc != OK:
+        raise PabError(f"pab_plan: {load().pab_strerror(rc).decode()}")
+    return info.asdict()
+
+
+def design_bandpass(n_taps: int, f_lo: float, f_hi: float):
+    import numpy as np
+    h = np.zeros(n_taps, dtype=np.float32)
+    rc = load().pab_design_bandpass(n_taps, f_lo, f_hi, h.ctypes.data_as(C.POINTER(C.c_float)))
+    if rc != OK:
+        raise PabError(f"pab_design_bandpass: {load().pab_strerror(rc).decode()}")
+    return h
+
+
+def design_hilbert(half_len: int):
+    import numpy as np
+    g = np.zeros(2 * half_len + 1, dtype=np.float32)
+    rc = load().pab_design_hilbert(half_len, g.ctypes.data_as(C.POINTER(C.c_float)))
+    if rc != OK:
+        raise PabError(f"pab_design_hilbert: {load().pab_strerror(rc).decode()}")
+    return g
+
+
+def shard_frames(n_frames: int, rank: int, world: int):
+    """Replicas-only multi-GPU: contiguous frame range [lo, hi) of `rank`; frames are
+    independent, so there is no exchange step and no collective on the data path."""
+    base, rem = divmod(n_frames, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+class Beamformer:
+    """pab_create / pab_set_* / pab_beamform / pab_destroy for one geometry on the current CUDA device."""
+
+    def __init__(self, g, dtype: str = "float32", scale: float = 1.0, post: dict | None = None,
+                 variant: str = "auto"):
+        self._L = load()
+        self._h = C.c_void_p()
+        self.geom = g
+        gr = _grid(g)
+        self._check(self._L.pab_create(C.byref(self._h), g.n_elem, g.n_samp, g.fs, g.c, g.pitch, C.byref(gr)),
+                    "pab_create")
+        self.dtype = dtype
+        self._check(self._L.pab_set_input(self._h, I16 if dtype == "int16" else F32, scale), "pab_set_input")
+        if post:
+            self.set_post(**post)
+        if variant != "auto":
+            self.set_variant(variant)
+
+    def _check(self, rc, what):
+        if rc != OK:
+            detail = self._L.pab_last_cuda_error(self._h).decode() if self._h else ""
+            raise PabError(f"{what}: {self._L.pab_strerror(rc).decode()} {detail}".strip())
+
+    def set_post(self, mode="log", f_center=10e6, f_halfwidth=2.5e6, n_taps_bp=64, n_taps_hilbert=63,
+                 dyn_range_db=60.0):
+        self._check(self._L.pab_set_post(self._h, _MODES[mode], f_center, f_halfwidth, n_taps_bp, n_taps_hilbert,
+                                         dyn_range_db), "pab_set_post")
+
+    def set_variant(self, variant: str):
+        self._check(self._L.pab_set_variant(self._h, _VARIANTS[variant]), "pab_set_variant")
+
+    def plan(self) -> dict:
+        info = PlanInfo()
+        self._check(self._L.pab_get_plan(self._h, C.byref(info)), "pab_get_plan")
+        return info.asdict()
+
+    def launch_count(self) -> int:
+        return int(self._L.pab_launch_count(self._h))
+
+    def beamform(self, rf, order: int, out=None, stream=None):
+        """rf: CUDA tensor [F][N][S] float32 or int16 -> out: CUDA tensor [F][nz][nx] float32 (enqueue only)."""
+        import torch
+        g = self.geom
+        assert rf.is_cuda and rf.is_contiguous() and rf.dim() == 3, "rf must be a contiguous CUDA tensor [F][N][S]"
+        assert tuple(rf.shape[1:]) == (g.n_elem, g.n_samp), rf.shape
+        assert rf.dtype == (torch.int16 if self.dtype == "int16" else torch.float32), rf.dtype
+        F = rf.shape[0]
+        if out is None:
+            out = torch.empty((F, g.nz, g.nx), dtype=torch.float32, device=rf.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and tuple(out.shape) == (F, g.nz, g.nx)
+        st = torch.cuda.current_stream(rf.device) if stream is None else stream
+        self._check(self._L.pab_beamform(self._h, rf.data_ptr(), F, order, out.data_ptr(), st.cuda_stream), "pab_beamform")
+        return out
+
+    def beamform_host(self, rf, order: int, out=None):
+        """rf: host array/tensor [F][N][S] (numpy or CPU torch, pinned or not) -> out: same kind, [F][nz][nx]."""
+        import numpy as np
+        import torch
+        g = self.geom
+        is_torch = isinstance(rf, torch.Tensor)
+        F = rf.shape[0]
+        if is_torch:
+            assert not rf.is_cuda and rf.is_contiguous()
+            if out is None:
+                out = torch.empty((F, g.nz, g.nx), dtype=torch.float32, pin_memory=rf.is_pinned())
+            src, dst = rf.data_ptr(), out.data_ptr()
+        else:
+            rf = np.ascontiguousarray(rf)
+            if out is None:
+                out = np.empty((F, g.nz, g.nx), dtype=np.float32)
+            src, dst = rf.ctypes.data, out.ctypes.data
+        self._check(self._L.pab_beamform_host(self._h, src, F, order, dst), "pab_beamform_host")
+        return out
+
+    def close(self):
+        if self._h:
+            self._L.pab_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

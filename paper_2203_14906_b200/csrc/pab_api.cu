@@ -1,0 +1,213 @@
+// pab_api.cu -- the C ABI of libpab.so (include/pab.h): context, host logic, kernel launches.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+#include <cuda_runtime.h>
+#include "../../include/pab.h"
+#include "pab_plan.h"
+#include "pab_kernels.cuh"
+#include "pab_staged.cuh"
+
+using namespace pab;
+
+struct pab_ctx {
+    int N = 0, S = 0, Sp = 0;
+    float fs = 0, c = 0, pitch = 0;
+    pab_grid grid{};
+    int dtype = PAB_F32;
+    float scale = 1.0f;
+    int post_mode = PAB_RAW;
+    int n_taps_bp = 0, n_taps_h = 0, TpB = 0, TpH = 0;
+    float dyn_range_db = 60.0f;
+    int variant = PAB_VARIANT_AUTO;
+    pab_plan_info plan{};
+    int device = 0, sm_count = 0, smem_optin = 0;
+    // device tables
+    float2* d_xj = nullptr;
+    float2* d_xe = nullptr;
+    float4* d_zrow = nullptr;
+    float* d_stage = nullptr;        // staged RF of one batch (quad or lin layout)
+    size_t stage_bytes = 0;
+    float* d_img = nullptr;          // beamformed image of one batch when a post chain is on
+    float* d_taps_bp = nullptr;
+    float* d_taps_h = nullptr;
+    unsigned int* d_max = nullptr;   // [batch] per-frame max of the envelope
+    // host-buffer path (lazy)
+    void* d_in[2] = {nullptr, nullptr};
+    float* d_out[2] = {nullptr, nullptr};
+    cudaStream_t s_h2d = nullptr, s_run = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_run[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    long long launches = 0;
+    char err[256] = {0};
+};
+
+namespace {
+
+int cuda_fail(pab_ctx* ctx, cudaError_t e, const char* what) {
+    if (ctx) snprintf(ctx->err, sizeof ctx->err, "%s: %s", what, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? PAB_ERR_ALLOC : PAB_ERR_CUDA;
+}
+
+#define PAB_CUDA(ctx, call)                                          \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return cuda_fail((ctx), e_, #call);   \
+    } while (0)
+
+size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
+
+void free_all(pab_ctx* ctx) {
+    cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max);
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
+        if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
+        if (ctx->ev_run[b]) cudaEventDestroy(ctx->ev_run[b]);
+        if (ctx->ev_out[b]) cudaEventDestroy(ctx->ev_out[b]);
+    }
+    if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
+    if (ctx->s_run) cudaStreamDestroy(ctx->s_run);
+    if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* pab_version(void) { return "pab 0.1 sm_100a"; }
+
+const char* pab_strerror(int code) {
+    switch (code) {
+    case PAB_OK: return "ok";
+    case PAB_ERR_INVALID: return "invalid argument";
+    case PAB_ERR_DEVICE: return "no usable sm_100 CUDA device";
+    case PAB_ERR_ALLOC: return "allocation failed";
+    case PAB_ERR_CUDA: return "CUDA call failed";
+    default: return "unknown error code";
+    }
+}
+
+const char* pab_last_cuda_error(const pab_ctx* ctx) { return ctx ? ctx->err : ""; }
+long long pab_launch_count(const pab_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int pab_plan(int n_elem, int n_samp, float fs_hz, float c_m_s, float pitch_m, const pab_grid* grid,
+             int smem_limit_bytes, pab_plan_info* plan_out) {
+    if (!grid || !plan_out) return PAB_ERR_INVALID;
+    return plan_geometry(n_elem, n_samp, fs_hz, c_m_s, pitch_m, *grid, smem_limit_bytes, plan_out) ? PAB_OK
+                                                                                                    : PAB_ERR_INVALID;
+}
+
+int pab_get_plan(const pab_ctx* ctx, pab_plan_info* plan_out) {
+    if (!ctx || !plan_out) return PAB_ERR_INVALID;
+    *plan_out = ctx->plan;
+    return PAB_OK;
+}
+
+int pab_design_bandpass(int n_taps, double f_lo, double f_hi, float* h_host) {
+    if (!h_host || n_taps < 2 || n_taps > 256 || !(f_lo >= 0) || !(f_hi > f_lo) || !(f_hi <= 0.5)) return PAB_ERR_INVALID;
+    design_bandpass(n_taps, f_lo, f_hi, h_host);
+    return PAB_OK;
+}
+
+int pab_design_hilbert(int half_len, float* g_host) {
+    if (!g_host || half_len < 1 || half_len > 127) return PAB_ERR_INVALID;
+    design_hilbert(half_len, g_host);
+    return PAB_OK;
+}
+
+int pab_create(pab_ctx** out, int n_elem, int n_samp, float fs_hz, float c_m_s, float pitch_m, const pab_grid* grid) {
+    if (!out || !grid) return PAB_ERR_INVALID;
+    pab_plan_info plan;
+    if (!plan_geometry(n_elem, n_samp, fs_hz, c_m_s, pitch_m, *grid, 0, &plan)) return PAB_ERR_INVALID;
+    if ((long long)n_samp > (1 << 20) || (long long)grid->nx * grid->nz > (1LL << 30)) return PAB_ERR_INVALID;
+    int dev = 0, n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); return PAB_ERR_DEVICE; }
+    if (cudaGetDevice(&dev) != cudaSuccess) return PAB_ERR_DEVICE;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10) return PAB_ERR_DEVICE;
+
+    pab_ctx* ctx = new (std::nothrow) pab_ctx();
+    if (!ctx) return PAB_ERR_ALLOC;
+    ctx->N = n_elem; ctx->S = n_samp; ctx->Sp = round_up(n_samp, 4);
+    ctx->fs = fs_hz; ctx->c = c_m_s; ctx->pitch = pitch_m; ctx->grid = *grid;
+    ctx->device = dev; ctx->sm_count = prop.multiProcessorCount; ctx->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    plan_geometry(n_elem, n_samp, fs_hz, c_m_s, pitch_m, *grid, ctx->smem_optin, &plan);
+    ctx->plan = plan;
+
+    const DelayTables t = make_tables(n_elem, fs_hz, c_m_s, pitch_m, *grid);
+    // one batch of staged RF: quad layout, batch rounded up to whole quads (>= the lin layout of one frame)
+    ctx->stage_bytes = (size_t)plan.batch_frames * n_elem * (size_t)ctx->Sp * 4;
+    int rc = PAB_OK;
+    auto fail = [&](cudaError_t e, const char* what) { rc = cuda_fail(ctx, e, what); };
+    cudaError_t e;
+    if ((e = cudaMalloc(&ctx->d_xj, t.xj.size() * 4)) != cudaSuccess) fail(e, "cudaMalloc xj");
+    else if ((e = cudaMalloc(&ctx->d_xe, t.xe.size() * 4)) != cudaSuccess) fail(e, "cudaMalloc xe");
+    else if ((e = cudaMalloc(&ctx->d_zrow, t.zrow.size() * 4)) != cudaSuccess) fail(e, "cudaMalloc zrow");
+    else if ((e = cudaMalloc(&ctx->d_stage, ctx->stage_bytes)) != cudaSuccess) fail(e, "cudaMalloc stage");
+    else if ((e = cudaMalloc(&ctx->d_max, (size_t)plan.batch_frames * 4)) != cudaSuccess) fail(e, "cudaMalloc max");
+    else if ((e = cudaMemcpy(ctx->d_xj, t.xj.data(), t.xj.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) fail(e, "copy xj");
+    else if ((e = cudaMemcpy(ctx->d_xe, t.xe.data(), t.xe.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) fail(e, "copy xe");
+    else if ((e = cudaMemcpy(ctx->d_zrow, t.zrow.data(), t.zrow.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) fail(e, "copy zrow");
+    if (rc == PAB_OK) rc = staged_configure(ctx->smem_optin);
+    if (rc == PAB_OK &&
+        (cudaFuncSetAttribute(post_fir_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin) != cudaSuccess ||
+         cudaFuncSetAttribute(post_fir_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin) != cudaSuccess))
+        rc = PAB_ERR_CUDA;
+    if (rc != PAB_OK) { free_all(ctx); delete ctx; return rc; }
+    *out = ctx;
+    return PAB_OK;
+}
+
+void pab_destroy(pab_ctx* ctx) {
+    if (!ctx) return;
+    cudaDeviceSynchronize();
+    free_all(ctx);
+    delete ctx;
+}
+
+int pab_set_input(pab_ctx* ctx, int dtype, float scale) {
+    if (!ctx || (dtype != PAB_F32 && dtype != PAB_I16) || !(scale == scale) || scale == 0.0f) return PAB_ERR_INVALID;
+    ctx->dtype = dtype; ctx->scale = scale;
+    return PAB_OK;
+}
+
+int pab_set_variant(pab_ctx* ctx, int variant) {
+    if (!ctx || variant < PAB_VARIANT_AUTO || variant > PAB_VARIANT_STAGED) return PAB_ERR_INVALID;
+    if (variant == PAB_VARIANT_STAGED && ctx->plan.smem_bytes == 0) return PAB_ERR_INVALID;
+    ctx->variant = variant;
+    return PAB_OK;
+}
+
+int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz, int n_taps_bp, int n_taps_hilbert,
+                 float dyn_range_db) {
+    if (!ctx || mode < PAB_RAW || mode > PAB_LOG) return PAB_ERR_INVALID;
+    if (mode == PAB_RAW) { ctx->post_mode = PAB_RAW; return PAB_OK; }
+    const double fs_z = (double)ctx->c / (double)ctx->grid.dz;      // axial sampling rate, one-way (A13)
+    const double f_lo = ((double)f_center_hz - (double)f_halfwidth_hz) / fs_z;
+    const double f_hi = ((double)f_center_hz + (double)f_halfwidth_hz) / fs_z;
+    if (n_taps_bp < 2 || n_taps_bp > 256 || !(f_lo >= 0) || !(f_hi > f_lo) || !(f_hi <= 0.5)) return PAB_ERR_INVALID;
+    if (mode >= PAB_ENVELOPE && (n_taps_hilbert < 3 || n_taps_hilbert > 255 || !(n_taps_hilbert & 1))) return PAB_ERR_INVALID;
+    if (mode == PAB_LOG && !(dyn_range_db > 0)) return PAB_ERR_INVALID;
+    const int TpB = round_up(n_taps_bp, 8);
+    const int TpH = mode >= PAB_ENVELOPE ? round_up(n_taps_hilbert, 8) : 8;
+    std::vector<float> hb(TpB, 0.0f), hh(TpH, 0.0f);
+    design_bandpass(n_taps_bp, f_lo, f_hi, hb.data());
+    if (mode >= PAB_ENVELOPE) design_hilbert((n_taps_hilbert - 1) / 2, hh.data());
+    PAB_CUDA(ctx, cudaDeviceSynchronize());
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); ctx->d_taps_bp = ctx->d_taps_h = nullptr;
+    PAB_CUDA(ctx, cudaMalloc(&ctx->d_taps_bp, TpB * 4));
+    PAB_CUDA(ctx, cudaMalloc(&ctx->d_taps_h, TpH * 4));
+    PAB_CUDA(ctx, cudaMemcpy(ctx->d_taps_bp, hb.data(), TpB * 4, cudaMemcpyHostToDevice));
+    PAB_CUDA(ctx, cudaMemcpy(ctx->d_taps_h, hh.data(), TpH * 4, cudaMemcpyHostToDevice));
+    if (!ctx->d_img)
+        PAB_CUDA(ctx, cudaMalloc(&ctx->d_img, (size_t)ctx->plan.batch_frames * ctx->grid.nz * (size_t)ctx->grid.nx * 4));
+    ctx->post_mode = mode; ctx->n_taps_bp = n_taps_bp; ctx->n_taps_h = n_taps_hilbert;
+    ctx->TpB = TpB; ctx->TpH = TpH; ctx->dyn_range_db = dyn_range_db;
+    return PAB_OK;
+}
+
+}  // extern "C"
+
+#include "pab_run.inl"

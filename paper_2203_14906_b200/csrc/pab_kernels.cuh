@@ -175,7 +175,7 @@ __device__ __forceinline__ void fir8(const float* in_col, int in_r0, const float
 
 template <int TZ, bool ENV>
 __global__ void __launch_bounds__(256) post_fir_kernel(const PostParams P) {
-    extern __shared__ float smem[];
+    extern __shared__ float post_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int col0 = blockIdx.x * 32, r0 = blockIdx.y * TZ, f = blockIdx.z;
     const int col = col0 + lane;
@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(256) post_fir_kernel(const PostParams P) {
     const int YR = ENV ? ((TZ + P.TpH - 1 + 7) & ~7) : TZ;
     const int xr0 = yr0 + P.shiftB - P.TpB + 1;
     const int XR = YR + P.TpB - 1;
-    float* xs = smem;                    // [XR][32]
+    float* xs = post_smem;                    // [XR][32]
     float* ys = xs + XR * 32;            // [YR][32]   (ENV only)
     float* hb = ys + (ENV ? YR * 32 : 0);   // [TpB]
     float* hh = hb + P.TpB;              // [TpH]
@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(256) post_fir_kernel(const PostParams P) {
     }
     __syncthreads();
     float acc[8];
-    if (!ENV) {
+    if constexpr (!ENV) {
         for (int g = warp; g < TZ / 8; g += 8) {
             const int m0 = r0 + g * 8;
             fir8(xs + lane, xr0, hb, P.TpB, P.shiftB, m0, acc);
@@ -205,8 +205,7 @@ __global__ void __launch_bounds__(256) post_fir_kernel(const PostParams P) {
             for (int r = 0; r < 8; ++r)
                 if (m0 + r < P.nz && col < P.nx) P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = acc[r];
         }
-        return;
-    }
+    } else {
     for (int g = warp; g < YR / 8; g += 8) {
         const int m0 = yr0 + g * 8;
         fir8(xs + lane, xr0, hb, P.TpB, P.shiftB, m0, acc);
@@ -231,6 +230,7 @@ __global__ void __launch_bounds__(256) post_fir_kernel(const PostParams P) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
     if (lane == 0 && vmax > 0.0f) atomicMax(P.frame_max + f, __float_as_uint(vmax));
+    }
 }
 
 // a9: out = max(20 log10(env / M_frame), -DR); env = 0 or M = 0 gives -DR (A10).  In place.

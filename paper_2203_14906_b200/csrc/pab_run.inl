@@ -1,0 +1,179 @@
+// pab_run.inl -- included by pab_api.cu: batch driver and the two beamform entry points.
+
+namespace {
+
+template <typename T>
+void launch_ingest_quad(const void* rf, float* stage, int F, int N, int S, float scale, cudaStream_t st) {
+    const int nq = (F + 3) / 4;
+    dim3 grid((S + 1023) / 1024, N, nq);
+    ingest_quad_kernel<T><<<grid, 256, 0, st>>>((const T*)rf, (float4*)stage, F, N, S, scale);
+}
+template <typename T>
+void launch_ingest_lin(const void* rf, float* stage, int F, int N, int S, int Sp, float scale, cudaStream_t st) {
+    dim3 grid((Sp + 255) / 256, N, F);
+    ingest_lin_kernel<T><<<grid, 256, 0, st>>>((const T*)rf, stage, N, S, Sp, scale);
+}
+
+template <int K, int NQ>
+void launch_direct(const BfParams& P, int groups, cudaStream_t st) {
+    dim3 grid((P.nx + kDirectCols - 1) / kDirectCols, (P.nz + kDirectRows - 1) / kDirectRows, groups);
+    bf_direct_kernel<K, NQ><<<grid, 256, 0, st>>>(P);
+}
+
+template <int NQ>
+void launch_direct_order(int order, const BfParams& P, int groups, cudaStream_t st) {
+    switch (order) {
+    case 1: launch_direct<1, NQ>(P, groups, st); break;
+    case 2: launch_direct<2, NQ>(P, groups, st); break;
+    case 3: launch_direct<3, NQ>(P, groups, st); break;
+    case 4: launch_direct<4, NQ>(P, groups, st); break;
+    default: launch_direct<5, NQ>(P, groups, st); break;
+    }
+}
+
+// One batch (<= plan.batch_frames frames): ingest -> beamform -> post.  rf points at the batch's first frame
+// in the caller's layout, out at the batch's first image.
+int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaStream_t st) {
+    const int N = ctx->N, S = ctx->S, nx = ctx->grid.nx, nz = ctx->grid.nz;
+    const bool post = ctx->post_mode != PAB_RAW;
+    BfParams P{};
+    P.xj = ctx->d_xj; P.xe = ctx->d_xe; P.zrow = ctx->d_zrow;
+    P.N = N; P.S = S; P.Sp = ctx->Sp; P.nx = nx; P.nz = nz;
+    P.out = post ? ctx->d_img : out;
+    const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
+                            (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0 && staged_available());
+
+    if (F < 4) {
+        // lin layout, one frame per thread.  fp32 input with unit scale and 16-byte rows is read in place.
+        const bool in_place = ctx->dtype == PAB_F32 && ctx->scale == 1.0f && (S % 4) == 0 &&
+                              ((uintptr_t)rf % 16) == 0;
+        if (in_place) {
+            P.rf = (const float*)rf;
+        } else {
+            if (ctx->dtype == PAB_I16) launch_ingest_lin<int16_t>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
+            else launch_ingest_lin<float>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
+            ctx->launches++;
+            P.rf = ctx->d_stage;
+        }
+        P.n_frames = F;
+        if (use_staged) launch_staged(order, 0, P, F, ctx->plan, st);
+        else launch_direct_order<0>(order, P, F, st);
+        ctx->launches++;
+    } else {
+        if (ctx->dtype == PAB_I16) launch_ingest_quad<int16_t>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
+        else launch_ingest_quad<float>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
+        ctx->launches++;
+        const int nq = (F + 3) / 4;
+        const int n_oct = ctx->plan.frames_per_thread >= 8 ? nq / 2 : 0;   // groups of 2 quads
+        P.rf = ctx->d_stage;
+        P.n_frames = F;
+        if (n_oct > 0) {
+            if (use_staged) launch_staged(order, 2, P, n_oct, ctx->plan, st);
+            else launch_direct_order<2>(order, P, n_oct, st);
+            ctx->launches++;
+        }
+        const int rem_q = nq - 2 * n_oct;       // 0 or 1 quad left (or all quads when frames_per_thread = 4)
+        if (rem_q > 0) {
+            BfParams R = P;
+            R.rf = ctx->d_stage + (size_t)(2 * n_oct) * N * (size_t)S * 4;
+            R.out = P.out + (size_t)(8 * n_oct) * nz * (size_t)nx;
+            R.n_frames = F - 8 * n_oct;
+            if (use_staged) launch_staged(order, 1, R, rem_q, ctx->plan, st);
+            else launch_direct_order<1>(order, R, rem_q, st);
+            ctx->launches++;
+        }
+    }
+    if (post) {
+        PostParams Q{};
+        Q.x = ctx->d_img; Q.out = out; Q.frame_max = ctx->d_max;
+        Q.taps_bp = ctx->d_taps_bp; Q.taps_h = ctx->d_taps_h;
+        Q.TpB = ctx->TpB; Q.shiftB = ctx->n_taps_bp / 2;
+        Q.TpH = ctx->TpH; Q.shiftH = (ctx->n_taps_h - 1) / 2;
+        Q.nx = nx; Q.nz = nz;
+        constexpr int TZ = 128;
+        dim3 grid((nx + 31) / 32, (nz + TZ - 1) / TZ, F);
+        if (ctx->post_mode == PAB_BANDPASS) {
+            const size_t sm = ((size_t)(TZ + Q.TpB - 1) * 32 + Q.TpB + Q.TpH) * 4;
+            post_fir_kernel<TZ, false><<<grid, 256, sm, st>>>(Q);
+            ctx->launches++;
+        } else {
+            const int YR = (TZ + Q.TpH - 1 + 7) & ~7;
+            const size_t sm = ((size_t)(YR + Q.TpB - 1) * 32 + (size_t)YR * 32 + Q.TpB + Q.TpH) * 4;
+            cudaMemsetAsync(ctx->d_max, 0, (size_t)F * 4, st);
+            post_fir_kernel<TZ, true><<<grid, 256, sm, st>>>(Q);
+            ctx->launches++;
+            if (ctx->post_mode == PAB_LOG) {
+                dim3 g2((nx * nz + 1023) / 1024, F);
+                post_log_kernel<<<g2, 256, 0, st>>>(out, ctx->d_max, nx * nz, ctx->dyn_range_db);
+                ctx->launches++;
+            }
+        }
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "kernel launch");
+    return PAB_OK;
+}
+
+int check_args(pab_ctx* ctx, const void* rf, int n_frames, int order, const float* out) {
+    if (!ctx || !rf || !out || n_frames < 1 || order < 1 || order > 5) return PAB_ERR_INVALID;
+    if (((uintptr_t)rf % elem_size(ctx->dtype)) != 0 || ((uintptr_t)out % 4) != 0) return PAB_ERR_INVALID;
+    return PAB_OK;
+}
+
+}  // namespace
+
+extern "C" int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int order, float* out_dev, void* cuda_stream) {
+    int rc = check_args(ctx, rf_dev, n_frames, order, out_dev);
+    if (rc != PAB_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t frame_in = (size_t)ctx->N * ctx->S * elem_size(ctx->dtype);
+    const size_t frame_out = (size_t)ctx->grid.nz * ctx->grid.nx;
+    for (int f0 = 0; f0 < n_frames; f0 += ctx->plan.batch_frames) {
+        const int F = n_frames - f0 < ctx->plan.batch_frames ? n_frames - f0 : ctx->plan.batch_frames;
+        rc = run_batch(ctx, (const char*)rf_dev + (size_t)f0 * frame_in, F, order, out_dev + (size_t)f0 * frame_out, st);
+        if (rc != PAB_OK) return rc;
+    }
+    return PAB_OK;
+}
+
+extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host) {
+    int rc = check_args(ctx, rf_host, n_frames, order, out_host);
+    if (rc != PAB_OK) return rc;
+    const int B = ctx->plan.batch_frames;
+    const size_t frame_in = (size_t)ctx->N * ctx->S * elem_size(ctx->dtype);
+    const size_t frame_out = (size_t)ctx->grid.nz * ctx->grid.nx * 4;
+    if (!ctx->s_h2d) {
+        PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
+        PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_run, cudaStreamNonBlocking));
+        PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+        for (int b = 0; b < 2; ++b) {
+            PAB_CUDA(ctx, cudaMalloc(&ctx->d_in[b], (size_t)B * ctx->N * ctx->S * 4));   // sized for fp32
+            PAB_CUDA(ctx, cudaMalloc(&ctx->d_out[b], (size_t)B * frame_out));
+            PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_in[b], cudaEventDisableTiming));
+            PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_run[b], cudaEventDisableTiming));
+            PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_out[b], cudaEventDisableTiming));
+        }
+    }
+    // Double-buffered: H2D of batch b+1 and D2H of batch b-1 overlap the kernels of batch b.
+    int it = 0;
+    for (int f0 = 0; f0 < n_frames; f0 += B, ++it) {
+        const int F = n_frames - f0 < B ? n_frames - f0 : B;
+        const int b = it & 1;
+        if (it >= 2) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_run[b], 0));   // d_in[b] consumed
+        PAB_CUDA(ctx, cudaMemcpyAsync(ctx->d_in[b], (const char*)rf_host + (size_t)f0 * frame_in, (size_t)F * frame_in,
+                                      cudaMemcpyHostToDevice, ctx->s_h2d));
+        PAB_CUDA(ctx, cudaEventRecord(ctx->ev_in[b], ctx->s_h2d));
+        PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_run, ctx->ev_in[b], 0));
+        if (it >= 2) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_run, ctx->ev_out[b], 0));   // d_out[b] drained
+        rc = run_batch(ctx, ctx->d_in[b], F, order, ctx->d_out[b], ctx->s_run);
+        if (rc != PAB_OK) return rc;
+        PAB_CUDA(ctx, cudaEventRecord(ctx->ev_run[b], ctx->s_run));
+        PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_run[b], 0));
+        PAB_CUDA(ctx, cudaMemcpyAsync((char*)out_host + (size_t)f0 * frame_out, ctx->d_out[b], (size_t)F * frame_out,
+                                      cudaMemcpyDeviceToHost, ctx->s_d2h));
+        PAB_CUDA(ctx, cudaEventRecord(ctx->ev_out[b], ctx->s_d2h));
+    }
+    PAB_CUDA(ctx, cudaStreamSynchronize(ctx->s_d2h));
+    PAB_CUDA(ctx, cudaStreamSynchronize(ctx->s_run));
+    return PAB_OK;
+}

@@ -1,0 +1,256 @@
+// pab_staged.cuh -- the staged beamforming kernel: per pixel tile, the RF window every channel contributes
+// is brought into shared memory once by 1-D bulk async copies (TMA engine, cp.async.bulk, SASS UBLKCP)
+// issued by a producer warp, signalled through an mbarrier full/empty ring, and gathered from there by the
+// consumer warps (steps a1..a6 + a10 of DESIGN.md).
+//
+// Tile = 64 rows x 8 columns, 16 consumer warps (one column and 32 consecutive rows each: lanes along
+// depth, so a warp's gathers from one channel are <= ~1 sample apart per lane, bank-conflict free in the
+// quad layout) + 1 producer warp whose lanes each own one channel of the current chunk.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/pab.h"
+#include "pab_kernels.cuh"
+
+namespace pab {
+
+constexpr int kStgRows = 64, kStgCols = 8, kStgConsumerWarps = 16;
+constexpr int kStgThreads = (kStgConsumerWarps + 1) * 32;
+constexpr int kStgMaxStages = 4;
+
+// per staged channel: what a consumer needs besides the samples (32 bytes, read as two 128-bit broadcasts)
+struct __align__(16) ChanEntry {
+    float xe_hi, xe_lo;     // element position in samples
+    int base;               // byte offset into the data area such that sample i lives at base + i * BPS
+    int w0;                 // first staged sample
+    int w1m2;               // last valid i0 (staged end - 2)
+    int pad0, pad1, pad2;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
+struct StagedCfg {
+    int chunk;          // channels per stage (<= 32)
+    int stages;         // ring depth
+    int window;         // samples per channel slot per quad (multiple of 4)
+};
+
+// NQ = 0: lin layout, one frame per thread; NQ = 1, 2: quad layout, 4 NQ frames per thread.
+// grid: (ceil(nx/8), ceil(nz/64), groups)
+template <int K, int NQ>
+__global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParams P, const StagedCfg C) {
+    constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
+    constexpr int BPS = NQ == 0 ? 4 : 16;              // bytes per staged sample
+    constexpr int NCOPY = NQ == 0 ? 1 : NQ;            // bulk copies per channel
+    extern __shared__ __align__(128) unsigned char stg_smem[];
+    unsigned char* smem = stg_smem;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                 // full[stages], empty[stages]
+    ChanEntry* tab = reinterpret_cast<ChanEntry*>(smem + 64);           // [stages][chunk]
+    const int tab_bytes = (C.stages * C.chunk * (int)sizeof(ChanEntry) + 127) & ~127;
+    const uint32_t data0 = smem_u32(smem + 64 + tab_bytes);
+    const int slot_bytes = C.window * BPS * NCOPY;
+    const int stage_bytes = C.chunk * slot_bytes;
+    const uint32_t bar0 = smem_u32(bars);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int c0 = blockIdx.x * kStgCols, r0 = blockIdx.y * kStgRows;
+    const int n_chunks = (P.N + C.chunk - 1) / C.chunk;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C.stages; ++s) {
+            mbar_init(bar0 + 8 * s, C.chunk);                               // full: one arrival per producer lane
+            mbar_init(bar0 + 8 * (C.stages + s), kStgConsumerWarps);        // empty: one arrival per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == kStgConsumerWarps) {
+        // ---------------- producer warp: lane l stages channel (chunk * C.chunk + l) ----------------
+        if (lane >= C.chunk) return;
+        const int rl = min(r0 + kStgRows - 1, P.nz - 1), cl = min(c0 + kStgCols - 1, P.nx - 1);
+        const float4 zf = P.zrow[r0], zl = P.zrow[rl];
+        const float2 xa = P.xj[c0], xb = P.xj[cl];
+        const size_t chan_stride = NQ == 0 ? (size_t)P.Sp * 4 : (size_t)P.S * 16;        // bytes
+        const size_t grp_stride = (size_t)P.N * chan_stride;                              // one frame / one quad
+        const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)blockIdx.z * (NQ == 0 ? 1 : NQ) * grp_stride;
+        const int row_len = NQ == 0 ? P.Sp : P.S;
+        for (int ck = 0; ck < n_chunks; ++ck) {
+            const int s = ck % C.stages;
+            const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
+            mbar_wait(empty, ((ck / C.stages) & 1) ^ 1);
+            const int ch = ck * C.chunk + lane;
+            if (ch >= P.N) { mbar_arrive(full); continue; }
+            const float2 xe = __ldg(P.xe + ch);
+            const float xlo = (xa.x - xe.x) + (xa.y - xe.y), xhi = (xb.x - xe.x) + (xb.y - xe.y);
+            const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
+            const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
+            const float imin = fminf(sqrtf(fmaf(amin, amin, zf.y)), 2.0e6f);
+            const float imax = fminf(sqrtf(fmaf(amax, amax, zl.y)), 2.0e6f);
+            int w0 = max((int)floorf(imin) - 1, 0) & ~3;
+            int w1 = (int)floorf(imax) + 3;
+            if (NQ == 0) {
+                w1 = (w1 + 3) & ~3;
+                w0 = min(w0, row_len - 4);
+                w1 = min(max(w1, w0 + 4), row_len);
+            } else {
+                w0 = min(w0, (row_len - 2) & ~3);
+                w1 = min(max(w1, w0 + 2), row_len);
+            }
+            w1 = min(w1, w0 + C.window);
+            const int len = w1 - w0;
+            const int slot = s * stage_bytes + lane * slot_bytes;
+            ChanEntry e;
+            e.xe_hi = xe.x; e.xe_lo = xe.y;
+            e.base = slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
+            e.pad0 = e.pad1 = e.pad2 = 0;
+            tab[s * C.chunk + lane] = e;
+            const uint32_t bytes = (uint32_t)len * BPS;
+            mbar_arrive_expect_tx(full, bytes * NCOPY);
+            const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
+#pragma unroll
+            for (int q = 0; q < NCOPY; ++q)
+                bulk_g2s(data0 + slot + q * C.window * BPS, src + q * grp_stride, bytes, full);
+        }
+        return;
+    }
+
+    // ---------------- consumer warps ----------------
+    const int j = c0 + (warp & 7);
+    const int m = r0 + (warp >> 3) * 32 + lane;
+    const float2 xj = P.xj[min(j, P.nx - 1)];
+    const float4 row = P.zrow[min(m, P.nz - 1)];
+    float p[NF][K];
+#pragma unroll
+    for (int f = 0; f < NF; ++f)
+#pragma unroll
+        for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+
+    for (int ck = 0; ck < n_chunks; ++ck) {
+        const int s = ck % C.stages;
+        mbar_wait(bar0 + 8 * s, (ck / C.stages) & 1);
+        const int nch = min(C.chunk, P.N - ck * C.chunk);
+        const uint32_t tab_s = smem_u32(tab + s * C.chunk);
+#pragma unroll 2
+        for (int l = 0; l < nch; ++l) {
+            const float4 e0 = lds128(tab_s + l * 32);          // xe_hi, xe_lo, base, w0
+            const float e1 = lds32(tab_s + l * 32 + 16);       // w1m2
+            const Tap t = delay_tap((xj.x - e0.x) + (xj.y - e0.y), row, P.S);
+            const int i0 = min(max(t.i0, __float_as_int(e0.w)), __float_as_int(e1));
+            const uint32_t a = data0 + __float_as_int(e0.z) + i0 * BPS;
+            if constexpr (NQ == 0) {
+                const float s0 = lds32(a), s1 = lds32(a + 4);
+                accumulate<K>(fmaf(t.wa, s1, t.wb * s0), p[0]);
+            } else {
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    const float4 s0 = lds128(a + q * C.window * 16);
+                    const float4 s1 = lds128(a + q * C.window * 16 + 16);
+                    accumulate<K>(fmaf(t.wa, s1.x, t.wb * s0.x), p[4 * q + 0]);
+                    accumulate<K>(fmaf(t.wa, s1.y, t.wb * s0.y), p[4 * q + 1]);
+                    accumulate<K>(fmaf(t.wa, s1.z, t.wb * s0.z), p[4 * q + 2]);
+                    accumulate<K>(fmaf(t.wa, s1.w, t.wb * s0.w), p[4 * q + 3]);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar0 + 8 * (C.stages + s));
+    }
+
+    if (j < P.nx && m < P.nz) {
+        const size_t img = (size_t)P.nz * P.nx;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            const int frame = blockIdx.z * NF + f;
+            if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+        }
+    }
+}
+
+// ---- host side ----
+template <int K, int NQ>
+inline cudaError_t staged_set_attr(int smem_optin) {
+    return cudaFuncSetAttribute(bf_staged_kernel<K, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+}
+template <int NQ>
+inline cudaError_t staged_set_attr_orders(int smem_optin) {
+    cudaError_t e;
+    if ((e = staged_set_attr<1, NQ>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<2, NQ>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<3, NQ>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<4, NQ>(smem_optin)) != cudaSuccess) return e;
+    return staged_set_attr<5, NQ>(smem_optin);
+}
+inline int staged_configure(int smem_optin) {
+    if (staged_set_attr_orders<0>(smem_optin) != cudaSuccess) return PAB_ERR_CUDA;
+    if (staged_set_attr_orders<1>(smem_optin) != cudaSuccess) return PAB_ERR_CUDA;
+    if (staged_set_attr_orders<2>(smem_optin) != cudaSuccess) return PAB_ERR_CUDA;
+    return PAB_OK;
+}
+inline bool staged_available() { return true; }
+
+// Shared-memory plan of one launch: the plan's chunk is sized for 2 quads per channel; with fewer bytes per
+// sample the same chunk fits with room to spare.
+inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
+    const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
+    const size_t tab = ((size_t)c.stages * c.chunk * sizeof(ChanEntry) + 127) & ~(size_t)127;
+    return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy;
+}
+
+template <int K, int NQ>
+inline void launch_staged_k(const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
+    dim3 grid((P.nx + kStgCols - 1) / kStgCols, (P.nz + kStgRows - 1) / kStgRows, groups);
+    bf_staged_kernel<K, NQ><<<grid, kStgThreads, staged_smem_bytes(c, NQ), st>>>(P, c);
+}
+template <int NQ>
+inline void launch_staged_nq(int order, const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
+    switch (order) {
+    case 1: launch_staged_k<1, NQ>(P, groups, c, st); break;
+    case 2: launch_staged_k<2, NQ>(P, groups, c, st); break;
+    case 3: launch_staged_k<3, NQ>(P, groups, c, st); break;
+    case 4: launch_staged_k<4, NQ>(P, groups, c, st); break;
+    default: launch_staged_k<5, NQ>(P, groups, c, st); break;
+    }
+}
+inline void launch_staged(int order, int nq, const BfParams& P, int groups, const pab_plan_info& plan, cudaStream_t st) {
+    StagedCfg c{plan.chunk_channels, plan.stages, plan.window_samples};
+    if (nq == 0) launch_staged_nq<0>(order, P, groups, c, st);
+    else if (nq == 1) launch_staged_nq<1>(order, P, groups, c, st);
+    else launch_staged_nq<2>(order, P, groups, c, st);
+}
+
+}  // namespace pab
