@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's measurement contract for the DMAS-k hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+One step = one pass of the whole hot path (ingest, delay, interpolated gather,
+signed root, power sums, Newton combination, axial band-pass, Hilbert-FIR envelope, log compression, frame
+batching) over one batch of 64 synthetic frames of the headline workload C2b (BASELINE.json north_star:
+128 elements x 2048 samples x 1024x256 pixels, order 3, batched frames), through the C ABI (pab_beamform).
+`value` = frames/s with the RF already resident in HBM; `e2e` = the same through pab_beamform_host with host
+buffers (pinned), H2D and D2H inside the timed region.  Rank 0 prints ONE JSON line.
+
+Multi-GPU: frames are independent, the path has no exchange step: replicas only, one context per GPU, each
+rank runs its own 64-frame batch ("scaling": "weak"), no data-path collective; max-over-ranks timing.
+
+--impl reference times the fp64 CPU oracle (oracle/) as it stands on the host cores, on a bounded sample of
+the same workload (this tier's reference arm); rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+ORDER = 3
+FRAMES = 64
+WORKLOAD = "C2b"
+POST = dict(mode="log", f_center=10e6, f_halfwidth=2.5e6, n_taps_bp=64, n_taps_hilbert=63, dyn_range_db=60.0)
+N_SETS = 4          # rotating input/output buffer sets: 4 x (64 MiB RF + 64 MiB image) = 512 MiB > 126 MB L2
+METRIC = "beamformed frames/s, order-3 DMAS, 128ch (C2b: 128 el x 2048 samp x 1024x256 px, 64-frame batches, " \
+         "band-pass + envelope + log)"
+
+# Algorithmic work per item (pixel x element x frame) of the fused beamforming kernel at order 3, DESIGN.md
+# "Roofline": XU (MUFU) lane-ops = 2 (lg2 + ex2 of the cube root) + 1/64 (the delay sqrt, shared by the 64
+# frames of a batch); FP32-pipe slots = 6 + 3/64; HBM bytes = RF in + image out, once.
+XU_PER_ITEM = 2.0 + 1.0 / FRAMES
+FP32_PER_ITEM = 6.0 + 3.0 / FRAMES
+SM_COUNT = 148
+XU_LANES_PER_CLK_SM = 16
+FP32_LANES_PER_CLK_SM = 128
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.t.join(timeout=2)
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": float(max(power))}
+
+
+def make_inputs(n_frames: int, seed_offset: int = 0):
+    """Seeded synthetic C2b frames (paper_2203_14906_b200/synth.py)."""
+    from paper_2203_14906_b200 import synth
+    w = synth.make_config(WORKLOAD, seed=1012 + seed_offset, n_frames=n_frames)
+    return w.geom, w.rf
+
+
+def oracle_step(orc, rf, g, nthreads=0):
+    """The oracle's whole path on rf [F][N][S]: fp64 beamform (route B) + band-pass + envelope + log."""
+    img, used = orc.beamform(rf, g, ORDER, nthreads=nthreads, return_threads=True)
+    orc.post(img, g, POST["f_center"], POST["f_halfwidth"], POST["n_taps_bp"], POST["n_taps_hilbert"],
+             POST["dyn_range_db"], mode="log")
+    return used
+
+
+def time_oracle(n_frames: int, steps: int, warmup: int):
+    """frames/s of the oracle as it stands on the host cores; each step = n_frames frames of the C2b workload."""
+    import oracle as orc
+    orc.build()
+    g, rf = make_inputs(n_frames)
+    used = 1
+    for _ in range(warmup):
+        used = oracle_step(orc, rf, g)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        used = oracle_step(orc, rf, g)
+    dt = time.perf_counter() - t0
+    return n_frames * steps / dt, dt / steps * 1e3, used
+
+
+def run_reference(args, rank: int):
+    if rank != 0:
+        return
+    sample_frames = 2
+    fps, ms, cores = time_oracle(sample_frames, args.steps, args.warmup)
+    sample = f"{sample_frames} frames of C2b per step (of the 64-frame batch), fp64 route B + post chain, OpenMP"
+    line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD + "+post", "order": ORDER, "frames_per_step": sample_frames,
+                       "n_elem": 128, "n_samp": 2048, "nz": 1024, "nx": 256},
+            "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank: int, local_rank: int, world: int):
+    import torch
+    import torch.distributed as dist
+    from paper_2203_14906_b200 import binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    binding.load()                                  # raises when libpab.so is missing
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    g, rf_np = make_inputs(FRAMES, seed_offset=rank)
+    rf_host = torch.from_numpy(rf_np).pin_memory()
+    rf_sets = [torch.roll(rf_host, r, 0).to(dev) for r in range(N_SETS)]
+    out_sets = [torch.empty((FRAMES, g.nz, g.nx), dtype=torch.float32, device=dev) for _ in range(N_SETS)]
+    out_host = torch.empty((FRAMES, g.nz, g.nx), dtype=torch.float32).pin_memory()
+    bf = binding.Beamformer(g, post=POST)
+    stream = torch.cuda.current_stream(dev)
+    items_per_frame = g.nz * g.nx * g.n_elem
+    K, W = args.steps, max(args.warmup, 3)
+
+    def step(i):
+        bf.beamform(rf_sets[i % N_SETS], ORDER, out=out_sets[i % N_SETS], stream=stream)
+
+    # ---- device-resident throughput: K steps in one timed region, barrier + synchronize on both sides ----
+    for i in range(W):
+        step(i)
+    barrier()
+    bf.set_profile(8 * K + 8)
+    clocks = ClockSampler(local_rank)
+    if rank == 0:
+        clocks.start()
+        time.sleep(0.3)
+    barrier()
+    n0 = bf.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(K):
+        step(W + i)
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = bf.launch_count() - n0
+    prof = bf.get_profile(reset=True)
+    bf.set_profile(0)
+    clk = clocks.stop() if rank == 0 else None
+
+    # ---- end to end: pab_beamform_host, pinned host buffers, H2D + D2H inside the timed region ----
+    Ke = max(3, min(K, 10))
+    for _ in range(2):
+        bf.beamform_host(rf_host, ORDER, out=out_host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        bf.beamform_host(rf_host, ORDER, out=out_host)      # returns after the last D2H has finished
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    checksum = float(out_host[0, 512, 128])
+
+    # ---- beamform-only (raw output) throughput, for the stage breakdown ----
+    bf_raw = binding.Beamformer(g)
+    for i in range(3):
+        bf_raw.beamform(rf_sets[i % N_SETS], ORDER, out=out_sets[i % N_SETS], stream=stream)
+    torch.cuda.synchronize()
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    r0.record(stream)
+    for i in range(K):
+        bf_raw.beamform(rf_sets[i % N_SETS], ORDER, out=out_sets[i % N_SETS], stream=stream)
+    r1.record(stream)
+    torch.cuda.synchronize()
+    raw_ms = r0.elapsed_time(r1) / K
+    bf_raw.close()
+
+    t = torch.tensor([ms_total, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, e2e_ms = float(t[0]), float(t[1])
+    if rank == 0:
+        peaks = read_peaks()
+        ms_step = ms_total / K
+        fps = world * FRAMES * K / (ms_total * 1e-3)
+        bf_ms, bf_n = prof["beamform"]
+        bf_launch_ms = bf_ms / max(bf_n, 1)
+        frames_per_launch = FRAMES * K / max(bf_n, 1)
+        items_per_launch = items_per_frame * frames_per_launch
+        f_hz = peaks["sm_max_mhz"] * 1e6
+        xu_peak = SM_COUNT * XU_LANES_PER_CLK_SM * f_hz
+        fp32_peak = SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz
+        hbm_bytes = frames_per_launch * (g.n_elem * g.n_samp * 4 + g.nz * g.nx * 4)
+        t_xu = items_per_launch * XU_PER_ITEM / xu_peak
+        t_fp32 = items_per_launch * FP32_PER_ITEM / fp32_peak
+        t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
+        achieved = items_per_launch * XU_PER_ITEM / (bf_launch_ms * 1e-3)
+        roofline = {"bound": "alu", "kernel": "bf_staged_kernel<3,2> (fused delay+interp+root+power sums+Newton)",
+                    "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
+                    "frac": achieved / xu_peak, "traffic": None,
+                    "peak_source": f"148 SM x 16 XU lanes/clk x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, "
+                                   f"{peaks['source']}); DESIGN.md Roofline",
+                    "launch_ms": bf_launch_ms, "launches_timed": bf_n,
+                    "t_roof_ms": {"xu": t_xu * 1e3, "fp32": t_fp32 * 1e3, "hbm": t_hbm * 1e3},
+                    "algorithmic_per_item": {"xu_ops": XU_PER_ITEM, "fp32_slots": FP32_PER_ITEM,
+                                             "hbm_bytes": hbm_bytes / items_per_launch},
+                    "items_per_s": items_per_launch / (bf_launch_ms * 1e-3),
+                    "hbm_achieved_gbs": hbm_bytes / (bf_launch_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]}
+        stages = {k: {"ms_per_step": v[0] / K, "launches_per_step": v[1] / K} for k, v in prof.items()}
+        line = {"metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": WORKLOAD + "+post", "order": ORDER, "frames_per_step": FRAMES,
+                           "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx, "post": "log",
+                           "parallelism": f"replicas x{world}, no collective",
+                           "l2": f"inputs/outputs rotate over {N_SETS} buffer sets (512 MiB) > 126 MB L2"},
+                "items_per_s": fps * items_per_frame,
+                "e2e": {"value": world * FRAMES * Ke / (e2e_ms * 1e-3), "unit": "frames/s",
+                        "h2d_bytes_per_step": int(rf_host.numel() * 4), "d2h_bytes_per_step": int(out_host.numel() * 4),
+                        "ms_per_step": e2e_ms / Ke, "steps": Ke, "api": "pab_beamform_host (pinned host buffers)",
+                        "checksum": checksum},
+                "gpu_launches": int(launches), "clocks": clk, "roofline": roofline, "stages": stages,
+                "raw_only": {"ms_per_step": raw_ms, "frames_per_s": FRAMES / (raw_ms * 1e-3),
+                             "items_per_s": FRAMES * items_per_frame / (raw_ms * 1e-3)}}
+        if not args.no_cpu_baseline:
+            n_cpu = 16
+            cfps, cms, cores = time_oracle(n_cpu, 2, 0)
+            line["cpu_baseline"] = {"value": cfps, "unit": "frames/s", "cores": cores, "kind": "oracle",
+                                    "sample": f"2 passes over the first {n_cpu} frames of the step's 64-frame C2b batch, "
+                                              "fp64 route B + post chain"}
+        print(json.dumps(line), flush=True)
+    bf.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world != args.gpus and world == 1 and args.gpus > 1:
+        raise SystemExit("bench.py --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU)")
+    run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -150,6 +150,24 @@ int pab_design_hilbert(int half_len, float* g_host);
 /* pab_launch_count -- number of kernels this context has launched since it was created. */
 long long pab_launch_count(const pab_ctx* ctx);
 
+/* pipeline stages, for pab_get_profile */
+#define PAB_STAGE_INGEST   0   /* a1: int16/fp32 -> staged frame-interleaved fp32                                 */
+#define PAB_STAGE_BEAMFORM 1   /* a2..a6, a10: the fused delay + interpolate + power-sum + combination kernel     */
+#define PAB_STAGE_POST_FIR 2   /* a7, a8: axial band-pass + Hilbert-FIR envelope + per-frame max                  */
+#define PAB_STAGE_POST_LOG 3   /* a9: log compression                                                             */
+#define PAB_STAGE_COUNT    4
+
+/*
+ * pab_set_profile -- per-launch device timing for measurement: when max_launches > 0
+ * every kernel the context launches is bracketed by a pair of CUDA events recorded on the launching stream, up
+ * to max_launches launches (later ones are counted by pab_launch_count but not timed); 0 switches it off.
+ * Synchronises the device.  pab_get_profile sums the event durations of one stage since the last reset
+ * (waits for those launches to finish), returns the sum in milliseconds and the number of timed launches, and
+ * with reset != 0 forgets every recorded launch of every stage (read all stages first, reset on the last).
+ */
+int pab_set_profile(pab_ctx* ctx, int max_launches);
+int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset);
+
 /* pab_strerror -- static string for an error code.  pab_last_cuda_error -- the last cudaError_t string seen
  * by this context ("" if none). */
 const char* pab_strerror(int code);

@@ -16,13 +16,14 @@ OK, ERR_INVALID, ERR_DEVICE, ERR_ALLOC, ERR_CUDA = 0, -1, -2, -3, -4
 F32, I16 = 0, 1
 RAW, BANDPASS, ENVELOPE, LOG = 0, 1, 2, 3
 VARIANT_AUTO, VARIANT_DIRECT, VARIANT_STAGED = 0, 1, 2
+STAGES = ["ingest", "beamform", "post_fir", "post_log"]
 _MODES = {"raw": RAW, "bandpass": BANDPASS, "envelope": ENVELOPE, "log": LOG}
 _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_STAGED}
 
 # every symbol include/pab.h declares
 SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
-           "pab_launch_count", "pab_strerror", "pab_last_cuda_error", "pab_version"]
+           "pab_launch_count", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
 
 class Grid(C.Structure):
@@ -73,6 +74,8 @@ def load(build_if_missing: bool = False):
     L.pab_design_hilbert.argtypes = [ip, C.POINTER(C.c_float)]
     L.pab_launch_count.argtypes = [vp]
     L.pab_launch_count.restype = C.c_longlong
+    L.pab_set_profile.argtypes = [vp, ip]
+    L.pab_get_profile.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong), ip]
     L.pab_strerror.argtypes = [ip]
     L.pab_strerror.restype = C.c_char_p
     L.pab_last_cuda_error.argtypes = [vp]
@@ -160,6 +163,20 @@ class Beamformer:
 
     def launch_count(self) -> int:
         return int(self._L.pab_launch_count(self._h))
+
+    def set_profile(self, max_launches: int):
+        self._check(self._L.pab_set_profile(self._h, max_launches), "pab_set_profile")
+
+    def get_profile(self, reset: bool = True) -> dict:
+        """{stage: (total_ms, n_launches)} of the timed launches since the last reset."""
+        out = {}
+        for i, name in enumerate(STAGES):
+            ms, n = C.c_double(), C.c_longlong()
+            last = i == len(STAGES) - 1
+            self._check(self._L.pab_get_profile(self._h, i, C.byref(ms), C.byref(n), 1 if (reset and last) else 0),
+                        "pab_get_profile")
+            out[name] = (ms.value, n.value)
+        return out
 
     def beamform(self, rf, order: int, out=None, stream=None):
         """rf: CUDA tensor [F][N][S] float32 or int16 -> out: CUDA tensor [F][nz][nx] float32 (enqueue only)."""

@@ -40,6 +40,11 @@ struct pab_ctx {
     cudaStream_t s_h2d = nullptr, s_run = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_run[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
     long long launches = 0;
+    // per-launch device timing (pab_set_profile): events 2*slot, 2*slot+1 bracket launch `slot`
+    bool profiling = false;
+    std::vector<cudaEvent_t> prof_ev;
+    std::vector<int> prof_stage;
+    int prof_used = 0;
     char err[256] = {0};
 };
 
@@ -67,6 +72,8 @@ void free_all(pab_ctx* ctx) {
         if (ctx->ev_run[b]) cudaEventDestroy(ctx->ev_run[b]);
         if (ctx->ev_out[b]) cudaEventDestroy(ctx->ev_out[b]);
     }
+    for (cudaEvent_t e : ctx->prof_ev) cudaEventDestroy(e);
+    ctx->prof_ev.clear();
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_run) cudaStreamDestroy(ctx->s_run);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
@@ -170,6 +177,34 @@ void pab_destroy(pab_ctx* ctx) {
 int pab_set_input(pab_ctx* ctx, int dtype, float scale) {
     if (!ctx || (dtype != PAB_F32 && dtype != PAB_I16) || !(scale == scale) || scale == 0.0f) return PAB_ERR_INVALID;
     ctx->dtype = dtype; ctx->scale = scale;
+    return PAB_OK;
+}
+
+int pab_set_profile(pab_ctx* ctx, int max_launches) {
+    if (!ctx || max_launches < 0 || max_launches > (1 << 20)) return PAB_ERR_INVALID;
+    PAB_CUDA(ctx, cudaDeviceSynchronize());
+    for (cudaEvent_t e : ctx->prof_ev) cudaEventDestroy(e);
+    ctx->prof_ev.clear(); ctx->prof_stage.clear(); ctx->prof_used = 0;
+    ctx->profiling = max_launches > 0;
+    if (!ctx->profiling) return PAB_OK;
+    ctx->prof_ev.resize((size_t)2 * max_launches, nullptr);
+    ctx->prof_stage.assign(max_launches, 0);
+    for (auto& e : ctx->prof_ev) PAB_CUDA(ctx, cudaEventCreate(&e));
+    return PAB_OK;
+}
+
+int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset) {
+    if (!ctx || stage < 0 || stage >= PAB_STAGE_COUNT || !total_ms || !n_launches) return PAB_ERR_INVALID;
+    double ms = 0.0; long long n = 0;
+    for (int s = 0; s < ctx->prof_used; ++s) {
+        if (ctx->prof_stage[s] != stage) continue;
+        PAB_CUDA(ctx, cudaEventSynchronize(ctx->prof_ev[2 * s + 1]));
+        float t = 0.0f;
+        PAB_CUDA(ctx, cudaEventElapsedTime(&t, ctx->prof_ev[2 * s], ctx->prof_ev[2 * s + 1]));
+        ms += t; ++n;
+    }
+    *total_ms = ms; *n_launches = n;
+    if (reset) ctx->prof_used = 0;
     return PAB_OK;
 }
 

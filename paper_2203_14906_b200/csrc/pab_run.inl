@@ -2,6 +2,22 @@
 
 namespace {
 
+// One kernel launch: counts it, and brackets it with CUDA events on its stream when profiling is on.
+struct Span {
+    pab_ctx* c; int stage; cudaStream_t st; int slot = -1;
+    Span(pab_ctx* c_, int stage_, cudaStream_t st_) : c(c_), stage(stage_), st(st_) {
+        if (c->profiling && c->prof_used < (int)c->prof_ev.size() / 2) {
+            slot = c->prof_used++;
+            c->prof_stage[slot] = stage;
+            cudaEventRecord(c->prof_ev[2 * slot], st);
+        }
+    }
+    ~Span() {
+        c->launches++;
+        if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], st);
+    }
+};
+
 template <typename T>
 void launch_ingest_quad(const void* rf, float* stage, int F, int N, int S, float scale, cudaStream_t st) {
     const int nq = (F + 3) / 4;
@@ -50,27 +66,33 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         if (in_place) {
             P.rf = (const float*)rf;
         } else {
-            if (ctx->dtype == PAB_I16) launch_ingest_lin<int16_t>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
-            else launch_ingest_lin<float>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
-            ctx->launches++;
+            {
+                Span sp(ctx, PAB_STAGE_INGEST, st);
+                if (ctx->dtype == PAB_I16) launch_ingest_lin<int16_t>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
+                else launch_ingest_lin<float>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
+            }
             P.rf = ctx->d_stage;
         }
         P.n_frames = F;
-        if (use_staged) launch_staged(order, 0, P, F, ctx->plan, st);
-        else launch_direct_order<0>(order, P, F, st);
-        ctx->launches++;
+        {
+            Span sp(ctx, PAB_STAGE_BEAMFORM, st);
+            if (use_staged) launch_staged(order, 0, P, F, ctx->plan, st);
+            else launch_direct_order<0>(order, P, F, st);
+        }
     } else {
-        if (ctx->dtype == PAB_I16) launch_ingest_quad<int16_t>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
-        else launch_ingest_quad<float>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
-        ctx->launches++;
+        {
+            Span sp(ctx, PAB_STAGE_INGEST, st);
+            if (ctx->dtype == PAB_I16) launch_ingest_quad<int16_t>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
+            else launch_ingest_quad<float>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
+        }
         const int nq = (F + 3) / 4;
         const int n_oct = ctx->plan.frames_per_thread >= 8 ? nq / 2 : 0;   // groups of 2 quads
         P.rf = ctx->d_stage;
         P.n_frames = F;
         if (n_oct > 0) {
+            Span sp(ctx, PAB_STAGE_BEAMFORM, st);
             if (use_staged) launch_staged(order, 2, P, n_oct, ctx->plan, st);
             else launch_direct_order<2>(order, P, n_oct, st);
-            ctx->launches++;
         }
         const int rem_q = nq - 2 * n_oct;       // 0 or 1 quad left (or all quads when frames_per_thread = 4)
         if (rem_q > 0) {
@@ -78,9 +100,9 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.rf = ctx->d_stage + (size_t)(2 * n_oct) * N * (size_t)S * 4;
             R.out = P.out + (size_t)(8 * n_oct) * nz * (size_t)nx;
             R.n_frames = F - 8 * n_oct;
+            Span sp(ctx, PAB_STAGE_BEAMFORM, st);
             if (use_staged) launch_staged(order, 1, R, rem_q, ctx->plan, st);
             else launch_direct_order<1>(order, R, rem_q, st);
-            ctx->launches++;
         }
     }
     if (post) {
@@ -94,18 +116,20 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         dim3 grid((nx + 31) / 32, (nz + TZ - 1) / TZ, F);
         if (ctx->post_mode == PAB_BANDPASS) {
             const size_t sm = ((size_t)(TZ + Q.TpB - 1) * 32 + Q.TpB + Q.TpH) * 4;
+            Span sp(ctx, PAB_STAGE_POST_FIR, st);
             post_fir_kernel<TZ, false><<<grid, 256, sm, st>>>(Q);
-            ctx->launches++;
         } else {
             const int YR = (TZ + Q.TpH - 1 + 7) & ~7;
             const size_t sm = ((size_t)(YR + Q.TpB - 1) * 32 + (size_t)YR * 32 + Q.TpB + Q.TpH) * 4;
             cudaMemsetAsync(ctx->d_max, 0, (size_t)F * 4, st);
-            post_fir_kernel<TZ, true><<<grid, 256, sm, st>>>(Q);
-            ctx->launches++;
+            {
+                Span sp(ctx, PAB_STAGE_POST_FIR, st);
+                post_fir_kernel<TZ, true><<<grid, 256, sm, st>>>(Q);
+            }
             if (ctx->post_mode == PAB_LOG) {
                 dim3 g2((nx * nz + 1023) / 1024, F);
+                Span sp(ctx, PAB_STAGE_POST_LOG, st);
                 post_log_kernel<<<g2, 256, 0, st>>>(out, ctx->d_max, nx * nz, ctx->dyn_range_db);
-                ctx->launches++;
             }
         }
     }
