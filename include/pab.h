@@ -64,8 +64,11 @@ typedef struct {
     int   chunk_channels;        /* channels staged per pipeline stage                                             */
     int   stages;                /* pipeline depth                                                                 */
     int   smem_bytes;            /* dynamic shared memory per block, bytes; 0 when the staged kernel does not fit  */
-    int   frames_per_thread;     /* frames each thread carries in registers when n_frames >= 4 (4 or 8)            */
+    int   frames_per_thread;     /* frames each thread carries in registers when enough frames are given (4, 8, 16)*/
     int   batch_frames;          /* internal frame batch per pass (ingest -> beamform -> post)                     */
+    int   in_range;              /* 1 when every (pixel, element) delay index lies inside the record and z0 is at
+                                    least one sample deep: the kernels then skip the out-of-record masks (A6)     */
+    int   reserved;
     double zs_per_row;           /* dz * fs / c : delay samples per pixel row                                      */
     double xs_per_col;           /* dx * fs / c : delay samples per pixel column at grazing incidence              */
 } pab_plan_info;
@@ -101,6 +104,11 @@ int pab_set_input(pab_ctx* ctx, int dtype, float scale);
  */
 int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz, int n_taps_bp,
                  int n_taps_hilbert, float dyn_range_db);
+
+/* pab_set_tuning -- override the plan's blocking (autotuning / experiments); 0 keeps the default of a field.
+ *   frames_per_thread 4, 8 or 16;  stages 2..4;  chunk_channels 1..32 (clamped to what fits in shared memory).
+ * Recomputes the plan (pab_get_plan shows the result).  Synchronises the device.  PAB_ERR_INVALID on bad values. */
+int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_channels);
 
 /* pab_set_variant -- force a beamforming kernel variant (testing / benchmarking).  PAB_ERR_INVALID when the
  * staged variant is requested but its plan does not fit in shared memory. */

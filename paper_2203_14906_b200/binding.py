@@ -21,7 +21,7 @@ _MODES = {"raw": RAW, "bandpass": BANDPASS, "envelope": ENVELOPE, "log": LOG}
 _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_STAGED}
 
 # every symbol include/pab.h declares
-SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_beamform", "pab_beamform_host",
+SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
            "pab_launch_count", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
@@ -34,7 +34,7 @@ class Grid(C.Structure):
 class PlanInfo(C.Structure):
     _fields_ = [("tile_z", C.c_int), ("tile_x", C.c_int), ("window_samples", C.c_int), ("chunk_channels", C.c_int),
                 ("stages", C.c_int), ("smem_bytes", C.c_int), ("frames_per_thread", C.c_int),
-                ("batch_frames", C.c_int), ("zs_per_row", C.c_double), ("xs_per_col", C.c_double)]
+                ("batch_frames", C.c_int), ("in_range", C.c_int), ("reserved", C.c_int), ("zs_per_row", C.c_double), ("xs_per_col", C.c_double)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -64,6 +64,7 @@ def load(build_if_missing: bool = False):
     L.pab_set_input.argtypes = [vp, ip, fp]
     L.pab_set_post.argtypes = [vp, ip, fp, fp, ip, ip, fp]
     L.pab_set_variant.argtypes = [vp, ip]
+    L.pab_set_tuning.argtypes = [vp, ip, ip, ip]
     L.pab_beamform.argtypes = [vp, vp, ip, ip, vp, vp]
     L.pab_beamform_host.argtypes = [vp, vp, ip, ip, vp]
     L.pab_destroy.argtypes = [vp]
@@ -155,6 +156,9 @@ class Beamformer:
 
     def set_variant(self, variant: str):
         self._check(self._L.pab_set_variant(self._h, _VARIANTS[variant]), "pab_set_variant")
+
+    def set_tuning(self, frames_per_thread: int = 0, stages: int = 0, chunk_channels: int = 0):
+        self._check(self._L.pab_set_tuning(self._h, frames_per_thread, stages, chunk_channels), "pab_set_tuning")
 
     def plan(self) -> dict:
         info = PlanInfo()

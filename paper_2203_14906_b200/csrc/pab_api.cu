@@ -23,6 +23,7 @@ struct pab_ctx {
     float dyn_range_db = 60.0f;
     int variant = PAB_VARIANT_AUTO;
     pab_plan_info plan{};
+    PlanTuning tuning{};
     int device = 0, sm_count = 0, smem_optin = 0;
     // device tables
     float2* d_xj = nullptr;
@@ -205,6 +206,19 @@ int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_laun
     }
     *total_ms = ms; *n_launches = n;
     if (reset) ctx->prof_used = 0;
+    return PAB_OK;
+}
+
+int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_channels) {
+    if (!ctx) return PAB_ERR_INVALID;
+    PlanTuning t;
+    t.frames_per_thread = frames_per_thread; t.stages = stages; t.chunk_channels = chunk_channels;
+    pab_plan_info plan;
+    if (!plan_geometry(ctx->N, ctx->S, ctx->fs, ctx->c, ctx->pitch, ctx->grid, ctx->smem_optin, &plan, t)) return PAB_ERR_INVALID;
+    PAB_CUDA(ctx, cudaDeviceSynchronize());
+    ctx->tuning = t;
+    ctx->plan = plan;
+    if (ctx->variant == PAB_VARIANT_STAGED && plan.smem_bytes == 0) ctx->variant = PAB_VARIANT_AUTO;
     return PAB_OK;
 }
 

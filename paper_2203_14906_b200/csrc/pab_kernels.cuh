@@ -22,7 +22,7 @@ struct BfParams {
     float* out;            // image of this launch's first frame
     const float2* xj;      // [nx]  pixel column x_j in samples (x fs / c), fp32 hi + lo
     const float2* xe;      // [N]   element x in samples, fp32 hi + lo
-    const float4* zrow;    // [nz]  (zs, zs^2, zf - 1/2, zi as int bits), zs = z fs / c = zi + zf
+    const float4* zrow;    // [nz]  (zs, zs^2, zf - 1/2, zi - 0x4B400000 as int bits), zs = z fs / c = zi + zf
     int N, S, Sp, nx, nz;
     int n_frames;          // valid frames in this launch (stores beyond are skipped)
 };
@@ -94,9 +94,10 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll 4
         for (int i = 0; i < P.N; ++i, chan += P.Sp) {
             const float2 xe = __ldg(P.xe + i);
-            const Tap t = delay_tap((xj.x - xe.x) + (xj.y - xe.y), row, P.S);
+            const float xs = (xj.x - xe.x) + (xj.y - xe.y);
+            const Tap t = delay_tap<false>(xs, xs * xs, row, P.S);
             const float s0 = __ldg(chan + t.i0), s1 = __ldg(chan + t.i0 + 1);
-            accumulate<K>(fmaf(t.wa, s1, t.wb * s0), p[0]);
+            accumulate<K>(interp<false>(t, s0, s1), p[0]);
         }
     } else {
         const size_t quad_stride = (size_t)P.N * (size_t)P.S;      // float4 units
@@ -104,15 +105,16 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll 2
         for (int i = 0; i < P.N; ++i, chan += P.S) {
             const float2 xe = __ldg(P.xe + i);
-            const Tap t = delay_tap((xj.x - xe.x) + (xj.y - xe.y), row, P.S);
+            const float xs = (xj.x - xe.x) + (xj.y - xe.y);
+            const Tap t = delay_tap<false>(xs, xs * xs, row, P.S);
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
                 const float4 s0 = __ldg(chan + q * quad_stride + t.i0);
                 const float4 s1 = __ldg(chan + q * quad_stride + t.i0 + 1);
-                accumulate<K>(fmaf(t.wa, s1.x, t.wb * s0.x), p[4 * q + 0]);
-                accumulate<K>(fmaf(t.wa, s1.y, t.wb * s0.y), p[4 * q + 1]);
-                accumulate<K>(fmaf(t.wa, s1.z, t.wb * s0.z), p[4 * q + 2]);
-                accumulate<K>(fmaf(t.wa, s1.w, t.wb * s0.w), p[4 * q + 3]);
+                accumulate<K>(interp<false>(t, s0.x, s1.x), p[4 * q + 0]);
+                accumulate<K>(interp<false>(t, s0.y, s1.y), p[4 * q + 1]);
+                accumulate<K>(interp<false>(t, s0.z, s1.z), p[4 * q + 2]);
+                accumulate<K>(interp<false>(t, s0.w, s1.w), p[4 * q + 3]);
             }
         }
     }

@@ -82,28 +82,51 @@ __device__ __forceinline__ float combine(const float (&p)[K]) {
 }
 
 // Step a2 + the index half of a3, once per (pixel, element), shared by every frame a thread carries.
-//   xs   lateral offset pixel - element in samples;  row: (zs, zs^2, zf - 1/2, zi) with zs = z fs / c = zi + zf
-//   idx = zs + xs^2 / (sqrt(xs^2 + zs^2) + zs)   (== fs sqrt(dx^2 + z^2) / c, without the
-//   cancellation and without one float carrying a 12-bit integer part: DESIGN.md "Delay index precision")
-// Returns i0 = floor(idx) clamped into [0, S-2]; wa, wb = interpolation weights of rf[i0+1], rf[i0]
-// (both 0 when the delayed sample falls outside the record: reading A6).
+//   xs   lateral offset pixel - element in samples, xs2 = xs^2
+//   row  (zs, zs^2, zf - 1/2, zi - 0x4B400000 as int bits) with zs = z fs / c = zi + zf, zi = floor(zs)
+//   idx = fs sqrt(dx^2 + z^2) / c = zs + delta, where delta >= 0 solves
+//         delta (delta + 2 zs) = xs^2.
+// One MUFU (rsqrt) gives d0 ~ sqrt(xs^2 + zs^2) to ~2 ulp; delta0 = d0 - zs then carries an absolute error of
+// ~ulp(d0), and one Newton step on f(delta) = delta (delta + 2 zs) - xs^2 (f' = 2 (delta + zs) ~ 2 d0, step
+// -f r / 2) squares it away in absolute terms: the result is good to ~1 ulp of delta, not of the 11-12 bit
+// index.  The integer part of zs never enters a float.
+// INR = true: the host has checked that every (pixel, element) index of the geometry lies inside the record
+// and z > 0, so no validity mask is produced and s = s0 + wa (s1 - s0).  INR = false: i0 is clamped into
+// [0, S-2] and wa, wb are both 0 when the delayed sample falls outside the record (reading A6).
 struct Tap { int i0; float wa, wb; };
 
-__device__ __forceinline__ Tap delay_tap(float xs, const float4 row, int S) {
-    const float xs2 = xs * xs;
-    const float d = sqrt_approx(fmaf(xs, xs, row.y));
-    const float delta = fminf(xs2 * rcp_approx(fmaxf(d + row.x, 1e-30f)), 2097152.0f);
+template <bool INR>
+__device__ __forceinline__ Tap delay_tap(float xs, float xs2, const float4 row, int S) {
+    float q = fmaf(xs, xs, row.y);
+    if constexpr (!INR) q = fmaxf(q, 1e-30f);
+    const float r = rsqrt_approx(q);
+    const float d0 = q * r;
+    const float delta0 = d0 - row.x;
+    const float f = fmaf(delta0, d0 + row.x, -xs2);
+    float delta = fmaf(-f, 0.5f * r, delta0);
+    if constexpr (!INR) delta = fminf(fmaxf(delta, 0.0f), 2097152.0f);
     const float w = row.z + delta;                              // idx - zi - 1/2  >= -1/2
     const float t = w + 12582912.0f;                            // round to nearest integer: floor(idx - zi)
     const float fl = t - 12582912.0f;
-    int i0 = __float_as_int(row.w) + (__float_as_int(t) - 0x4B400000);
-    float a = (w - fl) + 0.5f;
-    const bool ok = (i0 >= 0) && (i0 <= S - 2);
-    Tap r;
-    r.i0 = ok ? i0 : 0;
-    r.wa = ok ? a : 0.0f;
-    r.wb = ok ? 1.0f - a : 0.0f;
-    return r;
+    const int i0 = __float_as_int(row.w) + __float_as_int(t);   // zi + (int)fl
+    const float a = (w - fl) + 0.5f;
+    Tap o;
+    if constexpr (INR) {
+        o.i0 = i0; o.wa = a; o.wb = 0.0f;
+    } else {
+        const bool ok = (unsigned)i0 <= (unsigned)(S - 2);
+        o.i0 = ok ? i0 : 0;
+        o.wa = ok ? a : 0.0f;
+        o.wb = ok ? 1.0f - a : 0.0f;
+    }
+    return o;
+}
+
+// Step a3: the interpolated sample from its two neighbours.
+template <bool INR>
+__device__ __forceinline__ float interp(const Tap& t, float s0, float s1) {
+    if constexpr (INR) return fmaf(t.wa, s1 - s0, s0);
+    else return fmaf(t.wa, s1, t.wb * s0);
 }
 
 }  // namespace pab

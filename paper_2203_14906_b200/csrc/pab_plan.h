@@ -24,44 +24,67 @@ inline int window_bound(int tile_z, int tile_x, double zs_per_row, double xs_per
     return round_up((int)std::ceil(span) + 12, 4);
 }
 
+struct PlanTuning {
+    int frames_per_thread = 0;   // 4, 8 or 16; 0 = default
+    int stages = 0;              // 2..4; 0 = default
+    int chunk_channels = 0;      // 1..32; 0 = as many as fit
+};
+constexpr int kDefaultFramesPerThread = 16;
+
 inline bool plan_geometry(int n_elem, int n_samp, double fs, double c, double pitch, const pab_grid& g,
-                          int smem_limit, pab_plan_info* out) {
+                          int smem_limit, pab_plan_info* out, const PlanTuning& tune = PlanTuning()) {
     if (n_elem < 1 || n_samp < 2 || !(fs > 0) || !(c > 0) || !(pitch > 0)) return false;
     if (g.nx < 1 || g.nz < 1 || !(g.dx > 0) || !(g.dz > 0) || !(g.z0 >= 0)) return false;
+    if (tune.frames_per_thread != 0 && tune.frames_per_thread != 4 && tune.frames_per_thread != 8 &&
+        tune.frames_per_thread != 16) return false;
+    if (tune.stages != 0 && (tune.stages < 2 || tune.stages > 4)) return false;
+    if (tune.chunk_channels < 0 || tune.chunk_channels > kStagedMaxChunk) return false;
     if (smem_limit <= 0) smem_limit = kSmemOptin;
     pab_plan_info p{};
     p.tile_z = kStagedTileZ;
     p.tile_x = kStagedTileX;
     p.zs_per_row = (double)g.dz * fs / c;
     p.xs_per_col = (double)g.dx * fs / c;
-    p.frames_per_thread = 8;
+    p.frames_per_thread = tune.frames_per_thread ? tune.frames_per_thread : kDefaultFramesPerThread;
     double w = (p.tile_z - 1) * p.zs_per_row + (p.tile_x - 1) * p.xs_per_col;
     p.window_samples = w < 1e6 ? window_bound(p.tile_z, p.tile_x, p.zs_per_row, p.xs_per_col) : 1 << 20;
     if (p.window_samples > round_up(n_samp, 4)) p.window_samples = round_up(n_samp, 4);
-    // bytes of one channel slot at 8 frames per thread: window x 2 quads x 16 B, + its 32-byte table entry;
+    // bytes of one channel slot: window x (frames_per_thread / 4) quads x 16 B, + its 64-byte table entry;
     // 64 bytes of barriers and up to 128 bytes of table padding on top
-    const long long slot = (long long)p.window_samples * 32 + 32;
+    const int nq = p.frames_per_thread / 4;
+    const long long slot = (long long)p.window_samples * 16 * nq + 64;
     const int overhead = 64 + 128;
-    p.stages = 3;
+    p.stages = tune.stages ? tune.stages : 3;
     auto fit = [&](int stages) {
         long long ch = (smem_limit - overhead) / (stages * slot);
         if (ch > kStagedMaxChunk) ch = kStagedMaxChunk;
         if (ch > n_elem) ch = n_elem;
+        if (tune.chunk_channels && ch > tune.chunk_channels) ch = tune.chunk_channels;
         return (int)ch;
     };
     int chunk = fit(p.stages);
-    if (chunk < 4) { p.stages = 2; chunk = fit(p.stages); }
+    if (chunk < 4 && !tune.stages) { p.stages = 2; chunk = fit(p.stages); }
     if (chunk >= 1) {
         p.chunk_channels = chunk;
-        p.smem_bytes = 64 + round_up(p.stages * chunk * 32, 128) + p.stages * chunk * p.window_samples * 32;
+        p.smem_bytes = 64 + round_up(p.stages * chunk * 64, 128) + p.stages * chunk * p.window_samples * 16 * nq;
     } else {
         p.chunk_channels = 0; p.stages = 0; p.smem_bytes = 0;   // staged kernel does not fit: direct only
+    }
+    // every delay index of the geometry inside the record, and z > 0 (so the rsqrt argument is never 0)?
+    {
+        const double k = fs / c;
+        const double xe_max = ((double)n_elem - 1.0) / 2.0 * pitch;
+        const double xa = std::fabs((double)g.x0), xb = std::fabs((double)g.x0 + (g.nx - 1) * (double)g.dx);
+        const double ax = ((xa > xb ? xa : xb) + xe_max) * k;
+        const double zl = ((double)g.z0 + (g.nz - 1) * (double)g.dz) * k;
+        const double idx_max = std::sqrt(ax * ax + zl * zl);
+        p.in_range = (idx_max + 1.0 < (double)n_samp - 1.0) && ((double)g.z0 * k >= 1.0) ? 1 : 0;
     }
     // internal frame batch: keep one batch of staged RF well inside the 126 MB L2
     const double frame_bytes = (double)n_elem * n_samp * 4.0;
     int b = (int)(64.0 * 1048576.0 / frame_bytes);
-    b = b / 8 * 8;
-    if (b < 8) b = 8;
+    b = b / 16 * 16;
+    if (b < 16) b = 16;
     if (b > 64) b = 64;
     p.batch_frames = b;
     *out = p;
@@ -73,7 +96,7 @@ inline bool plan_geometry(int n_elem, int n_samp, double fs, double c, double pi
 struct DelayTables {
     std::vector<float> xj;     // [nx][2]
     std::vector<float> xe;     // [N][2]
-    std::vector<float> zrow;   // [nz][4]: zs, zs^2, zf - 1/2, zi (int bits)
+    std::vector<float> zrow;   // [nz][4]: zs, zs^2, zf - 1/2, zi - 0x4B400000 (int bits)
 };
 
 inline void split_hi_lo(double v, float* hi, float* lo) { *hi = (float)v; *lo = (float)(v - (double)*hi); }
@@ -91,7 +114,7 @@ inline DelayTables make_tables(int n_elem, double fs, double c, double pitch, co
         const double zs = ((double)g.z0 + m * (double)g.dz) * k;
         double zi = std::floor(zs);
         if (zi > 1.0e9) zi = 1.0e9;
-        const int32_t zii = (int32_t)zi;
+        const int32_t zii = (int32_t)zi - 0x4B400000;       // pre-biased: i0 = zii + bits(fl + 1.5 * 2^23)
         float zib;
         static_assert(sizeof(float) == sizeof(int32_t), "");
         __builtin_memcpy(&zib, &zii, 4);

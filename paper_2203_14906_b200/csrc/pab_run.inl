@@ -47,6 +47,12 @@ void launch_direct_order(int order, const BfParams& P, int groups, cudaStream_t 
     }
 }
 
+void launch_direct_nq(int order, int nq, const BfParams& P, int groups, cudaStream_t st) {
+    if (nq == 4) launch_direct_order<4>(order, P, groups, st);
+    else if (nq == 2) launch_direct_order<2>(order, P, groups, st);
+    else launch_direct_order<1>(order, P, groups, st);
+}
+
 // One batch (<= plan.batch_frames frames): ingest -> beamform -> post.  rf points at the batch's first frame
 // in the caller's layout, out at the batch's first image.
 int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaStream_t st) {
@@ -56,6 +62,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
     P.xj = ctx->d_xj; P.xe = ctx->d_xe; P.zrow = ctx->d_zrow;
     P.N = N; P.S = S; P.Sp = ctx->Sp; P.nx = nx; P.nz = nz;
     P.out = post ? ctx->d_img : out;
+    const bool in_range = ctx->plan.in_range != 0;
     const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
                             (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0 && staged_available());
 
@@ -76,7 +83,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         P.n_frames = F;
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, 0, P, F, ctx->plan, st);
+            if (use_staged) launch_staged(order, 0, in_range, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, st);
             else launch_direct_order<0>(order, P, F, st);
         }
     } else {
@@ -85,24 +92,23 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             if (ctx->dtype == PAB_I16) launch_ingest_quad<int16_t>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
             else launch_ingest_quad<float>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
         }
-        const int nq = (F + 3) / 4;
-        const int n_oct = ctx->plan.frames_per_thread >= 8 ? nq / 2 : 0;   // groups of 2 quads
-        P.rf = ctx->d_stage;
-        P.n_frames = F;
-        if (n_oct > 0) {
-            Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, 2, P, n_oct, ctx->plan, st);
-            else launch_direct_order<2>(order, P, n_oct, st);
-        }
-        const int rem_q = nq - 2 * n_oct;       // 0 or 1 quad left (or all quads when frames_per_thread = 4)
-        if (rem_q > 0) {
+        // quads are consumed in groups of frames_per_thread / 4, then the remainder in halves (4 -> 2 -> 1)
+        int nq = (F + 3) / 4, q0 = 0;
+        // orders 4 and 5 carry at most 8 frames per thread (16 x 5 accumulators would spill)
+        int g0 = ctx->plan.frames_per_thread / 4;
+        if (order >= 4 && g0 > 2) g0 = 2;
+        for (int g = g0; g >= 1 && nq > 0; g >>= 1) {
+            const int groups = nq / g;
+            if (groups == 0) continue;
             BfParams R = P;
-            R.rf = ctx->d_stage + (size_t)(2 * n_oct) * N * (size_t)S * 4;
-            R.out = P.out + (size_t)(8 * n_oct) * nz * (size_t)nx;
-            R.n_frames = F - 8 * n_oct;
+            R.rf = ctx->d_stage + (size_t)q0 * N * (size_t)S * 4;
+            R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
+            R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, 1, R, rem_q, ctx->plan, st);
-            else launch_direct_order<1>(order, R, rem_q, st);
+            if (use_staged) launch_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, st);
+            else launch_direct_nq(order, g, R, groups, st);
+            q0 += groups * g;
+            nq -= groups * g;
         }
     }
     if (post) {

@@ -18,14 +18,15 @@ constexpr int kStgRows = 64, kStgCols = 8, kStgConsumerWarps = 16;
 constexpr int kStgThreads = (kStgConsumerWarps + 1) * 32;
 constexpr int kStgMaxStages = 4;
 
-// per staged channel: what a consumer needs besides the samples (32 bytes, read as two 128-bit broadcasts)
+// per staged channel: what a consumer needs besides the samples (64 bytes; every read is a warp broadcast)
 struct __align__(16) ChanEntry {
-    float xe_hi, xe_lo;     // element position in samples
-    int base;               // byte offset into the data area such that sample i lives at base + i * BPS
+    float xs[8];            // pixel column c of the tile minus the element, in samples (hi + lo difference)
+    int base;               // shared-space address such that sample i of the first quad lives at base + i * BPS
     int w0;                 // first staged sample
     int w1m2;               // last valid i0 (staged end - 2)
-    int pad0, pad1, pad2;
+    int pad[5];
 };
+static_assert(sizeof(ChanEntry) == 64, "ChanEntry is 64 bytes");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -69,9 +70,10 @@ struct StagedCfg {
     int window;         // samples per channel slot per quad (multiple of 4)
 };
 
-// NQ = 0: lin layout, one frame per thread; NQ = 1, 2: quad layout, 4 NQ frames per thread.
+// NQ = 0: lin layout, one frame per thread; NQ = 1, 2, 4: quad layout, 4 NQ frames per thread.
+// INR: every delay index of the geometry lies inside the record (checked on the host): no masks, no clamps.
 // grid: (ceil(nx/8), ceil(nz/64), groups)
-template <int K, int NQ>
+template <int K, int NQ, bool INR>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParams P, const StagedCfg C) {
     constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
     constexpr int BPS = NQ == 0 ? 4 : 16;              // bytes per staged sample
@@ -82,7 +84,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
     ChanEntry* tab = reinterpret_cast<ChanEntry*>(smem + 64);           // [stages][chunk]
     const int tab_bytes = (C.stages * C.chunk * (int)sizeof(ChanEntry) + 127) & ~127;
     const uint32_t data0 = smem_u32(smem + 64 + tab_bytes);
-    const int slot_bytes = C.window * BPS * NCOPY;
+    const int quad_bytes = C.window * BPS;
+    const int slot_bytes = quad_bytes * NCOPY;
     const int stage_bytes = C.chunk * slot_bytes;
     const uint32_t bar0 = smem_u32(bars);
 
@@ -102,9 +105,11 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
     if (warp == kStgConsumerWarps) {
         // ---------------- producer warp: lane l stages channel (chunk * C.chunk + l) ----------------
         if (lane >= C.chunk) return;
-        const int rl = min(r0 + kStgRows - 1, P.nz - 1), cl = min(c0 + kStgCols - 1, P.nx - 1);
+        const int rl = min(r0 + kStgRows - 1, P.nz - 1);
         const float4 zf = P.zrow[r0], zl = P.zrow[rl];
-        const float2 xa = P.xj[c0], xb = P.xj[cl];
+        float2 xj[kStgCols];
+#pragma unroll
+        for (int c = 0; c < kStgCols; ++c) xj[c] = P.xj[min(c0 + c, P.nx - 1)];
         const size_t chan_stride = NQ == 0 ? (size_t)P.Sp * 4 : (size_t)P.S * 16;        // bytes
         const size_t grp_stride = (size_t)P.N * chan_stride;                              // one frame / one quad
         const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)blockIdx.z * (NQ == 0 ? 1 : NQ) * grp_stride;
@@ -116,7 +121,10 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
             const int ch = ck * C.chunk + lane;
             if (ch >= P.N) { mbar_arrive(full); continue; }
             const float2 xe = __ldg(P.xe + ch);
-            const float xlo = (xa.x - xe.x) + (xa.y - xe.y), xhi = (xb.x - xe.x) + (xb.y - xe.y);
+            ChanEntry e;
+#pragma unroll
+            for (int c = 0; c < kStgCols; ++c) e.xs[c] = (xj[c].x - xe.x) + (xj[c].y - xe.y);
+            const float xlo = e.xs[0], xhi = e.xs[kStgCols - 1];
             const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
             const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
             const float imin = fminf(sqrtf(fmaf(amin, amin, zf.y)), 2.0e6f);
@@ -134,25 +142,24 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
             w1 = min(w1, w0 + C.window);
             const int len = w1 - w0;
             const int slot = s * stage_bytes + lane * slot_bytes;
-            ChanEntry e;
-            e.xe_hi = xe.x; e.xe_lo = xe.y;
-            e.base = slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
-            e.pad0 = e.pad1 = e.pad2 = 0;
+            e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) e.pad[k] = 0;
             tab[s * C.chunk + lane] = e;
             const uint32_t bytes = (uint32_t)len * BPS;
             mbar_arrive_expect_tx(full, bytes * NCOPY);
             const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
 #pragma unroll
             for (int q = 0; q < NCOPY; ++q)
-                bulk_g2s(data0 + slot + q * C.window * BPS, src + q * grp_stride, bytes, full);
+                bulk_g2s(data0 + slot + q * quad_bytes, src + q * grp_stride, bytes, full);
         }
         return;
     }
 
     // ---------------- consumer warps ----------------
-    const int j = c0 + (warp & 7);
+    const int col = warp & 7;
+    const int j = c0 + col;
     const int m = r0 + (warp >> 3) * 32 + lane;
-    const float2 xj = P.xj[min(j, P.nx - 1)];
     const float4 row = P.zrow[min(m, P.nz - 1)];
     float p[NF][K];
 #pragma unroll
@@ -164,26 +171,31 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
         const int s = ck % C.stages;
         mbar_wait(bar0 + 8 * s, (ck / C.stages) & 1);
         const int nch = min(C.chunk, P.N - ck * C.chunk);
-        const uint32_t tab_s = smem_u32(tab + s * C.chunk);
+        const uint32_t tab_s = smem_u32(tab + s * C.chunk) + col * 4;
 #pragma unroll 2
         for (int l = 0; l < nch; ++l) {
-            const float4 e0 = lds128(tab_s + l * 32);          // xe_hi, xe_lo, base, w0
-            const float e1 = lds32(tab_s + l * 32 + 16);       // w1m2
-            const Tap t = delay_tap((xj.x - e0.x) + (xj.y - e0.y), row, P.S);
-            const int i0 = min(max(t.i0, __float_as_int(e0.w)), __float_as_int(e1));
-            const uint32_t a = data0 + __float_as_int(e0.z) + i0 * BPS;
+            const float xs = lds32(tab_s + l * 64);
+            const int base = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 32));
+            const Tap t = delay_tap<INR>(xs, xs * xs, row, P.S);
+            int i0 = t.i0;
+            if constexpr (!INR) {
+                const int w0 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 36));
+                const int w1m2 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 40));
+                i0 = min(max(i0, w0), w1m2);
+            }
+            const uint32_t a = (uint32_t)base + i0 * BPS;
             if constexpr (NQ == 0) {
                 const float s0 = lds32(a), s1 = lds32(a + 4);
-                accumulate<K>(fmaf(t.wa, s1, t.wb * s0), p[0]);
+                accumulate<K>(interp<INR>(t, s0, s1), p[0]);
             } else {
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) {
-                    const float4 s0 = lds128(a + q * C.window * 16);
-                    const float4 s1 = lds128(a + q * C.window * 16 + 16);
-                    accumulate<K>(fmaf(t.wa, s1.x, t.wb * s0.x), p[4 * q + 0]);
-                    accumulate<K>(fmaf(t.wa, s1.y, t.wb * s0.y), p[4 * q + 1]);
-                    accumulate<K>(fmaf(t.wa, s1.z, t.wb * s0.z), p[4 * q + 2]);
-                    accumulate<K>(fmaf(t.wa, s1.w, t.wb * s0.w), p[4 * q + 3]);
+                    const float4 s0 = lds128(a + q * quad_bytes);
+                    const float4 s1 = lds128(a + q * quad_bytes + 16);
+                    accumulate<K>(interp<INR>(t, s0.x, s1.x), p[4 * q + 0]);
+                    accumulate<K>(interp<INR>(t, s0.y, s1.y), p[4 * q + 1]);
+                    accumulate<K>(interp<INR>(t, s0.z, s1.z), p[4 * q + 2]);
+                    accumulate<K>(interp<INR>(t, s0.w, s1.w), p[4 * q + 3]);
                 }
             }
         }
@@ -202,55 +214,71 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
 }
 
 // ---- host side ----
-template <int K, int NQ>
+template <int K, int NQ, bool INR>
 inline cudaError_t staged_set_attr(int smem_optin) {
-    return cudaFuncSetAttribute(bf_staged_kernel<K, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    return cudaFuncSetAttribute(bf_staged_kernel<K, NQ, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
-template <int NQ>
+template <int NQ, bool INR>
 inline cudaError_t staged_set_attr_orders(int smem_optin) {
     cudaError_t e;
-    if ((e = staged_set_attr<1, NQ>(smem_optin)) != cudaSuccess) return e;
-    if ((e = staged_set_attr<2, NQ>(smem_optin)) != cudaSuccess) return e;
-    if ((e = staged_set_attr<3, NQ>(smem_optin)) != cudaSuccess) return e;
-    if ((e = staged_set_attr<4, NQ>(smem_optin)) != cudaSuccess) return e;
-    return staged_set_attr<5, NQ>(smem_optin);
+    if ((e = staged_set_attr<1, NQ, INR>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<2, NQ, INR>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<3, NQ, INR>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<4, NQ, INR>(smem_optin)) != cudaSuccess) return e;
+    return staged_set_attr<5, NQ, INR>(smem_optin);
+}
+template <bool INR>
+inline bool staged_configure_inr(int smem_optin) {
+    return staged_set_attr_orders<0, INR>(smem_optin) == cudaSuccess && staged_set_attr_orders<1, INR>(smem_optin) == cudaSuccess &&
+           staged_set_attr_orders<2, INR>(smem_optin) == cudaSuccess && staged_set_attr_orders<4, INR>(smem_optin) == cudaSuccess;
 }
 inline int staged_configure(int smem_optin) {
-    if (staged_set_attr_orders<0>(smem_optin) != cudaSuccess) return PAB_ERR_CUDA;
-    if (staged_set_attr_orders<1>(smem_optin) != cudaSuccess) return PAB_ERR_CUDA;
-    if (staged_set_attr_orders<2>(smem_optin) != cudaSuccess) return PAB_ERR_CUDA;
-    return PAB_OK;
+    return staged_configure_inr<false>(smem_optin) && staged_configure_inr<true>(smem_optin) ? PAB_OK : PAB_ERR_CUDA;
 }
 inline bool staged_available() { return true; }
 
-// Shared-memory plan of one launch: the plan's chunk is sized for 2 quads per channel; with fewer bytes per
-// sample the same chunk fits with room to spare.
+// Shared-memory bytes of one launch: the plan's chunk is sized for `frames_per_thread / 4` quads per channel;
+// with fewer bytes per sample the same chunk fits with room to spare.
 inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
     const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
     const size_t tab = ((size_t)c.stages * c.chunk * sizeof(ChanEntry) + 127) & ~(size_t)127;
     return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy;
 }
 
-template <int K, int NQ>
+template <int K, int NQ, bool INR>
 inline void launch_staged_k(const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
     dim3 grid((P.nx + kStgCols - 1) / kStgCols, (P.nz + kStgRows - 1) / kStgRows, groups);
-    bf_staged_kernel<K, NQ><<<grid, kStgThreads, staged_smem_bytes(c, NQ), st>>>(P, c);
+    bf_staged_kernel<K, NQ, INR><<<grid, kStgThreads, staged_smem_bytes(c, NQ), st>>>(P, c);
 }
-template <int NQ>
+template <int NQ, bool INR>
 inline void launch_staged_nq(int order, const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
     switch (order) {
-    case 1: launch_staged_k<1, NQ>(P, groups, c, st); break;
-    case 2: launch_staged_k<2, NQ>(P, groups, c, st); break;
-    case 3: launch_staged_k<3, NQ>(P, groups, c, st); break;
-    case 4: launch_staged_k<4, NQ>(P, groups, c, st); break;
-    default: launch_staged_k<5, NQ>(P, groups, c, st); break;
+    case 1: launch_staged_k<1, NQ, INR>(P, groups, c, st); break;
+    case 2: launch_staged_k<2, NQ, INR>(P, groups, c, st); break;
+    case 3: launch_staged_k<3, NQ, INR>(P, groups, c, st); break;
+    case 4: launch_staged_k<4, NQ, INR>(P, groups, c, st); break;
+    default: launch_staged_k<5, NQ, INR>(P, groups, c, st); break;
     }
 }
-inline void launch_staged(int order, int nq, const BfParams& P, int groups, const pab_plan_info& plan, cudaStream_t st) {
-    StagedCfg c{plan.chunk_channels, plan.stages, plan.window_samples};
-    if (nq == 0) launch_staged_nq<0>(order, P, groups, c, st);
-    else if (nq == 1) launch_staged_nq<1>(order, P, groups, c, st);
-    else launch_staged_nq<2>(order, P, groups, c, st);
+template <bool INR>
+inline void launch_staged_inr(int order, int nq, const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
+    if (nq == 0) launch_staged_nq<0, INR>(order, P, groups, c, st);
+    else if (nq == 1) launch_staged_nq<1, INR>(order, P, groups, c, st);
+    else if (nq == 2) launch_staged_nq<2, INR>(order, P, groups, c, st);
+    else launch_staged_nq<4, INR>(order, P, groups, c, st);
+}
+inline void launch_staged(int order, int nq, bool in_range, const BfParams& P, int groups, const pab_plan_info& plan,
+                          int chunk_cap, int smem_limit, cudaStream_t st) {
+    // the plan's chunk is sized for frames_per_thread / 4 quads per channel; fewer quads -> more channels per stage
+    const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (long long)sizeof(ChanEntry);
+    long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
+    if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
+    if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
+    if (chunk > P.N) chunk = P.N;
+    if (chunk < 1) chunk = 1;       // cannot happen: the plan fitted >= 1 channel at the largest nq
+    StagedCfg c{(int)chunk, plan.stages, plan.window_samples};
+    if (in_range) launch_staged_inr<true>(order, nq, P, groups, c, st);
+    else launch_staged_inr<false>(order, nq, P, groups, c, st);
 }
 
 }  // namespace pab
