@@ -258,7 +258,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         t_fp32 = items_per_launch * FP32_PER_ITEM / fp32_peak
         t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
         achieved = items_per_launch * XU_PER_ITEM / (bf_launch_ms * 1e-3)
-        roofline = {"bound": "alu", "kernel": "bf_staged_kernel<3,2> (fused delay+interp+root+power sums+Newton)",
+        roofline = {"bound": "alu", "kernel": "bf_staged_kernel<3,4,true> (fused delay+interp+root+power sums+Newton, 16 frames per thread)",
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
                     "frac": achieved / xu_peak, "traffic": None,
                     "peak_source": f"148 SM x 16 XU lanes/clk x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, "

@@ -9,6 +9,7 @@
 #include "pab_plan.h"
 #include "pab_kernels.cuh"
 #include "pab_staged.cuh"
+#include "pab_post.cuh"
 
 using namespace pab;
 
@@ -21,6 +22,9 @@ struct pab_ctx {
     int post_mode = PAB_RAW;
     int n_taps_bp = 0, n_taps_h = 0, TpB = 0, TpH = 0;
     float dyn_range_db = 60.0f;
+    PostTaps64 taps64{};             // fast post path (<= 64 taps): taps travel in the kernel parameters
+    bool post_fast = false;
+    int hilbert_parity = 2;          // 0 / 1: only Hilbert taps of that index parity are non-zero; 2: dense
     int variant = PAB_VARIANT_AUTO;
     pab_plan_info plan{};
     PlanTuning tuning{};
@@ -163,6 +167,7 @@ int pab_create(pab_ctx** out, int n_elem, int n_samp, float fs_hz, float c_m_s, 
         (cudaFuncSetAttribute(post_fir_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin) != cudaSuccess ||
          cudaFuncSetAttribute(post_fir_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin) != cudaSuccess))
         rc = PAB_ERR_CUDA;
+    if (rc == PAB_OK && post64_configure(ctx->smem_optin) != cudaSuccess) rc = PAB_ERR_CUDA;
     if (rc != PAB_OK) { free_all(ctx); delete ctx; return rc; }
     *out = ctx;
     return PAB_OK;
@@ -252,6 +257,19 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
     PAB_CUDA(ctx, cudaMemcpy(ctx->d_taps_h, hh.data(), TpH * 4, cudaMemcpyHostToDevice));
     if (!ctx->d_img)
         PAB_CUDA(ctx, cudaMalloc(&ctx->d_img, (size_t)ctx->plan.batch_frames * ctx->grid.nz * (size_t)ctx->grid.nx * 4));
+    // fast path: both filters fit 64 taps and are long enough for it to pay
+    ctx->post_fast = TpB > 32 && TpB <= 64 && (mode < PAB_ENVELOPE || (TpH > 32 && TpH <= 64));
+    if (ctx->post_fast) {
+        memset(&ctx->taps64, 0, sizeof ctx->taps64);
+        for (int t = 0; t < TpB; ++t) ctx->taps64.hb[t] = hb[t];
+        bool even_zero = true, odd_zero = true;
+        if (mode >= PAB_ENVELOPE)
+            for (int t = 0; t < TpH; ++t) {
+                ctx->taps64.hh[t] = hh[t];
+                if (hh[t] != 0.0f) { if (t & 1) odd_zero = false; else even_zero = false; }
+            }
+        ctx->hilbert_parity = odd_zero ? 0 : (even_zero ? 1 : 2);
+    }
     ctx->post_mode = mode; ctx->n_taps_bp = n_taps_bp; ctx->n_taps_h = n_taps_hilbert;
     ctx->TpB = TpB; ctx->TpH = TpH; ctx->dyn_range_db = dyn_range_db;
     return PAB_OK;

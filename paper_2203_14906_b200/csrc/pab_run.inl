@@ -120,7 +120,19 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         Q.nx = nx; Q.nz = nz;
         constexpr int TZ = 128;
         dim3 grid((nx + 31) / 32, (nz + TZ - 1) / TZ, F);
-        if (ctx->post_mode == PAB_BANDPASS) {
+        if (ctx->post_fast) {
+            const bool env = ctx->post_mode >= PAB_ENVELOPE;
+            if (env) cudaMemsetAsync(ctx->d_max, 0, (size_t)F * 4, st);
+            {
+                Span sp(ctx, PAB_STAGE_POST_FIR, st);
+                launch_post64(Q, ctx->taps64, env, ctx->hilbert_parity, F, st);
+            }
+            if (ctx->post_mode == PAB_LOG) {
+                dim3 g2((nx * nz + 1023) / 1024, F);
+                Span sp(ctx, PAB_STAGE_POST_LOG, st);
+                post_log_kernel<<<g2, 256, 0, st>>>(out, ctx->d_max, nx * nz, ctx->dyn_range_db);
+            }
+        } else if (ctx->post_mode == PAB_BANDPASS) {
             const size_t sm = ((size_t)(TZ + Q.TpB - 1) * 32 + Q.TpB + Q.TpH) * 4;
             Span sp(ctx, PAB_STAGE_POST_FIR, st);
             post_fir_kernel<TZ, false><<<grid, 256, sm, st>>>(Q);

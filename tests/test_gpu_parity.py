@@ -178,16 +178,20 @@ def test_post_chain_streaming_configs(pab, orc, cfg, frames):
             assert rel <= 2e-4, f"{cfg} {mode}: relative L2 {rel:.3e}"
 
 
-def test_post_chain_ragged_grid(pab, orc):
+@pytest.mark.parametrize("n_bp,n_h", [(31, 21), (64, 63), (50, 41), (96, 95)])
+def test_post_chain_ragged_grid(pab, orc, n_bp, n_h):
+    """Ragged grid and filter lengths on both post kernels: <= 32 and > 64 taps take the generic kernel,
+    33..64 taps the constant-bank fast path (with and without the structural zeros of the Hilbert FIR)."""
     rng = np.random.default_rng(5)
     g = synth.random_geometry(rng, 12, 700, 41, 203, in_range=True)
     rf = rng.standard_normal((3, 12, 700)).astype(np.float32)
     raw = orc.beamform(rf, g, 2)
     fs_z = g.c / g.dz
-    kw = dict(f_center=0.2 * fs_z, f_halfwidth=0.08 * fs_z, n_taps_bp=31, n_taps_hilbert=21, dyn_range_db=50.0)
-    gpu, _ = run_gpu(pab, g, rf, 2, post=dict(kw, mode="envelope"))
-    ref = orc.post(raw, g, kw["f_center"], kw["f_halfwidth"], 31, 21, 50.0, mode="envelope")
-    assert np.sqrt(np.sum((gpu - ref) ** 2) / np.sum(ref ** 2)) <= 2e-4
+    kw = dict(f_center=0.2 * fs_z, f_halfwidth=0.08 * fs_z, n_taps_bp=n_bp, n_taps_hilbert=n_h, dyn_range_db=50.0)
+    for mode in ("bandpass", "envelope"):
+        gpu, _ = run_gpu(pab, g, rf, 2, post=dict(kw, mode=mode))
+        ref = orc.post(raw, g, kw["f_center"], kw["f_halfwidth"], n_bp, n_h, 50.0, mode=mode)
+        assert np.sqrt(np.sum((gpu - ref) ** 2) / np.sum(ref ** 2)) <= 2e-4, mode
 
 
 def test_host_entry_point_matches_device_entry_point(pab):
