@@ -298,6 +298,73 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dist.destroy_process_group()
 
 
+# XU (MUFU) lane-ops and FP32-pipe slots per item, by order: (per item, per (pixel, element)) -- DESIGN.md Roofline
+_XU = {1: (0.0, 1.0), 2: (1.0, 1.0), 3: (2.0, 1.0), 4: (2.0, 1.0), 5: (2.0, 1.0)}
+_FP32 = {1: (3.0, 3.0), 2: (4.0, 3.0), 3: (6.0, 3.0), 4: (7.0, 3.0), 5: (9.0, 3.0)}
+
+
+def run_sweep(args):
+    """--sweep: every config and order of SURVEY.md section 8 (C1..C5, C2b) on one GPU, one JSON line each:
+    ms per call, frames/s, items/s, per-stage CUDA-event times and the roofline terms.  Not the driver's line."""
+    import torch
+    from paper_2203_14906_b200 import binding, synth
+    torch.cuda.set_device(0)
+    binding.load()
+    peaks = read_peaks()
+    f_hz = peaks["sm_max_mhz"] * 1e6
+    cases = [("C1", 1, (1, 2, 3, 4, 5), False), ("C2", 1, (1, 2, 3), False), ("C2b", 64, (1, 2, 3), False),
+             ("C3", 256, (3,), True), ("C4", 1, (4, 5), False), ("C4", 16, (4, 5), False), ("C5", 1024, (3,), True)]
+    for cfg, F, orders, post in cases:
+        gen = min(F, 64)
+        w = synth.make_config(cfg, n_frames=gen)
+        g = w.geom
+        call_frames = min(F, 64) if cfg == "C5" else F          # C5 streams in batches of 64 (BASELINE.json)
+        n_calls = F // call_frames
+        rf = torch.from_numpy(np.concatenate([w.rf] * (call_frames // gen), axis=0)).cuda()
+        dtype = "int16" if w.rf.dtype == np.int16 else "float32"
+        out = torch.empty((call_frames, g.nz, g.nx), dtype=torch.float32, device="cuda")
+        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None)
+        items = g.nz * g.nx * g.n_elem
+        for order in orders:
+            reps = max(3, min(50, int(0.2 / max(1e-5, items * F * 1e-12))))
+            for _ in range(3):
+                bf.beamform(rf, order, out=out)
+            torch.cuda.synchronize()
+            bf.set_profile(16 * reps * n_calls + 16)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps * n_calls):
+                bf.beamform(rf, order, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps                      # whole stream of F frames
+            prof = bf.get_profile()
+            bf.set_profile(0)
+            fpt = bf.plan()["frames_per_thread"] if F >= 4 else 1
+            if order >= 4:
+                fpt = min(fpt, 8)
+            share = min(fpt, F)                                  # frames sharing one delay computation (algorithmic: the batch)
+            batch = min(F, 64)
+            xu = _XU[order][0] + _XU[order][1] / batch
+            fp = _FP32[order][0] + _FP32[order][1] / batch
+            t_xu = items * F * xu / (SM_COUNT * XU_LANES_PER_CLK_SM * f_hz) * 1e3
+            t_fp = items * F * fp / (SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz) * 1e3
+            in_b = g.n_elem * g.n_samp * (2 if dtype == "int16" else 4)
+            t_hbm = F * (in_b + g.nz * g.nx * 4) / (peaks["hbm_gbs"] * 1e9) * 1e3
+            bf_ms = prof["beamform"][0] / reps
+            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw",
+                              "dtype_in": dtype, "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx,
+                              "ms_per_stream": round(ms, 5), "frames_per_s": round(F / (ms * 1e-3), 1),
+                              "items_per_s": round(items * F / (ms * 1e-3), 0),
+                              "stage_ms": {k: round(v[0] / reps, 5) for k, v in prof.items()},
+                              "beamform_launches": prof["beamform"][1] / reps, "frames_per_thread": share,
+                              "t_roof_ms": {"xu": round(t_xu, 5), "fp32": round(t_fp, 5), "hbm": round(t_hbm, 5)},
+                              "beamform_roofline_frac": round(max(t_xu, t_fp, t_hbm) / bf_ms, 4),
+                              "in_range": bf.plan()["in_range"]}), flush=True)
+        bf.close()
+        del rf, out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -305,12 +372,17 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="per-config table (C1..C5), one JSON line each; 1 GPU")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
         return
     if world != args.gpus and world == 1 and args.gpus > 1:
         raise SystemExit("bench.py --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU)")
