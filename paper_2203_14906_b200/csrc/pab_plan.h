@@ -80,12 +80,14 @@ inline bool plan_geometry(int n_elem, int n_samp, double fs, double c, double pi
         const double idx_max = std::sqrt(ax * ax + zl * zl);
         p.in_range = (idx_max + 1.0 < (double)n_samp - 1.0) && ((double)g.z0 * k >= 1.0) ? 1 : 0;
     }
-    // internal frame batch: keep one batch of staged RF well inside the 126 MB L2
+    // internal frame batch of the device path: as many frames per launch as 512 MiB of staged RF allow (<= 256), so
+    // that small pixel grids still give the persistent kernel many tiles per SM (tail balance); the staged copy is
+    // an intermediate that costs 2 x 4 bytes of HBM traffic per sample, far from binding (DESIGN.md Roofline).
     const double frame_bytes = (double)n_elem * n_samp * 4.0;
-    int b = (int)(64.0 * 1048576.0 / frame_bytes);
+    int b = (int)(512.0 * 1048576.0 / frame_bytes);
     b = b / 16 * 16;
     if (b < 16) b = 16;
-    if (b > 64) b = 64;
+    if (b > 256) b = 256;
     p.batch_frames = b;
     *out = p;
     return true;

@@ -83,7 +83,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         P.n_frames = F;
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, 0, in_range, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, st);
+            if (use_staged) launch_staged(order, 0, in_range, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_order<0>(order, P, F, st);
         }
     } else {
@@ -105,7 +105,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, st);
+            if (use_staged) launch_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, g, R, groups, st);
             q0 += groups * g;
             nq -= groups * g;
@@ -181,7 +181,10 @@ extern "C" int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int 
 extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host) {
     int rc = check_args(ctx, rf_host, n_frames, order, out_host);
     if (rc != PAB_OK) return rc;
-    const int B = ctx->plan.batch_frames;
+    // Host path batches: short calls are cut into 16-frame pieces so that H2D, kernels and D2H of successive pieces
+    // overlap inside one call; long streams use 64-frame pieces (more tiles per launch, negligible ramp).
+    const int Bcap = ctx->plan.batch_frames < 64 ? ctx->plan.batch_frames : 64;
+    const int B = (n_frames >= 256 || Bcap < 16) ? Bcap : 16;
     const size_t frame_in = (size_t)ctx->N * ctx->S * elem_size(ctx->dtype);
     const size_t frame_out = (size_t)ctx->grid.nz * ctx->grid.nx * 4;
     if (!ctx->s_h2d) {
@@ -189,8 +192,8 @@ extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames
         PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_run, cudaStreamNonBlocking));
         PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
         for (int b = 0; b < 2; ++b) {
-            PAB_CUDA(ctx, cudaMalloc(&ctx->d_in[b], (size_t)B * ctx->N * ctx->S * 4));   // sized for fp32
-            PAB_CUDA(ctx, cudaMalloc(&ctx->d_out[b], (size_t)B * frame_out));
+            PAB_CUDA(ctx, cudaMalloc(&ctx->d_in[b], (size_t)Bcap * ctx->N * ctx->S * 4));   // sized for fp32
+            PAB_CUDA(ctx, cudaMalloc(&ctx->d_out[b], (size_t)Bcap * frame_out));
             PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_in[b], cudaEventDisableTiming));
             PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_run[b], cudaEventDisableTiming));
             PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_out[b], cudaEventDisableTiming));

@@ -68,11 +68,14 @@ struct StagedCfg {
     int chunk;          // channels per stage (<= 32)
     int stages;         // ring depth
     int window;         // samples per channel slot per quad (multiple of 4)
+    int tiles_x, tiles_z, groups;   // tile grid: columns / 8, rows / 64, frame groups; tile t = (t % tiles_x, ...)
 };
 
 // NQ = 0: lin layout, one frame per thread; NQ = 1, 2, 4: quad layout, 4 NQ frames per thread.
 // INR: every delay index of the geometry lies inside the record (checked on the host): no masks, no clamps.
-// grid: (ceil(nx/8), ceil(nz/64), groups)
+// Persistent: grid = min(#tiles, resident CTAs); CTA b takes tiles b, b + gridDim.x, ...  The full/empty ring
+// runs on across tiles, so the producer warp is already copying the next tile's first chunks while the
+// consumer warps finish the current tile and store its images.
 template <int K, int NQ, bool INR>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParams P, const StagedCfg C) {
     constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
@@ -90,8 +93,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
     const uint32_t bar0 = smem_u32(bars);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int c0 = blockIdx.x * kStgCols, r0 = blockIdx.y * kStgRows;
     const int n_chunks = (P.N + C.chunk - 1) / C.chunk;
+    const int n_tiles = C.tiles_x * C.tiles_z * C.groups;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < C.stages; ++s) {
@@ -105,110 +108,124 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
     if (warp == kStgConsumerWarps) {
         // ---------------- producer warp: lane l stages channel (chunk * C.chunk + l) ----------------
         if (lane >= C.chunk) return;
-        const int rl = min(r0 + kStgRows - 1, P.nz - 1);
-        const float4 zf = P.zrow[r0], zl = P.zrow[rl];
-        float2 xj[kStgCols];
-#pragma unroll
-        for (int c = 0; c < kStgCols; ++c) xj[c] = P.xj[min(c0 + c, P.nx - 1)];
         const size_t chan_stride = NQ == 0 ? (size_t)P.Sp * 4 : (size_t)P.S * 16;        // bytes
         const size_t grp_stride = (size_t)P.N * chan_stride;                              // one frame / one quad
-        const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)blockIdx.z * (NQ == 0 ? 1 : NQ) * grp_stride;
         const int row_len = NQ == 0 ? P.Sp : P.S;
-        for (int ck = 0; ck < n_chunks; ++ck) {
-            const int s = ck % C.stages;
-            const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
-            mbar_wait(empty, ((ck / C.stages) & 1) ^ 1);
-            const int ch = ck * C.chunk + lane;
-            if (ch >= P.N) { mbar_arrive(full); continue; }
-            const float2 xe = __ldg(P.xe + ch);
-            ChanEntry e;
+        int s = 0;
+        uint32_t ph = 1;                                     // parity to wait for on empty[s]
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            const int bx = tile % C.tiles_x, by = (tile / C.tiles_x) % C.tiles_z, bz = tile / (C.tiles_x * C.tiles_z);
+            const int c0 = bx * kStgCols, r0 = by * kStgRows;
+            const int rl = min(r0 + kStgRows - 1, P.nz - 1);
+            const float4 zf = P.zrow[r0], zl = P.zrow[rl];
+            float2 xj[kStgCols];
 #pragma unroll
-            for (int c = 0; c < kStgCols; ++c) e.xs[c] = (xj[c].x - xe.x) + (xj[c].y - xe.y);
-            const float xlo = e.xs[0], xhi = e.xs[kStgCols - 1];
-            const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
-            const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
-            const float imin = fminf(sqrtf(fmaf(amin, amin, zf.y)), 2.0e6f);
-            const float imax = fminf(sqrtf(fmaf(amax, amax, zl.y)), 2.0e6f);
-            int w0 = max((int)floorf(imin) - 1, 0) & ~3;
-            int w1 = (int)floorf(imax) + 3;
-            if (NQ == 0) {
-                w1 = (w1 + 3) & ~3;
-                w0 = min(w0, row_len - 4);
-                w1 = min(max(w1, w0 + 4), row_len);
-            } else {
-                w0 = min(w0, (row_len - 2) & ~3);
-                w1 = min(max(w1, w0 + 2), row_len);
+            for (int c = 0; c < kStgCols; ++c) xj[c] = P.xj[min(c0 + c, P.nx - 1)];
+            const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)bz * (NQ == 0 ? 1 : NQ) * grp_stride;
+            for (int ck = 0; ck < n_chunks; ++ck) {
+                const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
+                mbar_wait(empty, ph);
+                const int ch = ck * C.chunk + lane;
+                if (ch < P.N) {
+                    const float2 xe = __ldg(P.xe + ch);
+                    ChanEntry e;
+#pragma unroll
+                    for (int c = 0; c < kStgCols; ++c) e.xs[c] = (xj[c].x - xe.x) + (xj[c].y - xe.y);
+                    const float xlo = e.xs[0], xhi = e.xs[kStgCols - 1];
+                    const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
+                    const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
+                    const float imin = fminf(sqrtf(fmaf(amin, amin, zf.y)), 2.0e6f);
+                    const float imax = fminf(sqrtf(fmaf(amax, amax, zl.y)), 2.0e6f);
+                    int w0 = max((int)floorf(imin) - 1, 0) & ~3;
+                    int w1 = (int)floorf(imax) + 3;
+                    if (NQ == 0) {
+                        w1 = (w1 + 3) & ~3;
+                        w0 = min(w0, row_len - 4);
+                        w1 = min(max(w1, w0 + 4), row_len);
+                    } else {
+                        w0 = min(w0, (row_len - 2) & ~3);
+                        w1 = min(max(w1, w0 + 2), row_len);
+                    }
+                    w1 = min(w1, w0 + C.window);
+                    const int len = w1 - w0;
+                    const int slot = s * stage_bytes + lane * slot_bytes;
+                    e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
+#pragma unroll
+                    for (int k = 0; k < 5; ++k) e.pad[k] = 0;
+                    tab[s * C.chunk + lane] = e;
+                    const uint32_t bytes = (uint32_t)len * BPS;
+                    mbar_arrive_expect_tx(full, bytes * NCOPY);
+                    const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
+#pragma unroll
+                    for (int q = 0; q < NCOPY; ++q)
+                        bulk_g2s(data0 + slot + q * quad_bytes, src + q * grp_stride, bytes, full);
+                } else {
+                    mbar_arrive(full);
+                }
+                if (++s == C.stages) { s = 0; ph ^= 1; }
             }
-            w1 = min(w1, w0 + C.window);
-            const int len = w1 - w0;
-            const int slot = s * stage_bytes + lane * slot_bytes;
-            e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
-#pragma unroll
-            for (int k = 0; k < 5; ++k) e.pad[k] = 0;
-            tab[s * C.chunk + lane] = e;
-            const uint32_t bytes = (uint32_t)len * BPS;
-            mbar_arrive_expect_tx(full, bytes * NCOPY);
-            const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
-#pragma unroll
-            for (int q = 0; q < NCOPY; ++q)
-                bulk_g2s(data0 + slot + q * quad_bytes, src + q * grp_stride, bytes, full);
         }
         return;
     }
 
     // ---------------- consumer warps ----------------
     const int col = warp & 7;
-    const int j = c0 + col;
-    const int m = r0 + (warp >> 3) * 32 + lane;
-    const float4 row = P.zrow[min(m, P.nz - 1)];
-    float p[NF][K];
+    int s = 0;
+    uint32_t ph = 0;                                         // parity to wait for on full[s]
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int bx = tile % C.tiles_x, by = (tile / C.tiles_x) % C.tiles_z, bz = tile / (C.tiles_x * C.tiles_z);
+        const int j = bx * kStgCols + col;
+        const int m = by * kStgRows + (warp >> 3) * 32 + lane;
+        const float4 row = P.zrow[min(m, P.nz - 1)];
+        float p[NF][K];
 #pragma unroll
-    for (int f = 0; f < NF; ++f)
+        for (int f = 0; f < NF; ++f)
 #pragma unroll
-        for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+            for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
 
-    for (int ck = 0; ck < n_chunks; ++ck) {
-        const int s = ck % C.stages;
-        mbar_wait(bar0 + 8 * s, (ck / C.stages) & 1);
-        const int nch = min(C.chunk, P.N - ck * C.chunk);
-        const uint32_t tab_s = smem_u32(tab + s * C.chunk) + col * 4;
+        for (int ck = 0; ck < n_chunks; ++ck) {
+            mbar_wait(bar0 + 8 * s, ph);
+            const int nch = min(C.chunk, P.N - ck * C.chunk);
+            const uint32_t tab_s = smem_u32(tab + s * C.chunk) + col * 4;
 #pragma unroll 2
-        for (int l = 0; l < nch; ++l) {
-            const float xs = lds32(tab_s + l * 64);
-            const int base = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 32));
-            const Tap t = delay_tap<INR>(xs, xs * xs, row, P.S);
-            int i0 = t.i0;
-            if constexpr (!INR) {
-                const int w0 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 36));
-                const int w1m2 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 40));
-                i0 = min(max(i0, w0), w1m2);
-            }
-            const uint32_t a = (uint32_t)base + i0 * BPS;
-            if constexpr (NQ == 0) {
-                const float s0 = lds32(a), s1 = lds32(a + 4);
-                accumulate<K>(interp<INR>(t, s0, s1), p[0]);
-            } else {
+            for (int l = 0; l < nch; ++l) {
+                const float xs = lds32(tab_s + l * 64);
+                const int base = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 32));
+                const Tap t = delay_tap<INR>(xs, xs * xs, row, P.S);
+                int i0 = t.i0;
+                if constexpr (!INR) {
+                    const int w0 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 36));
+                    const int w1m2 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 40));
+                    i0 = min(max(i0, w0), w1m2);
+                }
+                const uint32_t a = (uint32_t)base + i0 * BPS;
+                if constexpr (NQ == 0) {
+                    const float s0 = lds32(a), s1 = lds32(a + 4);
+                    accumulate<K>(interp<INR>(t, s0, s1), p[0]);
+                } else {
 #pragma unroll
-                for (int q = 0; q < NQ; ++q) {
-                    const float4 s0 = lds128(a + q * quad_bytes);
-                    const float4 s1 = lds128(a + q * quad_bytes + 16);
-                    accumulate<K>(interp<INR>(t, s0.x, s1.x), p[4 * q + 0]);
-                    accumulate<K>(interp<INR>(t, s0.y, s1.y), p[4 * q + 1]);
-                    accumulate<K>(interp<INR>(t, s0.z, s1.z), p[4 * q + 2]);
-                    accumulate<K>(interp<INR>(t, s0.w, s1.w), p[4 * q + 3]);
+                    for (int q = 0; q < NQ; ++q) {
+                        const float4 s0 = lds128(a + q * quad_bytes);
+                        const float4 s1 = lds128(a + q * quad_bytes + 16);
+                        accumulate<K>(interp<INR>(t, s0.x, s1.x), p[4 * q + 0]);
+                        accumulate<K>(interp<INR>(t, s0.y, s1.y), p[4 * q + 1]);
+                        accumulate<K>(interp<INR>(t, s0.z, s1.z), p[4 * q + 2]);
+                        accumulate<K>(interp<INR>(t, s0.w, s1.w), p[4 * q + 3]);
+                    }
                 }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar0 + 8 * (C.stages + s));
+            if (++s == C.stages) { s = 0; ph ^= 1; }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar0 + 8 * (C.stages + s));
-    }
 
-    if (j < P.nx && m < P.nz) {
-        const size_t img = (size_t)P.nz * P.nx;
+        if (j < P.nx && m < P.nz) {
+            const size_t img = (size_t)P.nz * P.nx;
 #pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            const int frame = blockIdx.z * NF + f;
-            if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+            for (int f = 0; f < NF; ++f) {
+                const int frame = bz * NF + f;
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+            }
         }
     }
 }
@@ -246,29 +263,37 @@ inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
 }
 
 template <int K, int NQ, bool INR>
-inline void launch_staged_k(const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
-    dim3 grid((P.nx + kStgCols - 1) / kStgCols, (P.nz + kStgRows - 1) / kStgRows, groups);
-    bf_staged_kernel<K, NQ, INR><<<grid, kStgThreads, staged_smem_bytes(c, NQ), st>>>(P, c);
+inline void launch_staged_k(const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
+    const size_t smem = staged_smem_bytes(c, NQ);
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_staged_kernel<K, NQ, INR>, kStgThreads, smem) != cudaSuccess ||
+        per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups;
+    const long long resident = (long long)sm_count * per_sm;
+    bf_staged_kernel<K, NQ, INR><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(P, c);
 }
 template <int NQ, bool INR>
-inline void launch_staged_nq(int order, const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
+inline void launch_staged_nq(int order, const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
     switch (order) {
-    case 1: launch_staged_k<1, NQ, INR>(P, groups, c, st); break;
-    case 2: launch_staged_k<2, NQ, INR>(P, groups, c, st); break;
-    case 3: launch_staged_k<3, NQ, INR>(P, groups, c, st); break;
-    case 4: launch_staged_k<4, NQ, INR>(P, groups, c, st); break;
-    default: launch_staged_k<5, NQ, INR>(P, groups, c, st); break;
+    case 1: launch_staged_k<1, NQ, INR>(P, c, sm_count, st); break;
+    case 2: launch_staged_k<2, NQ, INR>(P, c, sm_count, st); break;
+    case 3: launch_staged_k<3, NQ, INR>(P, c, sm_count, st); break;
+    case 4: launch_staged_k<4, NQ, INR>(P, c, sm_count, st); break;
+    default: launch_staged_k<5, NQ, INR>(P, c, sm_count, st); break;
     }
 }
 template <bool INR>
-inline void launch_staged_inr(int order, int nq, const BfParams& P, int groups, const StagedCfg& c, cudaStream_t st) {
-    if (nq == 0) launch_staged_nq<0, INR>(order, P, groups, c, st);
-    else if (nq == 1) launch_staged_nq<1, INR>(order, P, groups, c, st);
-    else if (nq == 2) launch_staged_nq<2, INR>(order, P, groups, c, st);
-    else launch_staged_nq<4, INR>(order, P, groups, c, st);
+inline void launch_staged_inr(int order, int nq, const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
+    if (nq == 0) launch_staged_nq<0, INR>(order, P, c, sm_count, st);
+    else if (nq == 1) launch_staged_nq<1, INR>(order, P, c, sm_count, st);
+    else if (nq == 2) launch_staged_nq<2, INR>(order, P, c, sm_count, st);
+    else launch_staged_nq<4, INR>(order, P, c, sm_count, st);
 }
 inline void launch_staged(int order, int nq, bool in_range, const BfParams& P, int groups, const pab_plan_info& plan,
-                          int chunk_cap, int smem_limit, cudaStream_t st) {
+                          int chunk_cap, int smem_limit, int sm_count, cudaStream_t st) {
     // the plan's chunk is sized for frames_per_thread / 4 quads per channel; fewer quads -> more channels per stage
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (long long)sizeof(ChanEntry);
     long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
@@ -276,9 +301,10 @@ inline void launch_staged(int order, int nq, bool in_range, const BfParams& P, i
     if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
     if (chunk > P.N) chunk = P.N;
     if (chunk < 1) chunk = 1;       // cannot happen: the plan fitted >= 1 channel at the largest nq
-    StagedCfg c{(int)chunk, plan.stages, plan.window_samples};
-    if (in_range) launch_staged_inr<true>(order, nq, P, groups, c, st);
-    else launch_staged_inr<false>(order, nq, P, groups, c, st);
+    StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
+                (P.nz + kStgRows - 1) / kStgRows, groups};
+    if (in_range) launch_staged_inr<true>(order, nq, P, c, sm_count, st);
+    else launch_staged_inr<false>(order, nq, P, c, sm_count, st);
 }
 
 }  // namespace pab

@@ -68,7 +68,9 @@ def test_plan_bounds_every_tile_window(binding, cfg):
     g = synth.geometry(cfg)
     p = binding.plan(g)
     assert p["tile_z"] == 64 and p["tile_x"] == 8
-    assert p["batch_frames"] % 8 == 0 and 8 <= p["batch_frames"] <= 64
+    assert p["batch_frames"] % 16 == 0 and 16 <= p["batch_frames"] <= 256
+    assert p["batch_frames"] * g.n_elem * g.n_samp * 4 <= 512 * 2 ** 20 or p["batch_frames"] == 16
+    assert p["frames_per_thread"] == 16 and p["in_range"] == (0 if cfg == "C1" else 1)   # C1 starts at z = 0
     assert 0 < p["smem_bytes"] <= 232448
     assert 1 <= p["chunk_channels"] <= min(32, g.n_elem) and p["stages"] in (2, 3)
     assert p["window_samples"] % 4 == 0
