@@ -106,9 +106,10 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
                  int n_taps_hilbert, float dyn_range_db);
 
 /* pab_set_tuning -- override the plan's blocking (autotuning / experiments); 0 keeps the default of a field.
- *   frames_per_thread 4, 8 or 16;  stages 2..4;  chunk_channels 1..32 (clamped to what fits in shared memory).
+ *   frames_per_thread 4, 8 or 16;  stages 2..4;  chunk_channels 1..32 (clamped to what fits in shared memory);
+ *   host_batch_frames 1..64: frames per piece of pab_beamform_host's copy / compute / copy pipeline.
  * Recomputes the plan (pab_get_plan shows the result).  Synchronises the device.  PAB_ERR_INVALID on bad values. */
-int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_channels);
+int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_channels, int host_batch_frames);
 
 /* pab_set_variant -- force a beamforming kernel variant (testing / benchmarking).  PAB_ERR_INVALID when the
  * staged variant is requested but its plan does not fit in shared memory. */

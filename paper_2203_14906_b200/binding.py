@@ -64,7 +64,7 @@ def load(build_if_missing: bool = False):
     L.pab_set_input.argtypes = [vp, ip, fp]
     L.pab_set_post.argtypes = [vp, ip, fp, fp, ip, ip, fp]
     L.pab_set_variant.argtypes = [vp, ip]
-    L.pab_set_tuning.argtypes = [vp, ip, ip, ip]
+    L.pab_set_tuning.argtypes = [vp, ip, ip, ip, ip]
     L.pab_beamform.argtypes = [vp, vp, ip, ip, vp, vp]
     L.pab_beamform_host.argtypes = [vp, vp, ip, ip, vp]
     L.pab_destroy.argtypes = [vp]
@@ -157,8 +157,10 @@ class Beamformer:
     def set_variant(self, variant: str):
         self._check(self._L.pab_set_variant(self._h, _VARIANTS[variant]), "pab_set_variant")
 
-    def set_tuning(self, frames_per_thread: int = 0, stages: int = 0, chunk_channels: int = 0):
-        self._check(self._L.pab_set_tuning(self._h, frames_per_thread, stages, chunk_channels), "pab_set_tuning")
+    def set_tuning(self, frames_per_thread: int = 0, stages: int = 0, chunk_channels: int = 0,
+                   host_batch_frames: int = 0):
+        self._check(self._L.pab_set_tuning(self._h, frames_per_thread, stages, chunk_channels, host_batch_frames),
+                    "pab_set_tuning")
 
     def plan(self) -> dict:
         info = PlanInfo()

@@ -214,10 +214,10 @@ int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_laun
     return PAB_OK;
 }
 
-int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_channels) {
-    if (!ctx) return PAB_ERR_INVALID;
+int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_channels, int host_batch_frames) {
+    if (!ctx || host_batch_frames < 0 || host_batch_frames > 64) return PAB_ERR_INVALID;
     PlanTuning t;
-    t.frames_per_thread = frames_per_thread; t.stages = stages; t.chunk_channels = chunk_channels;
+    t.frames_per_thread = frames_per_thread; t.stages = stages; t.chunk_channels = chunk_channels; t.host_batch_frames = host_batch_frames;
     pab_plan_info plan;
     if (!plan_geometry(ctx->N, ctx->S, ctx->fs, ctx->c, ctx->pitch, ctx->grid, ctx->smem_optin, &plan, t)) return PAB_ERR_INVALID;
     PAB_CUDA(ctx, cudaDeviceSynchronize());

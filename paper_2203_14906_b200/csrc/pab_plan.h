@@ -28,6 +28,7 @@ struct PlanTuning {
     int frames_per_thread = 0;   // 4, 8 or 16; 0 = default
     int stages = 0;              // 2..4; 0 = default
     int chunk_channels = 0;      // 1..32; 0 = as many as fit
+    int host_batch_frames = 0;   // frames per piece of the host entry point's copy/compute pipeline; 0 = default
 };
 constexpr int kDefaultFramesPerThread = 16;
 
