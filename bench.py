@@ -158,6 +158,16 @@ def run_reference(args, rank: int):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(values, world: int, device):
+    """Replicas-only timing rule: every rank measures its own replica, the job's time is the max over ranks."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
 def run_ours(args, rank: int, local_rank: int, world: int):
     import torch
     import torch.distributed as dist
@@ -238,10 +248,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     raw_ms = r0.elapsed_time(r1) / K
     bf_raw.close()
 
-    t = torch.tensor([ms_total, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, e2e_ms = float(t[0]), float(t[1])
+    ms_total, e2e_ms = max_over_ranks([ms_total, e2e_ms], world, dev)
     if rank == 0:
         peaks = read_peaks()
         ms_step = ms_total / K
