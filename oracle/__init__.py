@@ -130,6 +130,36 @@ def beamform(rf, g, order: int, route: int = ROUTE_RECUR, scale=1.0, nthreads: i
     return (out, used) if return_threads else out
 
 
+def coherence_factor(s) -> float:
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    L = lib()
+    L.orc_coherence_factor.restype = C.c_double
+    return L.orc_coherence_factor(_dptr(s), C.c_int(s.size))
+
+
+def beamform_ex(rf, g, order: int, interp: str = "linear", weight: str = "none", route: int = ROUTE_RECUR, scale=1.0,
+                nthreads: int = 0):
+    """Reference image with the section 8(f) options: interp "linear" | "nearest" (A21), weight "none" | "cf" (A20)."""
+    rf, dt = _rf(rf)
+    F = rf.shape[0]
+    out = np.empty((F, g.nz, g.nx))
+    gr = _grid(g)
+    lib().orc_beamform_ex(C.c_void_p(rf.ctypes.data), C.c_int(dt), C.c_double(scale), C.c_int(F), C.c_int(g.n_elem),
+                          C.c_int(g.n_samp), C.c_double(g.fs), C.c_double(g.c), C.c_double(g.pitch), C.byref(gr),
+                          C.c_int(order), C.c_int(route), C.c_int({"linear": 0, "nearest": 1}[interp]),
+                          C.c_int({"none": 0, "cf": 1}[weight]), _dptr(out), C.c_int(nthreads))
+    return out
+
+
+def nearest_index(g) -> np.ndarray:
+    """n[nz][nx][N]: the nearest-sample index the oracle picks, -1 outside the record (A21)."""
+    out = np.empty((g.nz, g.nx, g.n_elem), dtype=np.int32)
+    gr = _grid(g)
+    lib().orc_nearest_index(C.c_int(g.n_elem), C.c_int(g.n_samp), C.c_double(g.fs), C.c_double(g.c),
+                            C.c_double(g.pitch), C.byref(gr), out.ctypes.data_as(C.POINTER(C.c_int)))
+    return out
+
+
 def beamform_pixels(rf, g, order: int, pix, route: int = ROUTE_RECUR, scale=1.0) -> np.ndarray:
     """out[F][n_pix] at sampled pixels pix[n_pix][2] = (row m, column j)."""
     rf, dt = _rf(rf)

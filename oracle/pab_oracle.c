@@ -26,6 +26,9 @@
  *                         repair A1; the as-printed form is also kept and shown NOT to be e5)
  *   orc_beamform          order 1 == orc_das bitwise (P1); point absorber peaks at its pixel (P8);
  *                         homogeneity and channel-reversal symmetry (P6)
+ *   orc_beamform_ex       interp = 0, weight = 0 == orc_beamform bitwise; nearest: numpy rint gather written
+ *                         independently, staircase-RF closed form; CF: hand value 6/7 for (1,2,3), CF = 1 for equal
+ *                         samples, 0 for +-a pairs, bounds [0,1], scale invariance, constant-RF closed form C(N,k) a
  *   orc_bandpass_taps     scipy.signal.firwin(scale=False) ; symmetry
  *   orc_hilbert_taps      antisymmetry, zero even taps, closed form 2/(pi t) * Hamming
  *   orc_fir_axial         numpy.convolve
@@ -247,6 +250,79 @@ void orc_beamform_pixels(const void* rf, int dtype, double scale, int F, int N, 
             out[(size_t)f * n_pix + p] = v;
         }
     free(s);
+}
+
+/* ---------------------------------------------------------------------------------------------------------
+ * f4 nearest-sample delays (the literal eq. 1) and f1 coherence-factor weighting.
+ * ------------------------------------------------------------------------------------------------------- */
+
+/* f4, reading A21: eq. (1) PAPER.md:29 indexes an integer sample, s_i[k + Delta_i].  Nearest-sample gather:
+ * n = floor(idx + 1/2); s_i = rf_i[n] when 0 <= n <= S-1, else 0 (A6). */
+static double nearest_chan(const void* rf, int dtype, double scale, size_t chan_off, int S, double idx) {
+    double n = floor(idx + 0.5);
+    if (!(n >= 0.0) || !(n <= (double)(S - 1))) return 0.0;
+    return rf_at(rf, dtype, scale, chan_off + (size_t)n);
+}
+
+/* f1, reading A20: PAPER.md:207 ("can be combined with coherence based real-time weighting factors") names no
+ * formula; the coherence factor of the beamforming literature is taken:
+ *   CF = (sum_i s_i)^2 / (N sum_i s_i^2),  0 when every s_i = 0;  N counts every element (A6: N is not reduced).
+ * 0 <= CF <= 1 by Cauchy-Schwarz, CF = 1 iff all s_i are equal. */
+double orc_coherence_factor(const double* s, int n) {
+    double sum = 0.0, sq = 0.0;
+    for (int i = 0; i < n; ++i) { sum += s[i]; sq += s[i] * s[i]; }
+    if (!(sq > 0.0)) return 0.0;
+    return sum * sum / ((double)n * sq);
+}
+
+/* Reference image with the options of rows f1 / f4: interp 0 = linear (O4), 1 = nearest (A21);
+ * weight 0 = none, 1 = out = CF * e_k (A20).  Same loops as orc_beamform otherwise.  Returns threads used. */
+int orc_beamform_ex(const void* rf, int dtype, double scale, int F, int N, int S, double fs, double c, double pitch,
+                    const orc_grid* g, int order, int route, int interp, int weight, double* out, int nthreads) {
+    int used = 1;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    else omp_set_num_threads(omp_get_num_procs());
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+    }
+#endif
+    for (int f = 0; f < F; ++f) {
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int m = 0; m < g->nz; ++m) {
+            double* s = (double*)malloc(sizeof(double) * (size_t)N);
+            for (int j = 0; j < g->nx; ++j) {
+                const double x = g->x0 + j * g->dx, z = g->z0 + m * g->dz;
+                for (int i = 0; i < N; ++i) {
+                    double idx = orc_delay_idx(x, z, orc_elem_x(i, N, pitch), fs, c);
+                    size_t off = ((size_t)f * N + i) * (size_t)S;
+                    s[i] = interp == 1 ? nearest_chan(rf, dtype, scale, off, S, idx)
+                                       : interp_chan(rf, dtype, scale, off, S, idx);
+                }
+                double v;
+                if (route == 0) v = orc_combine_brute(s, N, order);
+                else if (route == 2) v = orc_combine_closed(s, N, order, 1);
+                else v = orc_combine_recur(s, N, order);
+                if (weight == 1) v *= orc_coherence_factor(s, N);
+                out[((size_t)f * g->nz + m) * g->nx + j] = v;
+            }
+            free(s);
+        }
+    }
+    return used;
+}
+
+/* nearest-sample index n[nz][nx][N] as the oracle decides it (-1 when outside the record): test hook for A21 */
+void orc_nearest_index(int N, int S, double fs, double c, double pitch, const orc_grid* g, int* n_out) {
+    for (int m = 0; m < g->nz; ++m)
+        for (int j = 0; j < g->nx; ++j)
+            for (int i = 0; i < N; ++i) {
+                double idx = orc_delay_idx(g->x0 + j * g->dx, g->z0 + m * g->dz, orc_elem_x(i, N, pitch), fs, c);
+                double n = floor(idx + 0.5);
+                n_out[((size_t)m * g->nx + j) * N + i] = (n >= 0.0 && n <= (double)(S - 1)) ? (int)n : -1;
+            }
 }
 
 /* ---------------------------------------------------------------------------------------------------------

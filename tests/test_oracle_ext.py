@@ -1,0 +1,100 @@
+"""-m "not gpu": pins of the oracle's section 8(f) options: coherence-factor weighting (f1, reading A20) and
+nearest-sample delays (f4, reading A21).  Nothing here comes from the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2203_14906_b200 import synth
+
+
+@pytest.fixture(scope="module")
+def c1():
+    return synth.make_config("C1", n_frames=2)
+
+
+def test_ex_defaults_equal_plain_beamform_bitwise(orc, c1):
+    for k in (1, 3, 4):
+        assert np.array_equal(orc.beamform_ex(c1.rf, c1.geom, k), orc.beamform(c1.rf, c1.geom, k))
+
+
+def test_cf_hand_values(orc):
+    # (1 + 2 + 3)^2 / (3 (1 + 4 + 9)) = 36 / 42 = 6/7, by hand
+    assert orc.coherence_factor([1.0, 2.0, 3.0]) == pytest.approx(6.0 / 7.0, rel=1e-15)
+    assert orc.coherence_factor([2.5] * 9) == pytest.approx(1.0, rel=1e-15)          # equal samples: fully coherent
+    assert orc.coherence_factor([1.0, -1.0, 3.0, -3.0]) == 0.0                        # zero mean: incoherent
+    assert orc.coherence_factor([0.0, 0.0, 0.0]) == 0.0                               # all zero: defined as 0
+    # one non-zero channel of N: CF = 1/N (zeros count, A6)
+    assert orc.coherence_factor([0.0, 0.0, 4.0, 0.0]) == pytest.approx(0.25, rel=1e-15)
+
+
+def test_cf_bounds_scale_and_permutation_invariance(orc):
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        s = rng.standard_normal(17)
+        cf = orc.coherence_factor(s)
+        assert 0.0 <= cf <= 1.0
+        assert orc.coherence_factor(-3.7 * s) == pytest.approx(cf, rel=1e-13)
+        assert orc.coherence_factor(rng.permutation(s)) == pytest.approx(cf, rel=1e-13)
+        assert cf == pytest.approx(np.mean(s) ** 2 / np.mean(s ** 2), rel=1e-12)     # the same ratio, in numpy
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_cf_weighted_image(orc, c1, k):
+    g = c1.geom
+    plain = orc.beamform(c1.rf, g, k)
+    cfw = orc.beamform_ex(c1.rf, g, k, weight="cf")
+    s = orc.gather(c1.rf, g, frame=1)                                    # [nz][nx][N] delayed samples
+    cf = np.mean(s, axis=-1) ** 2 / np.maximum(np.mean(s ** 2, axis=-1), 1e-300)
+    assert np.allclose(cfw[1], cf * plain[1], rtol=1e-11, atol=1e-11 * np.abs(plain).max())
+    assert np.all(np.abs(cfw) <= np.abs(plain) * (1 + 1e-12))            # CF <= 1 never amplifies
+    # constant RF: CF = 1 on every fully in-range pixel, so the binomial closed form P4 still holds
+    rf = np.full_like(c1.rf, -2.5)
+    img = orc.beamform_ex(rf, g, k, weight="cf")
+    full = np.all(orc.delays(g) < g.n_samp - 1.001, axis=-1) & np.all(orc.delays(g) >= 0, axis=-1)
+    expect = math.comb(g.n_elem, k) * (-2.5 if k % 2 else 2.5)
+    assert np.allclose(img[0][full], expect, rtol=1e-11)
+    # homogeneity survives the weighting: CF is scale invariant
+    a = orc.beamform_ex((2.0 * c1.rf).astype(np.float32), g, k, weight="cf")
+    assert np.allclose(a, 2.0 * cfw, rtol=1e-11, atol=1e-12 * np.abs(cfw).max())
+
+
+def test_nearest_index_and_gather_against_numpy(orc, c1):
+    g = c1.geom
+    xe = g.elem_x()
+    x = g.pix_x()[None, :, None]
+    z = g.pix_z()[:, None, None]
+    idx = g.fs * np.sqrt((x - xe[None, None, :]) ** 2 + z ** 2) / g.c
+    n = np.floor(idx + 0.5).astype(np.int64)
+    ok = (n >= 0) & (n <= g.n_samp - 1)
+    assert np.array_equal(orc.nearest_index(g), np.where(ok, n, -1))
+    # DAS with nearest samples == numpy fancy-indexed gather, summed over elements
+    rf = c1.rf[0].astype(np.float64)
+    gathered = np.where(ok, rf[np.arange(g.n_elem)[None, None, :], np.clip(n, 0, g.n_samp - 1)], 0.0)
+    img = orc.beamform_ex(c1.rf[:1], g, 1, interp="nearest")[0]
+    assert np.allclose(img, gathered.sum(-1), rtol=1e-13, atol=1e-13)
+    # order 3 on the same gathered samples through the combination pin (route B on numpy-gathered samples)
+    img3 = orc.beamform_ex(c1.rf[:1], g, 3, interp="nearest")[0]
+    for (m, j) in ((0, 0), (57, 9), (127, 15)):
+        assert img3[m, j] == pytest.approx(orc.combine(gathered[m, j], 3), rel=1e-13)
+
+
+def test_nearest_staircase_closed_form(orc):
+    """RF = sample index n on every channel: nearest-sample DAS is sum_i round(idx_i) exactly; linear
+    interpolation gives sum_i idx_i (P7); they differ by at most N/2."""
+    g = synth.random_geometry(np.random.default_rng(8), 9, 600, 7, 33, in_range=True)
+    rf = np.tile(np.arange(g.n_samp, dtype=np.float32), (1, g.n_elem, 1))
+    idx = orc.delays(g)
+    near = orc.beamform_ex(rf, g, 1, interp="nearest")[0]
+    lin = orc.beamform_ex(rf, g, 1, interp="linear")[0]
+    assert np.array_equal(near, np.floor(idx + 0.5).sum(-1))
+    assert np.allclose(lin, idx.sum(-1), rtol=1e-12)
+    assert np.max(np.abs(near - lin)) <= g.n_elem / 2
+
+
+def test_nearest_out_of_record_is_zero(orc):
+    g = synth.random_geometry(np.random.default_rng(9), 5, 200, 6, 40, in_range=False)
+    rf = np.ones((1, g.n_elem, g.n_samp), dtype=np.float32)
+    img = orc.beamform_ex(rf, g, 1, interp="nearest")[0]
+    inside = (orc.nearest_index(g) >= 0).sum(-1)
+    assert np.array_equal(img, inside.astype(np.float64)) and inside.min() < g.n_elem
