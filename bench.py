@@ -319,9 +319,11 @@ def run_sweep(args):
     binding.load()
     peaks = read_peaks()
     f_hz = peaks["sm_max_mhz"] * 1e6
-    cases = [("C1", 1, (1, 2, 3, 4, 5), False), ("C2", 1, (1, 2, 3), False), ("C2b", 64, (1, 2, 3), False),
-             ("C3", 256, (3,), True), ("C4", 1, (4, 5), False), ("C4", 16, (4, 5), False), ("C5", 1024, (3,), True)]
-    for cfg, F, orders, post in cases:
+    cases = [("C1", 1, (1, 2, 3, 4, 5), False, "none"), ("C2", 1, (1, 2, 3), False, "none"),
+             ("C2b", 64, (1, 2, 3), False, "none"), ("C2b", 64, (3,), False, "cf"), ("C3", 256, (3,), True, "none"),
+             ("C4", 1, (4, 5), False, "none"), ("C4", 16, (4, 5), False, "none"), ("C4", 16, (5,), False, "cf"),
+             ("C5", 1024, (3,), True, "none")]
+    for cfg, F, orders, post, weight in cases:
         gen = min(F, 64)
         w = synth.make_config(cfg, n_frames=gen)
         g = w.geom
@@ -330,7 +332,7 @@ def run_sweep(args):
         rf = torch.from_numpy(np.concatenate([w.rf] * (call_frames // gen), axis=0)).cuda()
         dtype = "int16" if w.rf.dtype == np.int16 else "float32"
         out = torch.empty((call_frames, g.nz, g.nx), dtype=torch.float32, device="cuda")
-        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None)
+        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None, weight=weight)
         items = g.nz * g.nx * g.n_elem
         for order in orders:
             reps = max(3, min(50, int(0.2 / max(1e-5, items * F * 1e-12))))
@@ -350,16 +352,18 @@ def run_sweep(args):
             fpt = bf.plan()["frames_per_thread"] if F >= 4 else 1
             if order >= 4:
                 fpt = min(fpt, 8)
+            if weight == "cf":
+                fpt = min(fpt, 4 if order >= 4 else 8)
             share = min(fpt, F)                                  # frames sharing one delay computation (algorithmic: the batch)
             batch = min(F, 64)
             xu = _XU[order][0] + _XU[order][1] / batch
-            fp = _FP32[order][0] + _FP32[order][1] / batch
+            fp = _FP32[order][0] + _FP32[order][1] / batch + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
             t_xu = items * F * xu / (SM_COUNT * XU_LANES_PER_CLK_SM * f_hz) * 1e3
             t_fp = items * F * fp / (SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz) * 1e3
             in_b = g.n_elem * g.n_samp * (2 if dtype == "int16" else 4)
             t_hbm = F * (in_b + g.nz * g.nx * 4) / (peaks["hbm_gbs"] * 1e9) * 1e3
             bf_ms = prof["beamform"][0] / reps
-            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw",
+            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw", "weight": weight,
                               "dtype_in": dtype, "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx,
                               "ms_per_stream": round(ms, 5), "frames_per_s": round(F / (ms * 1e-3), 1),
                               "items_per_s": round(items * F / (ms * 1e-3), 0),

@@ -43,6 +43,10 @@ extern "C" {
 #define PAB_ENVELOPE 2   /* after band-pass and Hilbert-FIR envelope                                              */
 #define PAB_LOG      3   /* after band-pass, envelope and log compression, dB <= 0                                */
 
+/* pixel weighting (pab_set_weight) */
+#define PAB_WEIGHT_NONE 0   /* out = e_k                                                                          */
+#define PAB_WEIGHT_CF   1   /* out = CF e_k, CF = (sum_i s_i)^2 / (N sum_i s_i^2), 0 when every s_i = 0             */
+
 /* beamforming kernel variant (pab_set_variant) */
 #define PAB_VARIANT_AUTO   0   /* staged when its shared-memory plan fits, else direct                            */
 #define PAB_VARIANT_DIRECT 1   /* per-thread gathers through L1/L2 from the staged RF copy, no shared memory      */
@@ -104,6 +108,12 @@ int pab_set_input(pab_ctx* ctx, int dtype, float scale);
  */
 int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz, int n_taps_bp,
                  int n_taps_hilbert, float dyn_range_db);
+
+/* pab_set_weight -- coherence-factor weighting fused into the beamforming kernel ("can be combined
+ * with coherence based real-time weighting factors"; the paper gives no formula: DESIGN.md reading A20 takes the
+ * standard coherence factor over all N elements, out-of-record samples counting as zeros).  Default PAB_WEIGHT_NONE.
+ * With PAB_WEIGHT_CF a thread carries at most 8 frames (orders 1-3) or 4 frames (orders 4, 5). */
+int pab_set_weight(pab_ctx* ctx, int weight);
 
 /* pab_set_tuning -- override the plan's blocking (autotuning / experiments); 0 keeps the default of a field.
  *   frames_per_thread 4, 8 or 16;  stages 2..4;  chunk_channels 1..32 (clamped to what fits in shared memory);

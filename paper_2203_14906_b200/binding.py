@@ -16,12 +16,13 @@ OK, ERR_INVALID, ERR_DEVICE, ERR_ALLOC, ERR_CUDA = 0, -1, -2, -3, -4
 F32, I16 = 0, 1
 RAW, BANDPASS, ENVELOPE, LOG = 0, 1, 2, 3
 VARIANT_AUTO, VARIANT_DIRECT, VARIANT_STAGED = 0, 1, 2
+WEIGHT_NONE, WEIGHT_CF = 0, 1
 STAGES = ["ingest", "beamform", "post_fir", "post_log"]
 _MODES = {"raw": RAW, "bandpass": BANDPASS, "envelope": ENVELOPE, "log": LOG}
 _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_STAGED}
 
 # every symbol include/pab.h declares
-SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
+SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
            "pab_launch_count", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
@@ -64,6 +65,7 @@ def load(build_if_missing: bool = False):
     L.pab_set_input.argtypes = [vp, ip, fp]
     L.pab_set_post.argtypes = [vp, ip, fp, fp, ip, ip, fp]
     L.pab_set_variant.argtypes = [vp, ip]
+    L.pab_set_weight.argtypes = [vp, ip]
     L.pab_set_tuning.argtypes = [vp, ip, ip, ip, ip]
     L.pab_beamform.argtypes = [vp, vp, ip, ip, vp, vp]
     L.pab_beamform_host.argtypes = [vp, vp, ip, ip, vp]
@@ -130,7 +132,7 @@ class Beamformer:
     """pab_create / pab_set_* / pab_beamform / pab_destroy for one geometry on the current CUDA device."""
 
     def __init__(self, g, dtype: str = "float32", scale: float = 1.0, post: dict | None = None,
-                 variant: str = "auto"):
+                 variant: str = "auto", weight: str = "none"):
         self._L = load()
         self._h = C.c_void_p()
         self.geom = g
@@ -143,6 +145,8 @@ class Beamformer:
             self.set_post(**post)
         if variant != "auto":
             self.set_variant(variant)
+        if weight != "none":
+            self.set_weight(weight)
 
     def _check(self, rc, what):
         if rc != OK:
@@ -153,6 +157,9 @@ class Beamformer:
                  dyn_range_db=60.0):
         self._check(self._L.pab_set_post(self._h, _MODES[mode], f_center, f_halfwidth, n_taps_bp, n_taps_hilbert,
                                          dyn_range_db), "pab_set_post")
+
+    def set_weight(self, weight: str):
+        self._check(self._L.pab_set_weight(self._h, {"none": WEIGHT_NONE, "cf": WEIGHT_CF}[weight]), "pab_set_weight")
 
     def set_variant(self, variant: str):
         self._check(self._L.pab_set_variant(self._h, _VARIANTS[variant]), "pab_set_variant")

@@ -26,6 +26,7 @@ struct pab_ctx {
     bool post_fast = false;
     int hilbert_parity = 2;          // 0 / 1: only Hilbert taps of that index parity are non-zero; 2: dense
     int variant = PAB_VARIANT_AUTO;
+    int weight = PAB_WEIGHT_NONE;
     pab_plan_info plan{};
     PlanTuning tuning{};
     int device = 0, sm_count = 0, smem_optin = 0;
@@ -224,6 +225,12 @@ int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_ch
     ctx->tuning = t;
     ctx->plan = plan;
     if (ctx->variant == PAB_VARIANT_STAGED && plan.smem_bytes == 0) ctx->variant = PAB_VARIANT_AUTO;
+    return PAB_OK;
+}
+
+int pab_set_weight(pab_ctx* ctx, int weight) {
+    if (!ctx || (weight != PAB_WEIGHT_NONE && weight != PAB_WEIGHT_CF)) return PAB_ERR_INVALID;
+    ctx->weight = weight;
     return PAB_OK;
 }
 

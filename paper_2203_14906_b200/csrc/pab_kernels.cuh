@@ -25,6 +25,7 @@ struct BfParams {
     const float4* zrow;    // [nz]  (zs, zs^2, zf - 1/2, zi - 0x4B400000 as int bits), zs = z fs / c = zi + zf
     int N, S, Sp, nx, nz;
     int n_frames;          // valid frames in this launch (stores beyond are skipped)
+    float inv_n;           // 1 / N, for the coherence factor (row f1)
 };
 
 // ------------------------------------------------------------------------------------------------------
@@ -74,7 +75,7 @@ __global__ void __launch_bounds__(256) ingest_lin_kernel(const T* __restrict__ r
 constexpr int kDirectCols = 8;
 constexpr int kDirectRows = 32;
 
-template <int K, int NQ>
+template <int K, int NQ, int W>
 __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
     constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -83,11 +84,11 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
     const float2 xj = P.xj[min(j, P.nx - 1)];
     const float4 row = P.zrow[min(m, P.nz - 1)];
 
-    float p[NF][K];
+    float p[NF][kAcc<K, W>];
 #pragma unroll
     for (int f = 0; f < NF; ++f)
 #pragma unroll
-        for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+        for (int k = 0; k < kAcc<K, W>; ++k) p[f][k] = 0.0f;
 
     if constexpr (NQ == 0) {
         const float* chan = P.rf + (size_t)blockIdx.z * P.N * (size_t)P.Sp;
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
             const float xs = (xj.x - xe.x) + (xj.y - xe.y);
             const Tap t = delay_tap<false>(xs, xs * xs, row, P.S);
             const float s0 = __ldg(chan + t.i0), s1 = __ldg(chan + t.i0 + 1);
-            accumulate<K>(interp<false>(t, s0, s1), p[0]);
+            accumulate_w<K, W>(interp<false>(t, s0, s1), p[0]);
         }
     } else {
         const size_t quad_stride = (size_t)P.N * (size_t)P.S;      // float4 units
@@ -111,10 +112,10 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
             for (int q = 0; q < NQ; ++q) {
                 const float4 s0 = __ldg(chan + q * quad_stride + t.i0);
                 const float4 s1 = __ldg(chan + q * quad_stride + t.i0 + 1);
-                accumulate<K>(interp<false>(t, s0.x, s1.x), p[4 * q + 0]);
-                accumulate<K>(interp<false>(t, s0.y, s1.y), p[4 * q + 1]);
-                accumulate<K>(interp<false>(t, s0.z, s1.z), p[4 * q + 2]);
-                accumulate<K>(interp<false>(t, s0.w, s1.w), p[4 * q + 3]);
+                accumulate_w<K, W>(interp<false>(t, s0.x, s1.x), p[4 * q + 0]);
+                accumulate_w<K, W>(interp<false>(t, s0.y, s1.y), p[4 * q + 1]);
+                accumulate_w<K, W>(interp<false>(t, s0.z, s1.z), p[4 * q + 2]);
+                accumulate_w<K, W>(interp<false>(t, s0.w, s1.w), p[4 * q + 3]);
             }
         }
     }
@@ -124,7 +125,7 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
             const int frame = blockIdx.z * NF + f;
-            if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+            if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[f], P.inv_n);
         }
     }
 }

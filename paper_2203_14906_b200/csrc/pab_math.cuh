@@ -81,6 +81,32 @@ __device__ __forceinline__ float combine(const float (&p)[K]) {
     }
 }
 
+// Row f1 (reading A20): coherence-factor weighting, out = CF e_k with CF = (sum s)^2 / (N sum s^2).
+// W = 0: none; W = 1: CF.  The accumulator row of one frame is p[0..K-1] (the power sums) followed, for W = 1,
+// by sum s^2 and, for even K only (where p_K = sum |s|), by sum s: kAcc<K, W> floats.
+template <int K, int W> constexpr int kAcc = K + (W == 0 ? 0 : ((K & 1) ? 1 : 2));
+
+template <int K, int W>
+__device__ __forceinline__ void accumulate_w(float s, float (&p)[kAcc<K, W>]) {
+    accumulate<K>(s, reinterpret_cast<float (&)[K]>(p));
+    if constexpr (W == 1) {
+        p[K] = fmaf(s, s, p[K]);
+        if constexpr ((K & 1) == 0) p[K + 1] += s;
+    }
+}
+
+// inv_n = 1 / N.  sum s^2 = 0 (every sample zero or outside the record) gives CF = 0.
+template <int K, int W>
+__device__ __forceinline__ float combine_w(const float (&p)[kAcc<K, W>], float inv_n) {
+    const float e = combine<K>(reinterpret_cast<const float (&)[K]>(p));
+    if constexpr (W == 0) return e;
+    else {
+        const float sum = (K & 1) ? p[K - 1] : p[K + 1];
+        const float sq = p[K];
+        return sq > 0.0f ? e * (sum * sum * inv_n) * rcp_approx(sq) : 0.0f;
+    }
+}
+
 // Step a2 + the index half of a3, once per (pixel, element), shared by every frame a thread carries.
 //   xs   lateral offset pixel - element in samples, xs2 = xs^2
 //   row  (zs, zs^2, zf - 1/2, zi - 0x4B400000 as int bits) with zs = z fs / c = zi + zf, zi = floor(zs)

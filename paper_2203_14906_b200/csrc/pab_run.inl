@@ -30,27 +30,35 @@ void launch_ingest_lin(const void* rf, float* stage, int F, int N, int S, int Sp
     ingest_lin_kernel<T><<<grid, 256, 0, st>>>((const T*)rf, stage, N, S, Sp, scale);
 }
 
-template <int K, int NQ>
+template <int K, int NQ, int W>
 void launch_direct(const BfParams& P, int groups, cudaStream_t st) {
     dim3 grid((P.nx + kDirectCols - 1) / kDirectCols, (P.nz + kDirectRows - 1) / kDirectRows, groups);
-    bf_direct_kernel<K, NQ><<<grid, 256, 0, st>>>(P);
+    bf_direct_kernel<K, NQ, W><<<grid, 256, 0, st>>>(P);
 }
 
-template <int NQ>
-void launch_direct_order(int order, const BfParams& P, int groups, cudaStream_t st) {
+template <int NQ, int W>
+void launch_direct_order_w(int order, const BfParams& P, int groups, cudaStream_t st) {
     switch (order) {
-    case 1: launch_direct<1, NQ>(P, groups, st); break;
-    case 2: launch_direct<2, NQ>(P, groups, st); break;
-    case 3: launch_direct<3, NQ>(P, groups, st); break;
-    case 4: launch_direct<4, NQ>(P, groups, st); break;
-    default: launch_direct<5, NQ>(P, groups, st); break;
+    case 1: launch_direct<1, NQ, W>(P, groups, st); break;
+    case 2: launch_direct<2, NQ, W>(P, groups, st); break;
+    case 3: launch_direct<3, NQ, W>(P, groups, st); break;
+    case 4: launch_direct<4, NQ, W>(P, groups, st); break;
+    default: launch_direct<5, NQ, W>(P, groups, st); break;
     }
 }
 
-void launch_direct_nq(int order, int nq, const BfParams& P, int groups, cudaStream_t st) {
-    if (nq == 4) launch_direct_order<4>(order, P, groups, st);
-    else if (nq == 2) launch_direct_order<2>(order, P, groups, st);
-    else launch_direct_order<1>(order, P, groups, st);
+// nq = 0: lin layout, one frame per thread; 1, 2, 4 quads per thread (4 only without weighting)
+void launch_direct_nq(int order, int nq, int weight, const BfParams& P, int groups, cudaStream_t st) {
+    if (weight == 0) {
+        if (nq == 4) launch_direct_order_w<4, 0>(order, P, groups, st);
+        else if (nq == 2) launch_direct_order_w<2, 0>(order, P, groups, st);
+        else if (nq == 1) launch_direct_order_w<1, 0>(order, P, groups, st);
+        else launch_direct_order_w<0, 0>(order, P, groups, st);
+    } else {
+        if (nq == 2) launch_direct_order_w<2, 1>(order, P, groups, st);
+        else if (nq == 1) launch_direct_order_w<1, 1>(order, P, groups, st);
+        else launch_direct_order_w<0, 1>(order, P, groups, st);
+    }
 }
 
 // One batch (<= plan.batch_frames frames): ingest -> beamform -> post.  rf points at the batch's first frame
@@ -61,6 +69,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
     BfParams P{};
     P.xj = ctx->d_xj; P.xe = ctx->d_xe; P.zrow = ctx->d_zrow;
     P.N = N; P.S = S; P.Sp = ctx->Sp; P.nx = nx; P.nz = nz;
+    P.inv_n = 1.0f / (float)N;
+    const int weight = ctx->weight;
     P.out = post ? ctx->d_img : out;
     const bool in_range = ctx->plan.in_range != 0;
     const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
@@ -83,8 +93,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         P.n_frames = F;
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, 0, in_range, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
-            else launch_direct_order<0>(order, P, F, st);
+            if (use_staged) launch_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
+            else launch_direct_nq(order, 0, weight, P, F, st);
         }
     } else {
         {
@@ -97,6 +107,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         // orders 4 and 5 carry at most 8 frames per thread (16 x 5 accumulators would spill)
         int g0 = ctx->plan.frames_per_thread / 4;
         if (order >= 4 && g0 > 2) g0 = 2;
+        if (weight != 0) g0 = g0 > (order >= 4 ? 1 : 2) ? (order >= 4 ? 1 : 2) : g0;     // CF: +1..2 accumulators per frame
         for (int g = g0; g >= 1 && nq > 0; g >>= 1) {
             const int groups = nq / g;
             if (groups == 0) continue;
@@ -105,8 +116,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
-            else launch_direct_nq(order, g, R, groups, st);
+            if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
+            else launch_direct_nq(order, g, weight, R, groups, st);
             q0 += groups * g;
             nq -= groups * g;
         }

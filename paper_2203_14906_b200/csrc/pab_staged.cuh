@@ -76,7 +76,7 @@ struct StagedCfg {
 // Persistent: grid = min(#tiles, resident CTAs); CTA b takes tiles b, b + gridDim.x, ...  The full/empty ring
 // runs on across tiles, so the producer warp is already copying the next tile's first chunks while the
 // consumer warps finish the current tile and store its images.
-template <int K, int NQ, bool INR>
+template <int K, int NQ, bool INR, int W>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParams P, const StagedCfg C) {
     constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
     constexpr int BPS = NQ == 0 ? 4 : 16;              // bytes per staged sample
@@ -177,11 +177,11 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
         const int j = bx * kStgCols + col;
         const int m = by * kStgRows + (warp >> 3) * 32 + lane;
         const float4 row = P.zrow[min(m, P.nz - 1)];
-        float p[NF][K];
+        float p[NF][kAcc<K, W>];
 #pragma unroll
         for (int f = 0; f < NF; ++f)
 #pragma unroll
-            for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+            for (int k = 0; k < kAcc<K, W>; ++k) p[f][k] = 0.0f;
 
         for (int ck = 0; ck < n_chunks; ++ck) {
             mbar_wait(bar0 + 8 * s, ph);
@@ -201,16 +201,16 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
                 const uint32_t a = (uint32_t)base + i0 * BPS;
                 if constexpr (NQ == 0) {
                     const float s0 = lds32(a), s1 = lds32(a + 4);
-                    accumulate<K>(interp<INR>(t, s0, s1), p[0]);
+                    accumulate_w<K, W>(interp<INR>(t, s0, s1), p[0]);
                 } else {
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
                         const float4 s0 = lds128(a + q * quad_bytes);
                         const float4 s1 = lds128(a + q * quad_bytes + 16);
-                        accumulate<K>(interp<INR>(t, s0.x, s1.x), p[4 * q + 0]);
-                        accumulate<K>(interp<INR>(t, s0.y, s1.y), p[4 * q + 1]);
-                        accumulate<K>(interp<INR>(t, s0.z, s1.z), p[4 * q + 2]);
-                        accumulate<K>(interp<INR>(t, s0.w, s1.w), p[4 * q + 3]);
+                        accumulate_w<K, W>(interp<INR>(t, s0.x, s1.x), p[4 * q + 0]);
+                        accumulate_w<K, W>(interp<INR>(t, s0.y, s1.y), p[4 * q + 1]);
+                        accumulate_w<K, W>(interp<INR>(t, s0.z, s1.z), p[4 * q + 2]);
+                        accumulate_w<K, W>(interp<INR>(t, s0.w, s1.w), p[4 * q + 3]);
                     }
                 }
             }
@@ -224,30 +224,33 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
-                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[f], P.inv_n);
             }
         }
     }
 }
 
 // ---- host side ----
-template <int K, int NQ, bool INR>
+template <int K, int NQ, bool INR, int W>
 inline cudaError_t staged_set_attr(int smem_optin) {
-    return cudaFuncSetAttribute(bf_staged_kernel<K, NQ, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    return cudaFuncSetAttribute(bf_staged_kernel<K, NQ, INR, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
-template <int NQ, bool INR>
+template <int NQ, bool INR, int W>
 inline cudaError_t staged_set_attr_orders(int smem_optin) {
     cudaError_t e;
-    if ((e = staged_set_attr<1, NQ, INR>(smem_optin)) != cudaSuccess) return e;
-    if ((e = staged_set_attr<2, NQ, INR>(smem_optin)) != cudaSuccess) return e;
-    if ((e = staged_set_attr<3, NQ, INR>(smem_optin)) != cudaSuccess) return e;
-    if ((e = staged_set_attr<4, NQ, INR>(smem_optin)) != cudaSuccess) return e;
-    return staged_set_attr<5, NQ, INR>(smem_optin);
+    if ((e = staged_set_attr<1, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<2, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<3, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+    if ((e = staged_set_attr<4, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+    return staged_set_attr<5, NQ, INR, W>(smem_optin);
 }
 template <bool INR>
 inline bool staged_configure_inr(int smem_optin) {
-    return staged_set_attr_orders<0, INR>(smem_optin) == cudaSuccess && staged_set_attr_orders<1, INR>(smem_optin) == cudaSuccess &&
-           staged_set_attr_orders<2, INR>(smem_optin) == cudaSuccess && staged_set_attr_orders<4, INR>(smem_optin) == cudaSuccess;
+    // W = 1 (coherence factor) is instantiated for 1, 4 and 8 frames per thread only (run_batch caps the group)
+    return staged_set_attr_orders<0, INR, 0>(smem_optin) == cudaSuccess && staged_set_attr_orders<1, INR, 0>(smem_optin) == cudaSuccess &&
+           staged_set_attr_orders<2, INR, 0>(smem_optin) == cudaSuccess && staged_set_attr_orders<4, INR, 0>(smem_optin) == cudaSuccess &&
+           staged_set_attr_orders<0, INR, 1>(smem_optin) == cudaSuccess && staged_set_attr_orders<1, INR, 1>(smem_optin) == cudaSuccess &&
+           staged_set_attr_orders<2, INR, 1>(smem_optin) == cudaSuccess;
 }
 inline int staged_configure(int smem_optin) {
     return staged_configure_inr<false>(smem_optin) && staged_configure_inr<true>(smem_optin) ? PAB_OK : PAB_ERR_CUDA;
@@ -262,37 +265,44 @@ inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
     return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy;
 }
 
-template <int K, int NQ, bool INR>
+template <int K, int NQ, bool INR, int W>
 inline void launch_staged_k(const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
     const size_t smem = staged_smem_bytes(c, NQ);
     int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_staged_kernel<K, NQ, INR>, kStgThreads, smem) != cudaSuccess ||
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_staged_kernel<K, NQ, INR, W>, kStgThreads, smem) != cudaSuccess ||
         per_sm < 1) {
         cudaGetLastError();
         per_sm = 1;
     }
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups;
     const long long resident = (long long)sm_count * per_sm;
-    bf_staged_kernel<K, NQ, INR><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(P, c);
+    bf_staged_kernel<K, NQ, INR, W><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(P, c);
 }
-template <int NQ, bool INR>
+template <int NQ, bool INR, int W>
 inline void launch_staged_nq(int order, const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
     switch (order) {
-    case 1: launch_staged_k<1, NQ, INR>(P, c, sm_count, st); break;
-    case 2: launch_staged_k<2, NQ, INR>(P, c, sm_count, st); break;
-    case 3: launch_staged_k<3, NQ, INR>(P, c, sm_count, st); break;
-    case 4: launch_staged_k<4, NQ, INR>(P, c, sm_count, st); break;
-    default: launch_staged_k<5, NQ, INR>(P, c, sm_count, st); break;
+    case 1: launch_staged_k<1, NQ, INR, W>(P, c, sm_count, st); break;
+    case 2: launch_staged_k<2, NQ, INR, W>(P, c, sm_count, st); break;
+    case 3: launch_staged_k<3, NQ, INR, W>(P, c, sm_count, st); break;
+    case 4: launch_staged_k<4, NQ, INR, W>(P, c, sm_count, st); break;
+    default: launch_staged_k<5, NQ, INR, W>(P, c, sm_count, st); break;
     }
 }
 template <bool INR>
-inline void launch_staged_inr(int order, int nq, const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
-    if (nq == 0) launch_staged_nq<0, INR>(order, P, c, sm_count, st);
-    else if (nq == 1) launch_staged_nq<1, INR>(order, P, c, sm_count, st);
-    else if (nq == 2) launch_staged_nq<2, INR>(order, P, c, sm_count, st);
-    else launch_staged_nq<4, INR>(order, P, c, sm_count, st);
+inline void launch_staged_inr(int order, int nq, int weight, const BfParams& P, const StagedCfg& c, int sm_count,
+                              cudaStream_t st) {
+    if (weight == 0) {
+        if (nq == 0) launch_staged_nq<0, INR, 0>(order, P, c, sm_count, st);
+        else if (nq == 1) launch_staged_nq<1, INR, 0>(order, P, c, sm_count, st);
+        else if (nq == 2) launch_staged_nq<2, INR, 0>(order, P, c, sm_count, st);
+        else launch_staged_nq<4, INR, 0>(order, P, c, sm_count, st);
+    } else {
+        if (nq == 0) launch_staged_nq<0, INR, 1>(order, P, c, sm_count, st);
+        else if (nq == 1) launch_staged_nq<1, INR, 1>(order, P, c, sm_count, st);
+        else launch_staged_nq<2, INR, 1>(order, P, c, sm_count, st);
+    }
 }
-inline void launch_staged(int order, int nq, bool in_range, const BfParams& P, int groups, const pab_plan_info& plan,
+inline void launch_staged(int order, int nq, bool in_range, int weight, const BfParams& P, int groups, const pab_plan_info& plan,
                           int chunk_cap, int smem_limit, int sm_count, cudaStream_t st) {
     // the plan's chunk is sized for frames_per_thread / 4 quads per channel; fewer quads -> more channels per stage
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (long long)sizeof(ChanEntry);
@@ -303,8 +313,8 @@ inline void launch_staged(int order, int nq, bool in_range, const BfParams& P, i
     if (chunk < 1) chunk = 1;       // cannot happen: the plan fitted >= 1 channel at the largest nq
     StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
                 (P.nz + kStgRows - 1) / kStgRows, groups};
-    if (in_range) launch_staged_inr<true>(order, nq, P, c, sm_count, st);
-    else launch_staged_inr<false>(order, nq, P, c, sm_count, st);
+    if (in_range) launch_staged_inr<true>(order, nq, weight, P, c, sm_count, st);
+    else launch_staged_inr<false>(order, nq, weight, P, c, sm_count, st);
 }
 
 }  // namespace pab

@@ -26,8 +26,8 @@ def pab():
     return binding
 
 
-def run_gpu(pab, g, rf, order, variant="auto", dtype="float32", scale=1.0, post=None):
-    bf = pab.Beamformer(g, dtype=dtype, scale=scale, post=post, variant=variant)
+def run_gpu(pab, g, rf, order, variant="auto", dtype="float32", scale=1.0, post=None, weight="none"):
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, post=post, variant=variant, weight=weight)
     try:
         out = bf.beamform(torch.from_numpy(rf).cuda(), order)
         torch.cuda.synchronize()
@@ -244,3 +244,39 @@ def test_homogeneity_and_zero_channels_on_gpu(pab):
     z, _ = run_gpu(pab, w.geom, rf, 3)
     scale = np.max(np.abs(rf)) * 1.0
     assert np.max(np.abs(z)) <= 1e-5 * scale
+
+
+# ---- coherence-factor weighting (reading A20), fused into the beamforming kernel ----
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("order", [1, 2, 3, 4, 5])
+def test_cf_weighting_c1(pab, orc, variant, order):
+    w = synth.make_config("C1", n_frames=9)
+    ref = orc.beamform_ex(w.rf, w.geom, order, weight="cf")
+    for frames in (1, 4, 9):
+        gpu, _ = run_gpu(pab, w.geom, w.rf[:frames], order, variant, weight="cf")
+        for f in range(frames):
+            check_raw(gpu[f], ref[f], order)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cf_weighting_ragged_out_of_record(pab, orc, variant):
+    rng = np.random.default_rng(21)
+    g = synth.random_geometry(rng, 24, 514, 37, 129, in_range=False)
+    rf = rng.standard_normal((6, 24, 514)).astype(np.float32)
+    mask = edge_mask(orc, g)
+    for order in (2, 3):
+        gpu, _ = run_gpu(pab, g, rf, order, variant, weight="cf")
+        ref = orc.beamform_ex(rf, g, order, weight="cf")
+        for f in range(6):
+            check_raw(gpu[f], ref[f], order, mask)
+
+
+def test_cf_weighting_c2b_batch(pab, orc):
+    """Full-size grid, 24 frames (8 frames per thread with CF), order 3; two full frames against the oracle."""
+    w = synth.make_config("C2b", n_frames=24)
+    gpu, _ = run_gpu(pab, w.geom, w.rf, 3, weight="cf")
+    for f in (0, 23):
+        check_raw(gpu[f], orc.beamform_ex(w.rf[f:f + 1], w.geom, 3, weight="cf")[0], 3)
+    # all-zero frame: CF is defined as 0, the image must be exactly 0 (no NaN from 0/0)
+    z, _ = run_gpu(pab, w.geom, np.zeros_like(w.rf[:4]), 3, weight="cf")
+    assert np.all(z == 0.0)
