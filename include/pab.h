@@ -43,6 +43,10 @@ extern "C" {
 #define PAB_ENVELOPE 2   /* after band-pass and Hilbert-FIR envelope                                              */
 #define PAB_LOG      3   /* after band-pass, envelope and log compression, dB <= 0                                */
 
+/* delay handling (pab_set_interp) */
+#define PAB_INTERP_LINEAR  0   /* s_i = linear interpolation at the fractional delay index (A4); default           */
+#define PAB_INTERP_NEAREST 1   /* s_i = rf_i[floor(idx_i + 1/2)]: the literal integer-delay eq. (1) (A21)           */
+
 /* pixel weighting (pab_set_weight) */
 #define PAB_WEIGHT_NONE 0   /* out = e_k                                                                          */
 #define PAB_WEIGHT_CF   1   /* out = CF e_k, CF = (sum_i s_i)^2 / (N sum_i s_i^2), 0 when every s_i = 0             */
@@ -114,6 +118,14 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
  * standard coherence factor over all N elements, out-of-record samples counting as zeros).  Default PAB_WEIGHT_NONE.
  * With PAB_WEIGHT_CF a thread carries at most 8 frames (orders 1-3) or 4 frames (orders 4, 5). */
 int pab_set_weight(pab_ctx* ctx, int weight);
+
+/* pab_set_interp -- PAB_INTERP_NEAREST switches to the paper's literal eq. (1) (s_i[k + Delta_i] with an
+ * integer delay; reading A21): the delayed sample is the nearest RF sample, 0 outside the record.  The
+ * signed k-th root is then taken once per RF sample while the frames are staged and the integer delays come from a
+ * delay table in device memory (the paper's own arrangement), built here in fp64 with the oracle's
+ * expression: n_elem * nx * nz uint16 entries.  Synchronises the device on the first call.
+ * Errors: PAB_ERR_INVALID (n_samp > 65534, or combined with PAB_WEIGHT_CF), PAB_ERR_ALLOC, PAB_ERR_CUDA. */
+int pab_set_interp(pab_ctx* ctx, int interp);
 
 /* pab_set_tuning -- override the plan's blocking (autotuning / experiments); 0 keeps the default of a field.
  *   frames_per_thread 4, 8 or 16;  stages 2..4;  chunk_channels 1..32 (clamped to what fits in shared memory);

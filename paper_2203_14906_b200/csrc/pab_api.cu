@@ -10,6 +10,7 @@
 #include "pab_kernels.cuh"
 #include "pab_staged.cuh"
 #include "pab_post.cuh"
+#include "pab_nearest.cuh"
 
 using namespace pab;
 
@@ -27,6 +28,8 @@ struct pab_ctx {
     int hilbert_parity = 2;          // 0 / 1: only Hilbert taps of that index parity are non-zero; 2: dense
     int variant = PAB_VARIANT_AUTO;
     int weight = PAB_WEIGHT_NONE;
+    int interp = PAB_INTERP_LINEAR;
+    unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
     PlanTuning tuning{};
     int device = 0, sm_count = 0, smem_optin = 0;
@@ -71,7 +74,7 @@ size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
 
 void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
-    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max);
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near);
     for (int b = 0; b < 2; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -230,7 +233,29 @@ int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_ch
 
 int pab_set_weight(pab_ctx* ctx, int weight) {
     if (!ctx || (weight != PAB_WEIGHT_NONE && weight != PAB_WEIGHT_CF)) return PAB_ERR_INVALID;
+    if (weight == PAB_WEIGHT_CF && ctx->interp == PAB_INTERP_NEAREST) return PAB_ERR_INVALID;
     ctx->weight = weight;
+    return PAB_OK;
+}
+
+int pab_set_interp(pab_ctx* ctx, int interp) {
+    if (!ctx || (interp != PAB_INTERP_LINEAR && interp != PAB_INTERP_NEAREST)) return PAB_ERR_INVALID;
+    if (interp == PAB_INTERP_NEAREST) {
+        if (ctx->weight != PAB_WEIGHT_NONE || ctx->S > 65534) return PAB_ERR_INVALID;
+        if (!ctx->d_near) {
+            const size_t n = (size_t)ctx->N * ctx->grid.nx * (size_t)ctx->grid.nz;
+            PAB_CUDA(ctx, cudaMalloc(&ctx->d_near, n * sizeof(unsigned short)));
+            NearestGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
+                          (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz};
+            dim3 grid((ctx->grid.nz + 255) / 256, ctx->grid.nx, ctx->N);
+            if (grid.y > 65535u || grid.z > 65535u) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return PAB_ERR_INVALID; }
+            nearest_table_kernel<<<grid, 256>>>(G, ctx->d_near);
+            ctx->launches++;
+            cudaError_t e = cudaDeviceSynchronize();
+            if (e != cudaSuccess) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return cuda_fail(ctx, e, "nearest table"); }
+        }
+    }
+    ctx->interp = interp;
     return PAB_OK;
 }
 

@@ -76,7 +76,31 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
     const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
                             (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0 && staged_available());
 
-    if (F < 4) {
+    if (ctx->interp == PAB_INTERP_NEAREST) {
+        // row f4: rooted quad staging, then the table-driven gather kernel (always the quad layout)
+        {
+            Span sp(ctx, PAB_STAGE_INGEST, st);
+            if (ctx->dtype == PAB_I16) launch_ingest_root_quad<int16_t>(order, rf, ctx->d_stage, F, N, S, ctx->scale, st);
+            else launch_ingest_root_quad<float>(order, rf, ctx->d_stage, F, N, S, ctx->scale, st);
+        }
+        int nq = (F + 3) / 4, q0 = 0;
+        int g0 = ctx->plan.frames_per_thread / 4;
+        if (order >= 4 && g0 > 2) g0 = 2;
+        for (int g = g0; g >= 1 && nq > 0; g >>= 1) {
+            const int groups = nq / g;
+            if (groups == 0) continue;
+            BfParams R = P;
+            R.rf = ctx->d_stage + (size_t)q0 * N * (size_t)S * 4;
+            R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
+            R.n_frames = F - 4 * q0;
+            Span sp(ctx, PAB_STAGE_BEAMFORM, st);
+            if (use_staged) launch_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.chunk_channels,
+                                                  ctx->smem_optin, ctx->sm_count, ctx->d_near, st);
+            else launch_nearest_direct(order, g, R, groups, ctx->d_near, st);
+            q0 += groups * g;
+            nq -= groups * g;
+        }
+    } else if (F < 4) {
         // lin layout, one frame per thread.  fp32 input with unit scale and 16-byte rows is read in place.
         const bool in_place = ctx->dtype == PAB_F32 && ctx->scale == 1.0f && (S % 4) == 0 &&
                               ((uintptr_t)rf % 16) == 0;

@@ -26,8 +26,8 @@ def pab():
     return binding
 
 
-def run_gpu(pab, g, rf, order, variant="auto", dtype="float32", scale=1.0, post=None, weight="none"):
-    bf = pab.Beamformer(g, dtype=dtype, scale=scale, post=post, variant=variant, weight=weight)
+def run_gpu(pab, g, rf, order, variant="auto", dtype="float32", scale=1.0, post=None, weight="none", interp="linear"):
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, post=post, variant=variant, weight=weight, interp=interp)
     try:
         out = bf.beamform(torch.from_numpy(rf).cuda(), order)
         torch.cuda.synchronize()
@@ -280,3 +280,71 @@ def test_cf_weighting_c2b_batch(pab, orc):
     # all-zero frame: CF is defined as 0, the image must be exactly 0 (no NaN from 0/0)
     z, _ = run_gpu(pab, w.geom, np.zeros_like(w.rf[:4]), 3, weight="cf")
     assert np.all(z == 0.0)
+
+
+# ---- nearest-sample delays, the literal eq. (1) (reading A21) ----
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_nearest_integer_decisions_are_the_oracles_bit_exact(pab, orc, variant):
+    """RF = sample index on every channel, order 1: the image is sum_i round(idx_i), integers below 2^24, so fp32
+    sums are exact and the GPU image must equal the oracle's bit for bit: every integer delay decision
+    (including the out-of-record ones) is the oracle's."""
+    for cfg in ("C1", "C2"):
+        g = synth.geometry(cfg)
+        rf = np.tile(np.arange(g.n_samp, dtype=np.float32), (1, g.n_elem, 1))
+        gpu, _ = run_gpu(pab, g, rf, 1, variant, interp="nearest")
+        assert np.array_equal(gpu, orc.beamform_ex(rf, g, 1, interp="nearest"))
+    rng = np.random.default_rng(31)
+    g = synth.random_geometry(rng, 24, 514, 37, 129, in_range=False)          # runs past the end of the record
+    rf = np.tile(np.arange(g.n_samp, dtype=np.float32), (2, g.n_elem, 1))
+    gpu, _ = run_gpu(pab, g, rf, 1, variant, interp="nearest")
+    assert np.array_equal(gpu, orc.beamform_ex(rf, g, 1, interp="nearest"))
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("order", [1, 2, 3, 4, 5])
+def test_nearest_c1_all_orders_and_frame_counts(pab, orc, variant, order):
+    w = synth.make_config("C1", n_frames=19)
+    ref = orc.beamform_ex(w.rf, w.geom, order, interp="nearest")
+    for frames in (1, 4, 9, 19):
+        gpu, _ = run_gpu(pab, w.geom, w.rf[:frames], order, variant, interp="nearest")
+        for f in range(frames):
+            rel = check_raw(gpu[f], ref[f], order)
+            assert rel <= 2e-5          # no fp32 delay in this path: only fp32 roots and sums remain
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_nearest_ragged_int16_and_scale(pab, orc, variant):
+    rng = np.random.default_rng(33)
+    g = synth.random_geometry(rng, 33, 1001, 9, 70, in_range=False)
+    rf = rng.integers(-2000, 2000, (6, 33, 1001)).astype(np.int16)
+    for order, scale in ((3, 1.0), (2, 0.125), (5, 1.0)):
+        gpu, _ = run_gpu(pab, g, rf, order, variant, dtype="int16", scale=scale, interp="nearest")
+        ref = orc.beamform_ex(rf, g, order, interp="nearest", scale=scale)
+        for f in range(6):
+            check_raw(gpu[f], ref[f], order)
+
+
+def test_nearest_c2b_batch_and_post_chain(pab, orc):
+    w = synth.make_config("C2b", n_frames=20)
+    g = w.geom
+    gpu, _ = run_gpu(pab, g, w.rf, 3, interp="nearest")
+    for f in (0, 19):
+        check_raw(gpu[f], orc.beamform_ex(w.rf[f:f + 1], g, 3, interp="nearest")[0], 3)
+    post = dict(mode="envelope", f_center=10e6, f_halfwidth=2.5e6, n_taps_bp=64, n_taps_hilbert=63, dyn_range_db=60.0)
+    gpu, _ = run_gpu(pab, g, w.rf[:2], 3, interp="nearest", post=post)
+    ref = orc.post(orc.beamform_ex(w.rf[:2], g, 3, interp="nearest"), g, 10e6, 2.5e6, 64, 63, 60.0, mode="envelope")
+    assert np.sqrt(np.sum((gpu - ref) ** 2) / np.sum(ref ** 2)) <= 2e-4
+
+
+def test_nearest_rejects_unsupported_combinations(pab):
+    w = synth.make_config("C1")
+    bf = pab.Beamformer(w.geom, weight="cf")
+    try:
+        with pytest.raises(pab.PabError):
+            bf.set_interp("nearest")
+        bf.set_weight("none")
+        bf.set_interp("nearest")
+        with pytest.raises(pab.PabError):
+            bf.set_weight("cf")
+    finally:
+        bf.close()
