@@ -322,8 +322,10 @@ def run_sweep(args):
     cases = [("C1", 1, (1, 2, 3, 4, 5), False, "none"), ("C2", 1, (1, 2, 3), False, "none"),
              ("C2b", 64, (1, 2, 3), False, "none"), ("C2b", 64, (3,), False, "cf"), ("C3", 256, (3,), True, "none"),
              ("C4", 1, (4, 5), False, "none"), ("C4", 16, (4, 5), False, "none"), ("C4", 16, (5,), False, "cf"),
-             ("C5", 1024, (3,), True, "none")]
+             ("C5", 1024, (3,), True, "none"), ("C2b", 64, (1, 2, 3), False, "nearest"), ("C4", 16, (4, 5), False, "nearest")]
     for cfg, F, orders, post, weight in cases:
+        interp = "nearest" if weight == "nearest" else "linear"
+        weight = "none" if weight == "nearest" else weight
         gen = min(F, 64)
         w = synth.make_config(cfg, n_frames=gen)
         g = w.geom
@@ -332,7 +334,7 @@ def run_sweep(args):
         rf = torch.from_numpy(np.concatenate([w.rf] * (call_frames // gen), axis=0)).cuda()
         dtype = "int16" if w.rf.dtype == np.int16 else "float32"
         out = torch.empty((call_frames, g.nz, g.nx), dtype=torch.float32, device="cuda")
-        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None, weight=weight)
+        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None, weight=weight, interp=interp)
         items = g.nz * g.nx * g.n_elem
         for order in orders:
             reps = max(3, min(50, int(0.2 / max(1e-5, items * F * 1e-12))))
@@ -357,13 +359,17 @@ def run_sweep(args):
             share = min(fpt, F)                                  # frames sharing one delay computation (algorithmic: the batch)
             batch = min(F, 64)
             xu = _XU[order][0] + _XU[order][1] / batch
+            if interp == "nearest":          # no MUFU and no delay arithmetic in the hot loop; u, u^2.. accumulation only
+                xu = 0.0
             fp = _FP32[order][0] + _FP32[order][1] / batch + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
+            if interp == "nearest":
+                fp = {1: 1.0, 2: 3.0, 3: 4.0, 4: 5.0, 5: 7.0}[order]
             t_xu = items * F * xu / (SM_COUNT * XU_LANES_PER_CLK_SM * f_hz) * 1e3
             t_fp = items * F * fp / (SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz) * 1e3
             in_b = g.n_elem * g.n_samp * (2 if dtype == "int16" else 4)
             t_hbm = F * (in_b + g.nz * g.nx * 4) / (peaks["hbm_gbs"] * 1e9) * 1e3
             bf_ms = prof["beamform"][0] / reps
-            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw", "weight": weight,
+            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw", "weight": weight, "interp": interp,
                               "dtype_in": dtype, "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx,
                               "ms_per_stream": round(ms, 5), "frames_per_s": round(F / (ms * 1e-3), 1),
                               "items_per_s": round(items * F / (ms * 1e-3), 0),
@@ -376,6 +382,51 @@ def run_sweep(args):
         del rf, out
 
 
+# Paper Table II: ms per frame on a GeForce GT 730, DAS / DMAS / DMAS-3 / DMAS-4 / DMAS-5.  Context
+# only: the paper states neither N, S nor the precision (reading A19).
+_TABLE2_MS = {512: (2.912, 3.028, 3.309, 4.4, 5.133), 1024: (11.051, 11.6, 12.718, 17.121, 20.03),
+              2048: (43.438, 45.784, 50.205, 68.006, 79.653)}
+
+
+def run_table2(args):
+    """--table2: square pixel grids shaped like the paper's Table II (512^2, 1024^2, 2048^2), orders 1..5, 128
+    elements x 4096 samples, single frames and 16-frame batches, in both delay modes (nearest = the paper's own
+    integer-delay formulation with a delay table, linear = the interpolated path).  One JSON line per case."""
+    import torch
+    from paper_2203_14906_b200 import binding, synth
+    torch.cuda.set_device(0)
+    binding.load()
+    rng = np.random.default_rng(1020)
+    N, S, fs, c, pitch = 128, 4096, 40e6, 1540.0, 0.3e-3
+    rf16 = torch.from_numpy((rng.standard_normal((16, N, S)) * 0.3).astype(np.float32)).cuda()
+    for side in (512, 1024, 2048):
+        g = synth.Geometry(N, S, fs, c, pitch, side, side, -19.0e-3, 38.0e-3 / (side - 1), 5e-3, 60e-3 / (side - 1)).f32()
+        out = torch.empty((16, side, side), dtype=torch.float32, device="cuda")
+        for interp in ("nearest", "linear"):
+            bf = binding.Beamformer(g, interp=interp)
+            for F in (1, 16):
+                for order in (1, 2, 3, 4, 5):
+                    rf = rf16[:F]
+                    for _ in range(2):
+                        bf.beamform(rf, order, out=out[:F])
+                    torch.cuda.synchronize()
+                    reps = 5
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    for _ in range(reps):
+                        bf.beamform(rf, order, out=out[:F])
+                    e1.record()
+                    torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1) / reps / F
+                    print(json.dumps({"table2": f"{side}x{side}", "interp": interp, "order": order, "frames_per_call": F,
+                                      "n_elem": N, "n_samp": S, "ms_per_frame": round(ms, 5),
+                                      "frames_per_s": round(1e3 / ms, 1),
+                                      "items_per_s": round(side * side * N / (ms * 1e-3), 0),
+                                      "paper_gt730_ms_per_frame": _TABLE2_MS[side][order - 1]}), flush=True)
+            bf.close()
+        del out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -383,6 +434,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--table2", action="store_true", help="square grids shaped like the paper's Table II; 1 GPU")
     ap.add_argument("--sweep", action="store_true", help="per-config table (C1..C5), one JSON line each; 1 GPU")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -391,9 +443,9 @@ def main():
     if args.impl == "reference":
         run_reference(args, rank)
         return
-    if args.sweep:
+    if args.sweep or args.table2:
         if rank == 0:
-            run_sweep(args)
+            run_sweep(args) if args.sweep else run_table2(args)
         return
     if world != args.gpus and world == 1 and args.gpus > 1:
         raise SystemExit("bench.py --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU)")

@@ -243,11 +243,12 @@ int pab_set_interp(pab_ctx* ctx, int interp) {
     if (interp == PAB_INTERP_NEAREST) {
         if (ctx->weight != PAB_WEIGHT_NONE || ctx->S > 65534) return PAB_ERR_INVALID;
         if (!ctx->d_near) {
-            const size_t n = (size_t)ctx->N * ctx->grid.nx * (size_t)ctx->grid.nz;
+            const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z = (ctx->grid.nz + kStgRows - 1) / kStgRows;
+            const size_t n = (size_t)ctx->N * tiles_x * kStgCols * (size_t)tiles_z * kStgRows;
             PAB_CUDA(ctx, cudaMalloc(&ctx->d_near, n * sizeof(unsigned short)));
             NearestGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
                           (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz};
-            dim3 grid((ctx->grid.nz + 255) / 256, ctx->grid.nx, ctx->N);
+            dim3 grid((tiles_z * kStgRows + 255) / 256, tiles_x * kStgCols, ctx->N);
             if (grid.y > 65535u || grid.z > 65535u) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return PAB_ERR_INVALID; }
             nearest_table_kernel<<<grid, 256>>>(G, ctx->d_near);
             ctx->launches++;

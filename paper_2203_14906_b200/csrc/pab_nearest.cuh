@@ -7,8 +7,9 @@
 // is not taken in fp32: the paper's own data structure, a delay table in global memory ("all the
 // delays ... were calculated and stored in the GPU (global) memory"), is built once per geometry by an fp64
 // kernel that evaluates fs sqrt((x - xe)^2 + z^2) / c with individually rounded IEEE operations, and holds
-// n_i as uint16 (0xFFFF = outside the record), laid out [element][column][row] so a warp (lanes along depth)
-// reads 64 contiguous bytes per element.
+// n_i as uint16 (0xFFFF = outside the record), laid out tile-major, [tile row][tile column][element][8 columns][64
+// rows], so the 1 KB block one element contributes to one 64 x 8 pixel tile is contiguous: the producer warp brings
+// it into shared memory with one bulk copy next to that element's RF window.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -18,6 +19,7 @@
 namespace pab {
 
 constexpr unsigned short kNearestInvalid = 0xFFFFu;
+constexpr int kNearBlockBytes = kStgRows * kStgCols * 2;      // one element's delay-table block for one tile
 
 // geometry as the ABI carries it (floats), promoted to double unchanged -- the oracle does the same promotion
 struct NearestGeom {
@@ -25,20 +27,33 @@ struct NearestGeom {
     int N, S, nx, nz;
 };
 
-// table[(i * nx + j) * nz + m] = floor(idx + 1/2) or 0xFFFF.  grid: (ceil(nz/256), nx, N)
+// table[nearest_index(...)] = floor(idx + 1/2) or 0xFFFF.
+// grid: (ceil(nz_pad/256), nx_pad, N) with nz_pad, nx_pad the grid rounded up to whole tiles.
+__host__ __device__ __forceinline__ size_t nearest_index(int i, int j, int m, int N, int tiles_x) {
+    return ((((size_t)(m / kStgRows) * tiles_x + (size_t)(j / kStgCols)) * N + i) * kStgCols + (j % kStgCols)) * kStgRows + (m % kStgRows);
+}
 __global__ void __launch_bounds__(256) nearest_table_kernel(const NearestGeom G, unsigned short* __restrict__ table) {
     const int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, i = blockIdx.z;
-    if (m >= G.nz) return;
+    const int tiles_x = (G.nx + kStgCols - 1) / kStgCols, tiles_z = (G.nz + kStgRows - 1) / kStgRows;
+    if (m >= tiles_z * kStgRows) return;
     // every operation individually rounded (no fused multiply-add), in the order the definition is written
-    const double x = __dadd_rn(G.x0, __dmul_rn((double)j, G.dx));
-    const double z = __dadd_rn(G.z0, __dmul_rn((double)m, G.dz));
+    // padding pixels of edge tiles repeat the last real column / row, so their entries stay inside the tile's window
+    const int jc = min(j, G.nx - 1), mc = min(m, G.nz - 1);
+    const double x = __dadd_rn(G.x0, __dmul_rn((double)jc, G.dx));
+    const double z = __dadd_rn(G.z0, __dmul_rn((double)mc, G.dz));
     const double xe = __dmul_rn(__dsub_rn((double)i, __ddiv_rn(__dsub_rn((double)G.N, 1.0), 2.0)), G.pitch);
     const double ddx = __dsub_rn(x, xe);
     const double d = __dsqrt_rn(__dadd_rn(__dmul_rn(ddx, ddx), __dmul_rn(z, z)));
     const double idx = __ddiv_rn(__dmul_rn(G.fs, d), G.c);
     const double n = floor(__dadd_rn(idx, 0.5));
     const bool ok = n >= 0.0 && n <= (double)(G.S - 1);
-    table[((size_t)i * G.nx + j) * (size_t)G.nz + m] = ok ? (unsigned short)n : kNearestInvalid;
+    table[nearest_index(i, j, m, G.N, tiles_x)] = ok ? (unsigned short)n : kNearestInvalid;
+}
+
+__device__ __forceinline__ int lds_u16(uint32_t addr) {
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
+    return (int)v;
 }
 
 // signed k-th root of one RF sample, taken once while staging (accurate library roots: cost is per sample)
@@ -99,7 +114,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
     ChanEntry* tab = reinterpret_cast<ChanEntry*>(smem + 64);
     const int tab_bytes = (C.stages * C.chunk * (int)sizeof(ChanEntry) + 127) & ~127;
-    const uint32_t data0 = smem_u32(smem + 64 + tab_bytes);
+    const uint32_t ntab0 = smem_u32(smem + 64 + tab_bytes);             // [stages][chunk][8 cols][64 rows] uint16
+    const uint32_t data0 = ntab0 + C.stages * C.chunk * kNearBlockBytes;
     const int quad_bytes = C.window * BPS;
     const int slot_bytes = quad_bytes * NQ;
     const int stage_bytes = C.chunk * slot_bytes;
@@ -130,6 +146,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
             const float4 zf = P.zrow[r0], zl = P.zrow[rl];
             const float2 xa = P.xj[c0], xb = P.xj[min(c0 + kStgCols - 1, P.nx - 1)];
             const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)bz * NQ * grp_stride;
+            const char* tblk = reinterpret_cast<const char*>(table) + ((size_t)by * C.tiles_x + bx) * (size_t)P.N * kNearBlockBytes;
             for (int ck = 0; ck < n_chunks; ++ck) {
                 const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
                 mbar_wait(empty, ph);
@@ -156,7 +173,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
                     for (int k = 0; k < 5; ++k) e.pad[k] = 0;
                     tab[s * C.chunk + lane] = e;
                     const uint32_t bytes = (uint32_t)len * BPS;
-                    mbar_arrive_expect_tx(full, bytes * NQ);
+                    mbar_arrive_expect_tx(full, bytes * NQ + kNearBlockBytes);
+                    bulk_g2s(ntab0 + (s * C.chunk + lane) * kNearBlockBytes, tblk + (size_t)ch * kNearBlockBytes, kNearBlockBytes, full);
                     const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
 #pragma unroll
                     for (int q = 0; q < NQ; ++q)
@@ -171,14 +189,13 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
     }
 
     const int col = warp & 7;
-    const size_t tstride = (size_t)P.nx * (size_t)P.nz;         // table elements per channel
+    const uint32_t my = (uint32_t)((col * kStgRows + (warp >> 3) * 32 + lane) * 2);   // this pixel inside a table block
     int s = 0;
     uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int bx = tile % C.tiles_x, by = (tile / C.tiles_x) % C.tiles_z, bz = tile / (C.tiles_x * C.tiles_z);
         const int j = bx * kStgCols + col;
         const int m = by * kStgRows + (warp >> 3) * 32 + lane;
-        const unsigned short* tp = table + (size_t)min(j, P.nx - 1) * P.nz + min(m, P.nz - 1);
         float p[NF][K];
 #pragma unroll
         for (int f = 0; f < NF; ++f)
@@ -187,13 +204,12 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
 
         for (int ck = 0; ck < n_chunks; ++ck) {
             const int nch = min(C.chunk, P.N - ck * C.chunk);
-            // the table entries of this chunk do not depend on the staged data: fetch them before waiting
-            const unsigned short* tc = tp + (size_t)(ck * C.chunk) * tstride;
             mbar_wait(bar0 + 8 * s, ph);
             const uint32_t tab_s = smem_u32(tab + s * C.chunk);
+            const uint32_t ntab_s = ntab0 + s * C.chunk * kNearBlockBytes + my;
 #pragma unroll 4
             for (int l = 0; l < nch; ++l) {
-                int n = __ldg(tc + (size_t)l * tstride);
+                int n = lds_u16(ntab_s + l * kNearBlockBytes);
                 const int base = __float_as_int(lds32(tab_s + l * 64 + 32));
                 bool ok = true;
                 if constexpr (!INR) {
@@ -239,8 +255,9 @@ __global__ void __launch_bounds__(256) bf_nearest_direct_kernel(const BfParams P
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int j = blockIdx.x * kDirectCols + warp;
     const int m = blockIdx.y * kDirectRows + lane;
-    const size_t tstride = (size_t)P.nx * (size_t)P.nz;
-    const unsigned short* tp = table + (size_t)min(j, P.nx - 1) * P.nz + min(m, P.nz - 1);
+    const int tiles_x = (P.nx + kStgCols - 1) / kStgCols;
+    const size_t tstride = (size_t)kStgCols * kStgRows;        // table entries between consecutive elements of a tile
+    const unsigned short* tp = table + nearest_index(0, min(j, P.nx - 1), min(m, P.nz - 1), P.N, tiles_x);
     float p[NF][K];
 #pragma unroll
     for (int f = 0; f < NF; ++f)
@@ -277,7 +294,7 @@ __global__ void __launch_bounds__(256) bf_nearest_direct_kernel(const BfParams P
 template <int K, int NQ, bool INR>
 inline void launch_nearest_staged_k(const BfParams& P, const StagedCfg& c, const unsigned short* table, int sm_count,
                                     int smem_optin, cudaStream_t st) {
-    const size_t smem = staged_smem_bytes(c, NQ);
+    const size_t smem = staged_smem_bytes(c, NQ) + (size_t)c.stages * c.chunk * kNearBlockBytes;
     static bool configured = false;      // per instantiation; the attribute is per function, idempotent
     if (!configured) {
         cudaFuncSetAttribute(bf_nearest_staged_kernel<K, NQ, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
@@ -307,7 +324,7 @@ inline void launch_nearest_staged_inr(int order, int nq, const BfParams& P, cons
 // nq = 1, 2 or 4 quads per thread (4 only for orders <= 3)
 inline void launch_nearest_staged(int order, int nq, bool in_range, const BfParams& P, int groups, const pab_plan_info& plan,
                                   int chunk_cap, int smem_limit, int sm_count, const unsigned short* table, cudaStream_t st) {
-    const long long slot = (long long)plan.window_samples * 16 * nq + (long long)sizeof(ChanEntry);
+    const long long slot = (long long)plan.window_samples * 16 * nq + (long long)sizeof(ChanEntry) + kNearBlockBytes;
     long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
     if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
     if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
