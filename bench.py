@@ -47,6 +47,7 @@ METRIC = "beamformed frames/s, order-3 DMAS, 128ch (C2b: 128 el x 2048 samp x 10
 XU_PER_ITEM = 2.0 + 1.0 / FRAMES
 FP32_PER_ITEM = 6.0 + 3.0 / FRAMES
 SM_COUNT = 148
+NCU_TRAFFIC_BYTES = 47_247_872 + 20_565_504   # per 64-frame launch; profiles/r1_beamform_ncu_b.md
 XU_LANES_PER_CLK_SM = 16
 FP32_LANES_PER_CLK_SM = 128
 
@@ -267,7 +268,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         achieved = items_per_launch * XU_PER_ITEM / (bf_launch_ms * 1e-3)
         roofline = {"bound": "alu", "kernel": "bf_staged_kernel<3,4,true> (fused delay+interp+root+power sums+Newton, 16 frames per thread)",
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
-                    "frac": achieved / xu_peak, "traffic": None,
+                    "frac": achieved / xu_peak, "traffic": NCU_TRAFFIC_BYTES,
+                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
+                                      "kernel at this workload: profiles/r1_beamform_ncu_b.md",
                     "peak_source": f"148 SM x 16 XU lanes/clk x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, "
                                    f"{peaks['source']}); DESIGN.md Roofline",
                     "launch_ms": bf_launch_ms, "launches_timed": bf_n,
