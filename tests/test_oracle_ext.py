@@ -98,3 +98,31 @@ def test_nearest_out_of_record_is_zero(orc):
     img = orc.beamform_ex(rf, g, 1, interp="nearest")[0]
     inside = (orc.nearest_index(g) >= 0).sum(-1)
     assert np.array_equal(img, inside.astype(np.float64)) and inside.min() < g.n_elem
+
+
+# ---- row f2: orders above 5 ("this can be done for higher orders as well") ----
+@pytest.mark.parametrize("k", [6, 7, 8])
+def test_high_orders_recurrence_equals_definition(orc, k):
+    """Route B (the reference for the GPU) against route A, the definition: all k-subsets, signed k-th root of the
+    product of the un-rooted samples, the pattern of eqs. (2), (4)-(6) continued."""
+    import itertools
+    rng = np.random.default_rng(60 + k)
+    for n in (k, k + 1, 11):
+        s = rng.standard_normal(n) * 10.0 ** rng.uniform(-2, 2)
+        a = orc.combine(s, k, route=orc.ROUTE_BRUTE)
+        b = orc.combine(s, k, route=orc.ROUTE_RECUR)
+        py = sum(math.copysign(abs(math.prod(c)) ** (1.0 / k), math.prod(c)) for c in itertools.combinations(s, k))
+        assert a == pytest.approx(py, rel=1e-11, abs=1e-12 * abs(py))
+        assert b == pytest.approx(a, rel=1e-10, abs=1e-11 * np.max(np.abs(s)) * math.comb(n, k))
+    # fewer than k non-zero samples: exactly zero; constant samples: C(n, k) a or C(n, k) |a|
+    z = np.zeros(12); z[:k - 1] = rng.standard_normal(k - 1)
+    assert orc.combine(z, k) == 0.0
+    c = np.full(13, -1.75)
+    assert orc.combine(c, k) == pytest.approx(math.comb(13, k) * (-1.75 if k % 2 else 1.75), rel=1e-12)
+
+
+@pytest.mark.parametrize("k", [6, 8])
+def test_high_orders_image_homogeneity(orc, c1, k):
+    img = orc.beamform(c1.rf[:1], c1.geom, k)
+    twice = orc.beamform((-2.0 * c1.rf[:1]).astype(np.float32), c1.geom, k)
+    assert np.allclose(twice, 2.0 * img, rtol=1e-10, atol=1e-12 * np.abs(img).max())        # even k: x |alpha|
