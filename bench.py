@@ -309,8 +309,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
 
 
 # XU (MUFU) lane-ops and FP32-pipe slots per item, by order: (per item, per (pixel, element)) -- DESIGN.md Roofline
-_XU = {1: (0.0, 1.0), 2: (1.0, 1.0), 3: (2.0, 1.0), 4: (2.0, 1.0), 5: (2.0, 1.0)}
-_FP32 = {1: (3.0, 3.0), 2: (4.0, 3.0), 3: (6.0, 3.0), 4: (7.0, 3.0), 5: (9.0, 3.0)}
+_XU = {1: (0.0, 1.0), 2: (1.0, 1.0), 3: (2.0, 1.0), 4: (2.0, 1.0), 5: (2.0, 1.0), 6: (2.0, 1.0), 7: (2.0, 1.0), 8: (2.0, 1.0)}
+_FP32 = {1: (3.0, 3.0), 2: (4.0, 3.0), 3: (6.0, 3.0), 4: (7.0, 3.0), 5: (9.0, 3.0), 6: (14.0, 3.0), 7: (16.0, 3.0),
+         8: (18.0, 3.0)}
 
 
 def run_sweep(args):
@@ -325,7 +326,7 @@ def run_sweep(args):
     cases = [("C1", 1, (1, 2, 3, 4, 5), False, "none"), ("C2", 1, (1, 2, 3), False, "none"),
              ("C2b", 64, (1, 2, 3), False, "none"), ("C2b", 64, (3,), False, "cf"), ("C3", 256, (3,), True, "none"),
              ("C4", 1, (4, 5), False, "none"), ("C4", 16, (4, 5), False, "none"), ("C4", 16, (5,), False, "cf"),
-             ("C5", 1024, (3,), True, "none"), ("C2b", 64, (1, 2, 3), False, "nearest"), ("C4", 16, (4, 5), False, "nearest")]
+             ("C5", 1024, (3,), True, "none"), ("C2b", 64, (6, 8), False, "none"), ("C2b", 64, (1, 2, 3), False, "nearest"), ("C4", 16, (4, 5), False, "nearest")]
     for cfg, F, orders, post, weight in cases:
         interp = "nearest" if weight == "nearest" else "linear"
         weight = "none" if weight == "nearest" else weight
@@ -357,6 +358,8 @@ def run_sweep(args):
             fpt = bf.plan()["frames_per_thread"] if F >= 4 else 1
             if order >= 4:
                 fpt = min(fpt, 8)
+            if order >= 6:
+                fpt = min(fpt, 4)
             if weight == "cf":
                 fpt = min(fpt, 4 if order >= 4 else 8)
             share = min(fpt, F)                                  # frames sharing one delay computation (algorithmic: the batch)

@@ -28,7 +28,8 @@ extern "C" {
 #endif
 
 #define PAB_OK            0
-#define PAB_ERR_INVALID  (-1)   /* null pointer, non-positive size, order outside 1..5, misaligned pointer        */
+#define PAB_ERR_INVALID  (-1)   /* null pointer, non-positive size, order outside 1..8, misaligned pointer        */
+#define PAB_MAX_ORDER 8
 #define PAB_ERR_DEVICE   (-2)   /* no CUDA device, or the current device is not compute capability 10.x           */
 #define PAB_ERR_ALLOC    (-3)   /* device or pinned-host allocation failed                                        */
 #define PAB_ERR_CUDA     (-4)   /* a CUDA call or kernel launch failed (see pab_last_cuda_error)                  */
@@ -144,7 +145,8 @@ int pab_set_variant(pab_ctx* ctx, int variant);
  *              pab_set_input; aligned to its element size; read only; caller keeps it alive until the
  *              stream work finishes
  *   n_frames   >= 1; frames are independent; the library batches them internally
- *   order      k = 1..5 (1 = DAS eq. 1, 2 = DMAS eq. 3, 3..5 = eqs. 7, 8, 9)
+ *   order      k = 1..5 (1 = DAS eq. 1, 2 = DMAS eq. 3, 3..5 = eqs. 7, 8, 9); k = 6..8 (row f2: the same power-sum
+ *              scheme continued) with linear interpolation and no weighting only
  *   out_dev    device pointer, [n_frames][nz][nx], x fastest, fp32, 4-byte aligned; fully overwritten
  *   cuda_stream a cudaStream_t passed as void*; NULL = the legacy default stream
  * One context must not be used from two streams at once (shared scratch).

@@ -47,8 +47,7 @@ __device__ __forceinline__ void accumulate(float s, float (&p)[K]) {
         p[1] += u2;
         p[2] = fmaf(u2, u, p[2]);
         p[3] += fabsf(s);
-    } else {
-        static_assert(K == 5, "orders 1..5");
+    } else if constexpr (K == 5) {
         const float r = ex2_approx(lg2_approx(fabsf(s)) * 0.2f);
         const float u = copy_sign(r, s);                      // eq. (9): real fifth root (A3)
         const float u2 = r * r;
@@ -57,6 +56,19 @@ __device__ __forceinline__ void accumulate(float s, float (&p)[K]) {
         p[2] = fmaf(u2, u, p[2]);
         p[3] = fmaf(u2, u2, p[3]);
         p[4] += s;
+    } else {
+        // Row f2, orders above 5 ("this can be done for higher orders as well"): the same scheme,
+        // p_m += u^m for m < K and p_K += s (odd K) or |s| (even K).
+        static_assert(K >= 6 && K <= 8, "orders 1..8");
+        const float r = ex2_approx(lg2_approx(fabsf(s)) * (1.0f / (float)K));
+        const float u = copy_sign(r, s);
+        float pw = u;
+#pragma unroll
+        for (int m = 0; m < K - 1; ++m) {
+            p[m] += pw;
+            pw *= u;
+        }
+        p[K - 1] += (K & 1) ? s : fabsf(s);
     }
 }
 
@@ -75,7 +87,20 @@ __device__ __forceinline__ float combine(const float (&p)[K]) {
             else {
                 const float e4 = 0.25f * ((fmaf(e3, p[0], -e2 * p[1]) + e1 * p[2]) - p[3]);
                 if constexpr (K == 4) return e4;
-                else return 0.2f * (((fmaf(e4, p[0], -e3 * p[1]) + e2 * p[2]) - e1 * p[3]) + p[4]);
+                else if constexpr (K == 5) return 0.2f * (((fmaf(e4, p[0], -e3 * p[1]) + e2 * p[2]) - e1 * p[3]) + p[4]);
+                else {
+                    // orders 6..8: the recursion m e_m = sum_{i=1..m} (-1)^(i-1) e_{m-i} p_i written as a loop
+                    float e[K + 1];
+                    e[0] = 1.0f;
+#pragma unroll
+                    for (int m = 1; m <= K; ++m) {
+                        float acc = 0.0f;
+#pragma unroll
+                        for (int i = 1; i <= m; ++i) acc = (i & 1) ? fmaf(e[m - i], p[i - 1], acc) : fmaf(-e[m - i], p[i - 1], acc);
+                        e[m] = acc / (float)m;
+                    }
+                    return e[K];
+                }
             }
         }
     }

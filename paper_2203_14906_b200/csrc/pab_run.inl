@@ -43,7 +43,14 @@ void launch_direct_order_w(int order, const BfParams& P, int groups, cudaStream_
     case 2: launch_direct<2, NQ, W>(P, groups, st); break;
     case 3: launch_direct<3, NQ, W>(P, groups, st); break;
     case 4: launch_direct<4, NQ, W>(P, groups, st); break;
-    default: launch_direct<5, NQ, W>(P, groups, st); break;
+    case 5: launch_direct<5, NQ, W>(P, groups, st); break;
+    default:
+        if constexpr (NQ <= 1 && W == 0) {          // orders 6..8: at most 4 frames per thread, no weighting
+            if (order == 6) launch_direct<6, NQ, W>(P, groups, st);
+            else if (order == 7) launch_direct<7, NQ, W>(P, groups, st);
+            else launch_direct<8, NQ, W>(P, groups, st);
+        }
+        break;
     }
 }
 
@@ -131,6 +138,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         // orders 4 and 5 carry at most 8 frames per thread (16 x 5 accumulators would spill)
         int g0 = ctx->plan.frames_per_thread / 4;
         if (order >= 4 && g0 > 2) g0 = 2;
+        if (order >= 6) g0 = 1;
         if (weight != 0) g0 = g0 > (order >= 4 ? 1 : 2) ? (order >= 4 ? 1 : 2) : g0;     // CF: +1..2 accumulators per frame
         for (int g = g0; g >= 1 && nq > 0; g >>= 1) {
             const int groups = nq / g;
@@ -192,7 +200,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
 }
 
 int check_args(pab_ctx* ctx, const void* rf, int n_frames, int order, const float* out) {
-    if (!ctx || !rf || !out || n_frames < 1 || order < 1 || order > 5) return PAB_ERR_INVALID;
+    if (!ctx || !rf || !out || n_frames < 1 || order < 1 || order > PAB_MAX_ORDER) return PAB_ERR_INVALID;
+    if (order > 5 && (ctx->weight != PAB_WEIGHT_NONE || ctx->interp != PAB_INTERP_LINEAR)) return PAB_ERR_INVALID;
     if (((uintptr_t)rf % elem_size(ctx->dtype)) != 0 || ((uintptr_t)out % 4) != 0) return PAB_ERR_INVALID;
     return PAB_OK;
 }

@@ -242,6 +242,11 @@ inline cudaError_t staged_set_attr_orders(int smem_optin) {
     if ((e = staged_set_attr<2, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
     if ((e = staged_set_attr<3, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
     if ((e = staged_set_attr<4, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+    if constexpr (NQ <= 1 && W == 0) {
+        if ((e = staged_set_attr<6, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+        if ((e = staged_set_attr<7, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+        if ((e = staged_set_attr<8, NQ, INR, W>(smem_optin)) != cudaSuccess) return e;
+    }
     return staged_set_attr<5, NQ, INR, W>(smem_optin);
 }
 template <bool INR>
@@ -285,7 +290,14 @@ inline void launch_staged_nq(int order, const BfParams& P, const StagedCfg& c, i
     case 2: launch_staged_k<2, NQ, INR, W>(P, c, sm_count, st); break;
     case 3: launch_staged_k<3, NQ, INR, W>(P, c, sm_count, st); break;
     case 4: launch_staged_k<4, NQ, INR, W>(P, c, sm_count, st); break;
-    default: launch_staged_k<5, NQ, INR, W>(P, c, sm_count, st); break;
+    case 5: launch_staged_k<5, NQ, INR, W>(P, c, sm_count, st); break;
+    default:
+        if constexpr (NQ <= 1 && W == 0) {          // orders 6..8: at most 4 frames per thread, no weighting
+            if (order == 6) launch_staged_k<6, NQ, INR, W>(P, c, sm_count, st);
+            else if (order == 7) launch_staged_k<7, NQ, INR, W>(P, c, sm_count, st);
+            else launch_staged_k<8, NQ, INR, W>(P, c, sm_count, st);
+        }
+        break;
     }
 }
 template <bool INR>
