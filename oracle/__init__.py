@@ -160,6 +160,22 @@ def nearest_index(g) -> np.ndarray:
     return out
 
 
+METRIC_NAMES = ("mu_in", "mu_out", "sigma_out", "snr_db", "cr_db", "gcnr", "fwhm_m")
+
+
+def image_metrics(img, target, background, n_bins: int = 256, fwhm_row: int = -1, dx: float = 1.0) -> dict:
+    """Eqs. (10)-(12) + FWHM on one float32 image [nz][nx]; target / background = (r0, r1, c0, c1) (A22)."""
+    img = np.ascontiguousarray(img, dtype=np.float32)
+    nz, nx = img.shape
+    t = np.asarray(target, dtype=np.int32)
+    b = np.asarray(background, dtype=np.int32)
+    out = np.empty(7)
+    ip = C.POINTER(C.c_int)
+    lib().orc_image_metrics(img.ctypes.data_as(C.POINTER(C.c_float)), C.c_int(nz), C.c_int(nx), t.ctypes.data_as(ip),
+                            b.ctypes.data_as(ip), C.c_int(n_bins), C.c_int(fwhm_row), C.c_double(dx), _dptr(out))
+    return dict(zip(METRIC_NAMES, out.tolist()))
+
+
 def beamform_pixels(rf, g, order: int, pix, route: int = ROUTE_RECUR, scale=1.0) -> np.ndarray:
     """out[F][n_pix] at sampled pixels pix[n_pix][2] = (row m, column j)."""
     rf, dt = _rf(rf)

@@ -29,6 +29,8 @@
  *   orc_beamform_ex       interp = 0, weight = 0 == orc_beamform bitwise; nearest: numpy rint gather written
  *                         independently, staircase-RF closed form; CF: hand value 6/7 for (1,2,3), CF = 1 for equal
  *                         samples, 0 for +-a pairs, bounds [0,1], scale invariance, constant-RF closed form C(N,k) a
+ *   orc_image_metrics     numpy mean / std / histogram written independently; gCNR = 1 for disjoint and 0 for
+ *                         identical regions; SNR, CR of constant regions; FWHM of a sampled Gaussian = 2.3548 sigma
  *   orc_bandpass_taps     scipy.signal.firwin(scale=False) ; symmetry
  *   orc_hilbert_taps      antisymmetry, zero even taps, closed form 2/(pi t) * Hamming
  *   orc_fir_axial         numpy.convolve
@@ -323,6 +325,74 @@ void orc_nearest_index(int N, int S, double fs, double c, double pitch, const or
                 double n = floor(idx + 0.5);
                 n_out[((size_t)m * g->nx + j) * N + i] = (n >= 0.0 && n <= (double)(S - 1)) ? (int)n : -1;
             }
+}
+
+/* ---------------------------------------------------------------------------------------------------------
+ * image-quality metrics, eqs. (10)-(12) and FWHM.
+ * The image is the float32 array the beamformer delivers (envelope, linear scale); sums are in double.
+ * Readings A22: regions are pixel rectangles rows [r0, r1) x columns [c0, c1); sigma_out is the population
+ * standard deviation; gCNR's x is the amplitude divided by the largest amplitude of the two regions, binned into
+ * n_bins equal bins on [0, 1] (x = 1 in the last bin), the bin index decided in float32 arithmetic (the image's own
+ * precision) so that both implementations take the same integer decision; FWHM is measured on one image row inside
+ * the target's columns: width between the two half-maximum crossings next to the row's first maximum, crossings
+ * placed by linear interpolation, clipped to the region, in metres (pixels times dx).
+ * out[0..6] = mu_in, mu_out, sigma_out, SNR dB (eq. 10), CR dB (eq. 11), gCNR (eq. 12), FWHM m.
+ * ------------------------------------------------------------------------------------------------------- */
+void orc_image_metrics(const float* img, int nz, int nx, const int* tgt, const int* bkg, int n_bins, int fwhm_row,
+                       double dx, double* out) {
+    (void)nz;
+    double s_in = 0.0, s_out = 0.0;
+    float vmax = 0.0f;
+    long n_in = 0, n_out = 0;
+    for (int r = tgt[0]; r < tgt[1]; ++r)
+        for (int c = tgt[2]; c < tgt[3]; ++c) { float v = img[(size_t)r * nx + c]; s_in += v; ++n_in; if (v > vmax) vmax = v; }
+    for (int r = bkg[0]; r < bkg[1]; ++r)
+        for (int c = bkg[2]; c < bkg[3]; ++c) { float v = img[(size_t)r * nx + c]; s_out += v; ++n_out; if (v > vmax) vmax = v; }
+    double mu_in = s_in / (double)n_in, mu_out = s_out / (double)n_out, var = 0.0;
+    for (int r = bkg[0]; r < bkg[1]; ++r)
+        for (int c = bkg[2]; c < bkg[3]; ++c) { double d = (double)img[(size_t)r * nx + c] - mu_out; var += d * d; }
+    double sigma = sqrt(var / (double)n_out);
+    /* eq. (12): gCNR = 1 - sum_x min(h_i(x), h_o(x)) */
+    double* hi = (double*)calloc((size_t)n_bins, sizeof(double));
+    double* ho = (double*)calloc((size_t)n_bins, sizeof(double));
+    for (int pass = 0; pass < 2; ++pass) {
+        const int* R = pass == 0 ? tgt : bkg;
+        double* h = pass == 0 ? hi : ho;
+        for (int r = R[0]; r < R[1]; ++r)
+            for (int c = R[2]; c < R[3]; ++c) {
+                float v = img[(size_t)r * nx + c];
+                volatile float q = v / vmax;                    /* float32 division, then float32 product */
+                volatile float t = q * (float)n_bins;
+                int b = vmax > 0.0f ? (int)floorf(t) : 0;
+                if (b < 0) b = 0;
+                if (b > n_bins - 1) b = n_bins - 1;
+                h[b] += 1.0;
+            }
+    }
+    double ovl = 0.0;
+    for (int b = 0; b < n_bins; ++b) {
+        double a = hi[b] / (double)n_in, o = ho[b] / (double)n_out;
+        ovl += a < o ? a : o;
+    }
+    free(hi); free(ho);
+    /* FWHM on row fwhm_row, columns [c0, c1) of the target */
+    double fwhm = NAN;
+    if (fwhm_row >= 0) {
+        const float* p = img + (size_t)fwhm_row * nx;
+        int c0 = tgt[2], c1 = tgt[3], pk = c0;
+        for (int c = c0; c < c1; ++c) if (p[c] > p[pk]) pk = c;
+        double half = 0.5 * (double)p[pk], left = (double)c0, right = (double)(c1 - 1);
+        for (int c = pk; c > c0; --c)
+            if ((double)p[c - 1] < half) { left = (double)(c - 1) + (half - (double)p[c - 1]) / ((double)p[c] - (double)p[c - 1]); break; }
+        for (int c = pk; c < c1 - 1; ++c)
+            if ((double)p[c + 1] < half) { right = (double)c + ((double)p[c] - half) / ((double)p[c] - (double)p[c + 1]); break; }
+        fwhm = (right - left) * dx;
+    }
+    out[0] = mu_in; out[1] = mu_out; out[2] = sigma;
+    out[3] = 20.0 * log10(mu_in / sigma);        /* eq. (10) */
+    out[4] = 20.0 * log10(mu_in / mu_out);       /* eq. (11) */
+    out[5] = 1.0 - ovl;                          /* eq. (12) */
+    out[6] = fwhm;
 }
 
 /* ---------------------------------------------------------------------------------------------------------

@@ -126,3 +126,48 @@ def test_high_orders_image_homogeneity(orc, c1, k):
     img = orc.beamform(c1.rf[:1], c1.geom, k)
     twice = orc.beamform((-2.0 * c1.rf[:1]).astype(np.float32), c1.geom, k)
     assert np.allclose(twice, 2.0 * img, rtol=1e-10, atol=1e-12 * np.abs(img).max())        # even k: x |alpha|
+
+
+# ---- row f3: image-quality metrics, eqs. (10)-(12) and FWHM (reading A22) ----
+def test_metrics_against_numpy(orc):
+    rng = np.random.default_rng(70)
+    img = np.abs(rng.standard_normal((90, 70))).astype(np.float32)
+    img[20:40, 10:30] += 5.0
+    tgt, bkg = (20, 40, 10, 30), (50, 85, 35, 69)
+    m = orc.image_metrics(img, tgt, bkg, n_bins=64, fwhm_row=30, dx=0.25e-3)
+    a = img[20:40, 10:30].astype(np.float64)
+    b = img[50:85, 35:69].astype(np.float64)
+    assert m["mu_in"] == pytest.approx(a.mean(), rel=1e-13) and m["mu_out"] == pytest.approx(b.mean(), rel=1e-13)
+    assert m["sigma_out"] == pytest.approx(b.std(), rel=1e-12)
+    assert m["snr_db"] == pytest.approx(20 * np.log10(a.mean() / b.std()), rel=1e-12)          # eq. (10)
+    assert m["cr_db"] == pytest.approx(20 * np.log10(a.mean() / b.mean()), rel=1e-12)          # eq. (11)
+    vmax = max(a.max(), b.max())
+    ha, _ = np.histogram(a / vmax, bins=64, range=(0.0, 1.0))
+    hb, _ = np.histogram(b / vmax, bins=64, range=(0.0, 1.0))
+    gc = 1.0 - np.minimum(ha / a.size, hb / b.size).sum()
+    assert m["gcnr"] == pytest.approx(gc, abs=2.0 / min(a.size, b.size))   # bin edges: float32 here, float64 in numpy
+
+
+def test_metrics_closed_forms(orc):
+    img = np.full((40, 40), 2.0, dtype=np.float32)
+    img[:, 20:] = 0.5
+    img[::2, 20:] = 1.5                                      # background alternates 0.5 / 1.5: mean 1, std 0.5
+    m = orc.image_metrics(img, (0, 40, 0, 20), (0, 40, 20, 40), n_bins=16)
+    assert m["mu_in"] == 2.0 and m["mu_out"] == 1.0 and m["sigma_out"] == 0.5
+    assert m["snr_db"] == pytest.approx(20 * math.log10(4.0), rel=1e-14)
+    assert m["cr_db"] == pytest.approx(20 * math.log10(2.0), rel=1e-14)
+    assert m["gcnr"] == 1.0                                  # disjoint amplitude sets
+    same = orc.image_metrics(img, (0, 40, 20, 40), (0, 40, 20, 40), n_bins=16)
+    assert same["gcnr"] == 0.0 and same["cr_db"] == 0.0      # identical regions: full overlap
+    assert math.isnan(m["fwhm_m"])                           # no row asked for
+
+
+def test_fwhm_of_sampled_gaussian(orc):
+    x = np.arange(101, dtype=np.float64)
+    for sigma in (3.0, 7.5):
+        img = np.tile(np.exp(-0.5 * ((x - 48.3) / sigma) ** 2), (3, 1)).astype(np.float32)
+        m = orc.image_metrics(img, (0, 3, 0, 101), (0, 3, 0, 10), fwhm_row=1, dx=0.1e-3)
+        assert m["fwhm_m"] == pytest.approx(2.0 * math.sqrt(2.0 * math.log(2.0)) * sigma * 0.1e-3, rel=1e-2)   # linear interpolation of the crossings
+    tri = np.zeros((1, 21), dtype=np.float32)
+    tri[0, 5:16] = [0, 2, 4, 6, 8, 10, 8, 6, 4, 2, 0]       # triangle, peak 10 at column 10: half width = 5 columns
+    assert orc.image_metrics(tri, (0, 1, 0, 21), (0, 1, 0, 3), fwhm_row=0, dx=1.0)["fwhm_m"] == pytest.approx(5.0, rel=1e-14)
