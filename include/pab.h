@@ -201,6 +201,30 @@ long long pab_launch_count(const pab_ctx* ctx);
 int pab_set_profile(pab_ctx* ctx, int max_launches);
 int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset);
 
+/* Image-quality metrics of the paper's evaluation (SNR eq. 10, CR eq. 11, gCNR eq. 12, FWHM),
+ * SURVEY.md section 8(f) row f3, reading A22.  Regions are pixel rectangles. */
+typedef struct { int r0, r1, c0, c1; } pab_roi;          /* rows [r0, r1), columns [c0, c1), non-empty, inside the grid */
+typedef struct {
+    double mu_in, mu_out, sigma_out;                     /* means of the two regions, population std of the background */
+    double snr_db;                                       /* 20 log10(mu_in / sigma_out)                       eq. (10) */
+    double cr_db;                                        /* 20 log10(mu_in / mu_out)                          eq. (11) */
+    double gcnr;                                         /* 1 - sum_bins min(h_in, h_out), amplitudes / max   eq. (12) */
+    double fwhm_m;                                       /* half-maximum width on row fwhm_row, metres; NaN if row < 0 */
+} pab_metrics;
+
+/*
+ * pab_image_metrics -- the metrics of one image on the device.
+ *   img_dev    device pointer, [nz][nx] float32 (one frame of the context's grid; non-negative amplitudes, e.g. a
+ *              PAB_ENVELOPE output)
+ *   target, background   host pointers
+ *   n_bins     histogram bins of gCNR, 2..4096
+ *   fwhm_row   image row on which FWHM is measured inside the target's columns, or -1
+ *   out_host   host pointer, written on success
+ * Enqueues on cuda_stream and waits for it (the result goes to the host).  Errors: PAB_ERR_INVALID, PAB_ERR_CUDA.
+ */
+int pab_image_metrics(pab_ctx* ctx, const float* img_dev, const pab_roi* target, const pab_roi* background, int n_bins,
+                      int fwhm_row, pab_metrics* out_host, void* cuda_stream);
+
 /* pab_strerror -- static string for an error code.  pab_last_cuda_error -- the last cudaError_t string seen
  * by this context ("" if none). */
 const char* pab_strerror(int code);

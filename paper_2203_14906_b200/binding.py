@@ -25,7 +25,7 @@ _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_S
 # every symbol include/pab.h declares
 SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
-           "pab_launch_count", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
+           "pab_launch_count", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
 
 class Grid(C.Structure):
@@ -40,6 +40,14 @@ class PlanInfo(C.Structure):
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class Roi(C.Structure):
+    _fields_ = [("r0", C.c_int), ("r1", C.c_int), ("c0", C.c_int), ("c1", C.c_int)]
+
+
+class Metrics(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("mu_in", "mu_out", "sigma_out", "snr_db", "cr_db", "gcnr", "fwhm_m")]
 
 
 class PabError(RuntimeError):
@@ -79,6 +87,7 @@ def load(build_if_missing: bool = False):
     L.pab_design_hilbert.argtypes = [ip, C.POINTER(C.c_float)]
     L.pab_launch_count.argtypes = [vp]
     L.pab_launch_count.restype = C.c_longlong
+    L.pab_image_metrics.argtypes = [vp, vp, C.POINTER(Roi), C.POINTER(Roi), ip, ip, C.POINTER(Metrics), vp]
     L.pab_set_profile.argtypes = [vp, ip]
     L.pab_get_profile.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong), ip]
     L.pab_strerror.argtypes = [ip]
@@ -213,6 +222,17 @@ class Beamformer:
         st = torch.cuda.current_stream(rf.device) if stream is None else stream
         self._check(self._L.pab_beamform(self._h, rf.data_ptr(), F, order, out.data_ptr(), st.cuda_stream), "pab_beamform")
         return out
+
+    def image_metrics(self, img, target, background, n_bins: int = 256, fwhm_row: int = -1, stream=None) -> dict:
+        """pab_image_metrics on one CUDA image [nz][nx] float32; target / background = (r0, r1, c0, c1)."""
+        import torch
+        g = self.geom
+        assert img.is_cuda and img.is_contiguous() and img.dtype == torch.float32 and tuple(img.shape) == (g.nz, g.nx)
+        t, b, m = Roi(*map(int, target)), Roi(*map(int, background)), Metrics()
+        st = torch.cuda.current_stream(img.device) if stream is None else stream
+        self._check(self._L.pab_image_metrics(self._h, img.data_ptr(), C.byref(t), C.byref(b), n_bins, fwhm_row,
+                                              C.byref(m), st.cuda_stream), "pab_image_metrics")
+        return {k: getattr(m, k) for k, _ in Metrics._fields_}
 
     def beamform_host(self, rf, order: int, out=None):
         """rf: host array/tensor [F][N][S] (numpy or CPU torch, pinned or not) -> out: same kind, [F][nz][nx]."""

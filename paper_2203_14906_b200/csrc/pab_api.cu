@@ -11,6 +11,7 @@
 #include "pab_staged.cuh"
 #include "pab_post.cuh"
 #include "pab_nearest.cuh"
+#include "pab_metrics.cuh"
 
 using namespace pab;
 
@@ -29,6 +30,7 @@ struct pab_ctx {
     int variant = PAB_VARIANT_AUTO;
     int weight = PAB_WEIGHT_NONE;
     int interp = PAB_INTERP_LINEAR;
+    void* d_metric = nullptr;            // MetricAcc + double[1] + 2 x 4096 histogram bins (row f3), lazy
     unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
     PlanTuning tuning{};
@@ -74,7 +76,7 @@ size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
 
 void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
-    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near);
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric);
     for (int b = 0; b < 2; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -305,6 +307,50 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
     }
     ctx->post_mode = mode; ctx->n_taps_bp = n_taps_bp; ctx->n_taps_h = n_taps_hilbert;
     ctx->TpB = TpB; ctx->TpH = TpH; ctx->dyn_range_db = dyn_range_db;
+    return PAB_OK;
+}
+
+int pab_image_metrics(pab_ctx* ctx, const float* img_dev, const pab_roi* target, const pab_roi* background, int n_bins,
+                      int fwhm_row, pab_metrics* out_host, void* cuda_stream) {
+    if (!ctx || !img_dev || !target || !background || !out_host || n_bins < 2 || n_bins > 4096) return PAB_ERR_INVALID;
+    const int nz = ctx->grid.nz, nx = ctx->grid.nx;
+    auto bad = [&](const pab_roi* r) { return r->r0 < 0 || r->r1 > nz || r->c0 < 0 || r->c1 > nx || r->r0 >= r->r1 || r->c0 >= r->c1; };
+    if (bad(target) || bad(background) || fwhm_row >= nz) return PAB_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t acc_bytes = 64, hist_off = 128, total = hist_off + 2 * 4096 * sizeof(unsigned int);
+    if (!ctx->d_metric) PAB_CUDA(ctx, cudaMalloc(&ctx->d_metric, total));
+    char* base = (char*)ctx->d_metric;
+    MetricAcc* acc = (MetricAcc*)base;
+    double* fw = (double*)(base + acc_bytes);
+    unsigned int* hist = (unsigned int*)(base + hist_off);
+    PAB_CUDA(ctx, cudaMemsetAsync(base, 0, total, st));
+    RoiPair R{{target->r0, target->r1, target->c0, target->c1}, {background->r0, background->r1, background->c0, background->c1}};
+    dim3 grid(32, 2);
+    metrics_sum_kernel<<<grid, 256, 0, st>>>(img_dev, nx, R, acc);
+    metrics_hist_kernel<<<grid, 256, 0, st>>>(img_dev, nx, R, acc, hist, n_bins);
+    ctx->launches += 2;
+    if (fwhm_row >= 0) { metrics_fwhm_kernel<<<1, 32, 0, st>>>(img_dev, nx, fwhm_row, target->c0, target->c1, fw); ctx->launches++; }
+    MetricAcc h{};
+    double fwh = 0.0;
+    std::vector<unsigned int> hh(2 * (size_t)n_bins);
+    PAB_CUDA(ctx, cudaMemcpyAsync(&h, acc, sizeof h, cudaMemcpyDeviceToHost, st));
+    PAB_CUDA(ctx, cudaMemcpyAsync(&fwh, fw, sizeof fwh, cudaMemcpyDeviceToHost, st));
+    PAB_CUDA(ctx, cudaMemcpyAsync(hh.data(), hist, hh.size() * sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
+    PAB_CUDA(ctx, cudaStreamSynchronize(st));
+    const double n_in = (double)(target->r1 - target->r0) * (target->c1 - target->c0);
+    const double n_out = (double)(background->r1 - background->r0) * (background->c1 - background->c0);
+    pab_metrics m{};
+    m.mu_in = h.sum_in / n_in; m.mu_out = h.sum_out / n_out; m.sigma_out = std::sqrt(h.var_out / n_out);
+    m.snr_db = 20.0 * std::log10(m.mu_in / m.sigma_out);
+    m.cr_db = 20.0 * std::log10(m.mu_in / m.mu_out);
+    double ovl = 0.0;
+    for (int b = 0; b < n_bins; ++b) {
+        const double a = hh[b] / n_in, o = hh[n_bins + b] / n_out;
+        ovl += a < o ? a : o;
+    }
+    m.gcnr = 1.0 - ovl;
+    m.fwhm_m = fwhm_row >= 0 ? fwh * (double)ctx->grid.dx : std::nan("");
+    *out_host = m;
     return PAB_OK;
 }
 

@@ -259,6 +259,20 @@ def make_config(cfg: str, seed: int | None = None, n_frames: int | None = None) 
     raise ValueError(cfg)
 
 
+def simulation1_phantom(seed: int = 1101, n_frames: int = 1) -> Workload:
+    """A phantom laid out like the paper's Simulation 1: 128 elements, pitch 0.1 mm, 7.5 MHz,
+    fs 100 MHz, c 1500 m/s, ten point targets as five pairs 3 mm apart at depths 17, 20, 23, 26, 29 mm, white noise
+    at 30 dB (A16).  Stands in for the k-Wave data, which is not available; pulses are this module's analytic model."""
+    rng = np.random.default_rng(seed)
+    nx, nz = 128, 512
+    g = Geometry(128, 2560, 100e6, 1500.0, 0.1 * _MM, nx, nz, -5.0 * _MM, 10.0 * _MM / nx, 15.0 * _MM,
+                 16.0 * _MM / nz).f32()
+    base = [(sx * 1.5 * _MM, z * _MM, 1.0, 0.0) for z in (17, 20, 23, 26, 29) for sx in (-1.0, 1.0)]
+    rf, truth = _frames(rng, g, base, 7.5e6, n_frames, 30.0, False)
+    post = dict(mode="envelope", f_center=7.5e6, f_halfwidth=4.0e6, n_taps_bp=64, n_taps_hilbert=63, dyn_range_db=60.0)
+    return Workload("SIM1", g, rf, (1, 2, 3, 4, 5), 7.5e6, post, truth, seed)
+
+
 def point_target_frame(g: Geometry, ix: int, iz: int, f0: float = 5e6, shape: str = "n") -> np.ndarray:
     """Noiseless single point absorber on the centre of pixel (iz, ix); [1][N][S] float32 (pin P8).
 

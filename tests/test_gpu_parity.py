@@ -383,3 +383,58 @@ def test_high_orders_reject_weight_and_nearest(pab):
             bf.beamform(rf, 5)
         finally:
             bf.close()
+
+
+# ---- image-quality metrics on the device (eqs. 10-12, FWHM; reading A22) ----
+def _sim1_rois(g, depth_mm=23.0):
+    r = int(round((depth_mm * 1e-3 - g.z0) / g.dz))
+    c = int(round((-1.5e-3 - g.x0) / g.dx))                       # the left target of the pair
+    cb = int(round((4.0e-3 - g.x0) / g.dx))                       # background: same depth, 5.5 mm to the side
+    return (r - 10, r + 10, c - 8, c + 9), (r - 10, r + 10, cb - 8, cb + 9), r
+
+
+def test_metrics_device_matches_oracle_on_simulation1_phantom(pab, orc):
+    w = synth.simulation1_phantom()
+    g = w.geom
+    post = {k: v for k, v in w.post.items()}
+    res = {}
+    for order in (1, 3, 5):
+        bf = pab.Beamformer(g, post=post)
+        try:
+            img = bf.beamform(torch.from_numpy(w.rf).cuda(), order)[0].contiguous()
+            torch.cuda.synchronize()
+            # the peak row of the target inside its box: where FWHM is measured
+            tgt, bkg, r = _sim1_rois(g)
+            box = img[tgt[0]:tgt[1], tgt[2]:tgt[3]]
+            row = tgt[0] + int(torch.argmax(box.max(dim=1).values))
+            for n_bins in (64, 256):
+                got = bf.image_metrics(img, tgt, bkg, n_bins=n_bins, fwhm_row=row)
+                ref = orc.image_metrics(img.cpu().numpy(), tgt, bkg, n_bins=n_bins, fwhm_row=row, dx=g.dx)
+                for k in ("mu_in", "mu_out", "sigma_out", "snr_db", "cr_db", "fwhm_m"):
+                    assert got[k] == pytest.approx(ref[k], rel=1e-9), (order, k)
+                assert got["gcnr"] == pytest.approx(ref["gcnr"], abs=1e-12), order      # same integer bin decisions
+            res[order] = got
+        finally:
+            bf.close()
+    # the paper's qualitative claim on the synthetic phantom: contrast and SNR grow with the order,
+    # the main lobe narrows
+    assert res[5]["cr_db"] > res[3]["cr_db"] > res[1]["cr_db"]
+    assert res[5]["snr_db"] > res[1]["snr_db"]
+    assert res[5]["fwhm_m"] < res[1]["fwhm_m"]
+
+
+def test_metrics_argument_errors(pab):
+    w = synth.make_config("C1")
+    bf = pab.Beamformer(w.geom)
+    try:
+        img = torch.ones((w.geom.nz, w.geom.nx), device="cuda")
+        with pytest.raises(pab.PabError):
+            bf.image_metrics(img, (0, 0, 0, 4), (0, 4, 0, 4))                      # empty target
+        with pytest.raises(pab.PabError):
+            bf.image_metrics(img, (0, 4, 0, 4), (0, 4, 0, w.geom.nx + 1))          # outside the grid
+        with pytest.raises(pab.PabError):
+            bf.image_metrics(img, (0, 4, 0, 4), (0, 4, 0, 4), n_bins=1)
+        m = bf.image_metrics(img, (0, 4, 0, 4), (4, 8, 0, 4), n_bins=8)
+        assert m["mu_in"] == 1.0 and m["cr_db"] == 0.0 and m["gcnr"] == 0.0 and np.isnan(m["fwhm_m"])
+    finally:
+        bf.close()
