@@ -374,6 +374,9 @@ def run_sweep(args):
             t_fp = items * F * fp / (SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz) * 1e3
             in_b = g.n_elem * g.n_samp * (2 if dtype == "int16" else 4)
             t_hbm = F * (in_b + g.nz * g.nx * 4) / (peaks["hbm_gbs"] * 1e9) * 1e3
+            # secondary ceiling (not in the roofline denominator): shared-memory bandwidth, 128 B/clk/SM; the
+            # interpolated path gathers 2 x 4 bytes per item, the nearest-sample path 4
+            t_sm = items * F * (4.0 if interp == "nearest" else 8.0) / (SM_COUNT * 128.0 * f_hz) * 1e3
             bf_ms = prof["beamform"][0] / reps
             print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw", "weight": weight, "interp": interp,
                               "dtype_in": dtype, "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx,
@@ -382,6 +385,7 @@ def run_sweep(args):
                               "stage_ms": {k: round(v[0] / reps, 5) for k, v in prof.items()},
                               "beamform_launches": prof["beamform"][1] / reps, "frames_per_thread": share,
                               "t_roof_ms": {"xu": round(t_xu, 5), "fp32": round(t_fp, 5), "hbm": round(t_hbm, 5)},
+                              "t_smem_ceiling_ms": round(t_sm, 5),
                               "beamform_roofline_frac": round(max(t_xu, t_fp, t_hbm) / bf_ms, 4),
                               "in_range": bf.plan()["in_range"]}), flush=True)
         bf.close()

@@ -244,6 +244,7 @@ int pab_set_interp(pab_ctx* ctx, int interp) {
     if (!ctx || (interp != PAB_INTERP_LINEAR && interp != PAB_INTERP_NEAREST)) return PAB_ERR_INVALID;
     if (interp == PAB_INTERP_NEAREST) {
         if (ctx->weight != PAB_WEIGHT_NONE || ctx->S > 65534) return PAB_ERR_INVALID;
+        PAB_CUDA(ctx, nearest_configure(ctx->smem_optin));
         if (!ctx->d_near) {
             const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z = (ctx->grid.nz + kStgRows - 1) / kStgRows;
             const size_t n = (size_t)ctx->N * tiles_x * kStgCols * (size_t)tiles_z * kStgRows;

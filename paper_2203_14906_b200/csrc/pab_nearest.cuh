@@ -295,14 +295,34 @@ template <int K, int NQ, bool INR>
 inline void launch_nearest_staged_k(const BfParams& P, const StagedCfg& c, const unsigned short* table, int sm_count,
                                     int smem_optin, cudaStream_t st) {
     const size_t smem = staged_smem_bytes(c, NQ) + (size_t)c.stages * c.chunk * kNearBlockBytes;
-    static bool configured = false;      // per instantiation; the attribute is per function, idempotent
-    if (!configured) {
-        cudaFuncSetAttribute(bf_nearest_staged_kernel<K, NQ, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-        configured = true;
-    }
+    (void)smem_optin;
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups;
     bf_nearest_staged_kernel<K, NQ, INR><<<(unsigned)(tiles < sm_count ? tiles : sm_count), kStgThreads, smem, st>>>(P, c, table);
 }
+// opt in to the large dynamic shared memory for every instantiation on the current device (pab_set_interp)
+template <int K, bool INR>
+inline cudaError_t nearest_set_attr_k(int smem_optin) {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(bf_nearest_staged_kernel<K, 1, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_nearest_staged_kernel<K, 2, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if constexpr (K <= 3)
+        if ((e = cudaFuncSetAttribute(bf_nearest_staged_kernel<K, 4, INR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    return cudaSuccess;
+}
+template <bool INR>
+inline cudaError_t nearest_set_attr_inr(int smem_optin) {
+    cudaError_t e;
+    if ((e = nearest_set_attr_k<1, INR>(smem_optin)) != cudaSuccess) return e;
+    if ((e = nearest_set_attr_k<2, INR>(smem_optin)) != cudaSuccess) return e;
+    if ((e = nearest_set_attr_k<3, INR>(smem_optin)) != cudaSuccess) return e;
+    if ((e = nearest_set_attr_k<4, INR>(smem_optin)) != cudaSuccess) return e;
+    return nearest_set_attr_k<5, INR>(smem_optin);
+}
+inline cudaError_t nearest_configure(int smem_optin) {
+    cudaError_t e = nearest_set_attr_inr<true>(smem_optin);
+    return e != cudaSuccess ? e : nearest_set_attr_inr<false>(smem_optin);
+}
+
 template <int K, bool INR>
 inline void launch_nearest_staged_nq(int nq, const BfParams& P, const StagedCfg& c, const unsigned short* table,
                                      int sm_count, int smem_optin, cudaStream_t st) {
