@@ -438,3 +438,35 @@ def test_metrics_argument_errors(pab):
         assert m["mu_in"] == 1.0 and m["cr_db"] == 0.0 and m["gcnr"] == 0.0 and np.isnan(m["fwhm_m"])
     finally:
         bf.close()
+
+
+def test_beamform_is_cuda_graph_capturable(pab, orc):
+    """pab_beamform only enqueues work on the caller's stream (kernels + one memset), so a whole step can be captured
+    into a CUDA graph and replayed: the launch-bound tiny config C1 is where that pays."""
+    w = synth.make_config("C1", n_frames=8)
+    post = dict(mode="log", f_center=2.0e6, f_halfwidth=0.8e6, n_taps_bp=64, n_taps_hilbert=63, dyn_range_db=60.0)
+    bf = pab.Beamformer(w.geom, post=post)
+    try:
+        rf = torch.from_numpy(w.rf).cuda()
+        out = torch.empty((8, w.geom.nz, w.geom.nx), device="cuda")
+        eager = bf.beamform(rf, 3).clone()
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            bf.beamform(rf, 3, out=out, stream=s)            # warm-up on the side stream
+        torch.cuda.current_stream().wait_stream(s)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            bf.beamform(rf, 3, out=out, stream=s)
+        out.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager)
+        rf.mul_(-1.0)                                        # new input in the same buffer, replay again
+        graph.replay()
+        torch.cuda.synchronize()
+        ref = bf.beamform(rf, 3)
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref)
+    finally:
+        bf.close()
