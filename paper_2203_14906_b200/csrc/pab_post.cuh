@@ -59,9 +59,21 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
     float* xs = post64_smem;            // [XR][32]
     float* ys = xs + XR * 32;           // [YR][32]   (ENV only)
     const float* img = P.x + (size_t)f * P.nz * P.nx;
-    for (int r = warp; r < XR; r += 8) {
-        const int gr = xr0 + r;
-        xs[r * 32 + lane] = (gr >= 0 && gr < P.nz && col < P.nx) ? img[(size_t)gr * P.nx + col] : 0.0f;
+    // tile load: 16 rows per warp in flight at a time (the loop is latency-bound otherwise)
+    constexpr int kRowsPerWarp = (XR + 7) / 8;
+#pragma unroll 1
+    for (int k0 = 0; k0 < kRowsPerWarp; k0 += 16) {
+        float v[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const int r = warp + 8 * (k0 + k), gr = xr0 + r;
+            v[k] = (r < XR && gr >= 0 && gr < P.nz && col < P.nx) ? __ldg(img + (size_t)gr * P.nx + col) : 0.0f;
+        }
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const int r = warp + 8 * (k0 + k);
+            if (r < XR) xs[r * 32 + lane] = v[k];
+        }
     }
     __syncthreads();
     float acc[8];
