@@ -22,7 +22,7 @@ struct BfParams {
     float* out;            // image of this launch's first frame
     const float2* xj;      // [nx]  pixel column x_j in samples (x fs / c), fp32 hi + lo
     const float2* xe;      // [N]   element x in samples, fp32 hi + lo
-    const float4* zrow;    // [nz]  (zs, zs^2, zf - 1/2, zi - 0x4B400000 as int bits), zs = z fs / c = zi + zf
+    const float4* zrow;    // [nz]  (zs_hi, 2 zs_lo, zf - 1/2, zi - 2 * 0x4B400000 as int bits), zs = z fs / c = zi + zf
     int N, S, Sp, nx, nz;
     int n_frames;          // valid frames in this launch (stores beyond are skipped)
     float inv_n;           // 1 / N, for the coherence factor (row f1)
@@ -95,8 +95,8 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll 4
         for (int i = 0; i < P.N; ++i, chan += P.Sp) {
             const float2 xe = __ldg(P.xe + i);
-            const float xs = (xj.x - xe.x) + (xj.y - xe.y);
-            const Tap t = delay_tap<false>(xs, xs * xs, row, P.S);
+            const float2 xs = lateral_offset(xj, xe);
+            const Tap t = delay_tap<false>(xs.x, xs.y, row, P.S);
             const float s0 = __ldg(chan + t.i0), s1 = __ldg(chan + t.i0 + 1);
             accumulate_w<K, W>(interp<false>(t, s0, s1), p[0]);
         }
@@ -106,8 +106,8 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll 2
         for (int i = 0; i < P.N; ++i, chan += P.S) {
             const float2 xe = __ldg(P.xe + i);
-            const float xs = (xj.x - xe.x) + (xj.y - xe.y);
-            const Tap t = delay_tap<false>(xs, xs * xs, row, P.S);
+            const float2 xs = lateral_offset(xj, xe);
+            const Tap t = delay_tap<false>(xs.x, xs.y, row, P.S);
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
                 const float4 s0 = __ldg(chan + q * quad_stride + t.i0);

@@ -133,33 +133,49 @@ __device__ __forceinline__ float combine_w(const float (&p)[kAcc<K, W>], float i
 }
 
 // Step a2 + the index half of a3, once per (pixel, element), shared by every frame a thread carries.
-//   xs   lateral offset pixel - element in samples, xs2 = xs^2
-//   row  (zs, zs^2, zf - 1/2, zi - 0x4B400000 as int bits) with zs = z fs / c = zi + zf, zi = floor(zs)
+//   xs, xs_lo2   lateral offset pixel - element in samples as hi + lo, lo passed doubled (2 lo)
+//   row  (zs_hi, 2 zs_lo, zf - 1/2, zi - 2 * 0x4B400000 as int bits): zs = z fs / c = zs_hi + zs_lo = zi + zf,
+//        zi = floor(zs), all from an fp64 host computation
 //   idx = fs sqrt(dx^2 + z^2) / c = zs + delta, where delta >= 0 solves
 //         delta (delta + 2 zs) = xs^2.
-// One MUFU (rsqrt) gives d0 ~ sqrt(xs^2 + zs^2) to ~2 ulp; delta0 = d0 - zs then carries an absolute error of
-// ~ulp(d0), and one Newton step on f(delta) = delta (delta + 2 zs) - xs^2 (f' = 2 (delta + zs) ~ 2 d0, step
-// -f r / 2) squares it away in absolute terms: the result is good to ~1 ulp of delta, not of the 11-12 bit
-// index.  The integer part of zs never enters a float.
+// The signed k-th root is not Lipschitz at 0, so an index error e costs ~e^(5/6) in the image: the index is
+// therefore carried to ~1e-6 samples, not to an fp32 ulp of the 11-12 bit index (DESIGN.md "Delay index
+// precision").  One MUFU (rsqrt) gives d0 ~ sqrt(xs^2 + zs^2); delta0 = d0 - zs; one Newton step on
+// f(delta) = delta (delta + 2 zs) - xs^2 (f' ~ 2 d0, step -f r / 2) with f evaluated in compensated arithmetic:
+// exact xs^2 = xs2 + xs2_lo (FMA), exact delta0 + 2 zs = t_hi + t_lo (Fast2Sum), and the first-order terms of
+// the low parts of xs and zs.  The correction is NOT folded back into delta0: delta0 is split exactly into an
+// integer n0 and a fraction, and the fractions (of zs, of delta0, the correction) are summed at full relative
+// precision; floor(zs) and n0 only ever meet as integers.
 // INR = true: the host has checked that every (pixel, element) index of the geometry lies inside the record
 // and z > 0, so no validity mask is produced and s = s0 + wa (s1 - s0).  INR = false: i0 is clamped into
 // [0, S-2] and wa, wb are both 0 when the delayed sample falls outside the record (reading A6).
 struct Tap { int i0; float wa, wb; };
 
 template <bool INR>
-__device__ __forceinline__ Tap delay_tap(float xs, float xs2, const float4 row, int S) {
-    float q = fmaf(xs, xs, row.y);
+__device__ __forceinline__ Tap delay_tap(float xs, float xs_lo2, const float4 row, int S) {
+    const float kMagic = 12582912.0f;                           // 1.5 * 2^23: adding it rounds to an integer
+    const float xs2 = xs * xs;
+    float q = fmaf(row.x, row.x, xs2);
     if constexpr (!INR) q = fmaxf(q, 1e-30f);
     const float r = rsqrt_approx(q);
     const float d0 = q * r;
-    const float delta0 = d0 - row.x;
-    const float f = fmaf(delta0, d0 + row.x, -xs2);
-    float delta = fmaf(-f, 0.5f * r, delta0);
-    if constexpr (!INR) delta = fminf(fmaxf(delta, 0.0f), 2097152.0f);
-    const float w = row.z + delta;                              // idx - zi - 1/2  >= -1/2
-    const float t = w + 12582912.0f;                            // round to nearest integer: floor(idx - zi)
-    const float fl = t - 12582912.0f;
-    const int i0 = __float_as_int(row.w) + __float_as_int(t);   // zi + (int)fl
+    float delta0 = d0 - row.x;
+    if constexpr (!INR) delta0 = fminf(fmaxf(delta0, 0.0f), 2097152.0f);
+    const float z2 = row.x + row.x;
+    const float t_hi = z2 + delta0;                             // delta0 + 2 zs_hi = t_hi + t_lo exactly
+    const float t_lo = delta0 - (t_hi - z2);
+    const float xs2_lo = fmaf(xs, xs, -xs2);                    // xs^2 = xs2 + xs2_lo exactly
+    float g = fmaf(delta0, t_lo, -xs2_lo);
+    g = fmaf(delta0, row.y, g);                                 // + delta0 * 2 zs_lo
+    g = fmaf(-xs, xs_lo2, g);                                   // - 2 xs xs_lo
+    const float f = fmaf(delta0, t_hi, -xs2) + g;
+    const float corr = -(f * (0.5f * r));                       // Newton step, kept apart from delta0
+    const float t0 = delta0 + kMagic;
+    const float n0 = t0 - kMagic;                               // nearest integer to delta0 (exact)
+    const float w = (row.z + (delta0 - n0)) + corr;             // idx - zi - n0 - 1/2, |w| <= ~1
+    const float t1 = w + kMagic;
+    const float fl = t1 - kMagic;
+    const int i0 = __float_as_int(row.w) + __float_as_int(t0) + __float_as_int(t1);   // zi + n0 + floor part
     const float a = (w - fl) + 0.5f;
     Tap o;
     if constexpr (INR) {
@@ -171,6 +187,17 @@ __device__ __forceinline__ Tap delay_tap(float xs, float xs2, const float4 row, 
         o.wb = ok ? 1.0f - a : 0.0f;
     }
     return o;
+}
+
+// pixel column minus element, in samples, as hi + 2 lo from the two hi + lo table entries (error-free differences)
+__device__ __forceinline__ float2 lateral_offset(float2 xj, float2 xe) {
+    const float a = xj.x - xe.x;
+    const float bv = a - xj.x;
+    const float ea = (xj.x - (a - bv)) - (xe.x + bv);           // a + ea = xj.x - xe.x exactly
+    const float l = ea + (xj.y - xe.y);
+    const float hi = a + l;
+    const float lo = l - (hi - a);
+    return make_float2(hi, lo + lo);
 }
 
 // Step a3: the interpolated sample from its two neighbours.

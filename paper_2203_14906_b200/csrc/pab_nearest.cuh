@@ -156,8 +156,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
                     const float xlo = (xa.x - xe.x) + (xa.y - xe.y), xhi = (xb.x - xe.x) + (xb.y - xe.y);
                     const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
                     const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
-                    const float imin = fminf(sqrtf(fmaf(amin, amin, zf.y)), 2.0e6f);
-                    const float imax = fminf(sqrtf(fmaf(amax, amax, zl.y)), 2.0e6f);
+                    const float imin = fminf(sqrtf(fmaf(amin, amin, zf.x * zf.x)), 2.0e6f);
+                    const float imax = fminf(sqrtf(fmaf(amax, amax, zl.x * zl.x)), 2.0e6f);
                     int w0 = max((int)floorf(imin) - 1, 0) & ~3;
                     int w1 = (int)floorf(imax) + 3;
                     w0 = min(w0, (P.S - 2) & ~3);
@@ -167,10 +167,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
                     const int slot = s * stage_bytes + lane * slot_bytes;
                     ChanEntry e;
 #pragma unroll
-                    for (int c = 0; c < kStgCols; ++c) e.xs[c] = 0.0f;
-                    e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
-#pragma unroll
-                    for (int k = 0; k < 5; ++k) e.pad[k] = 0;
+                    for (int c = 0; c < kStgCols; ++c) e.xs[c] = make_float2(0.0f, 0.0f);
+                    e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2; e.pad = 0;
                     tab[s * C.chunk + lane] = e;
                     const uint32_t bytes = (uint32_t)len * BPS;
                     mbar_arrive_expect_tx(full, bytes * NQ + kNearBlockBytes);
@@ -210,12 +208,12 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
 #pragma unroll 4
             for (int l = 0; l < nch; ++l) {
                 int n = lds_u16(ntab_s + l * kNearBlockBytes);
-                const int base = __float_as_int(lds32(tab_s + l * 64 + 32));
+                const int base = __float_as_int(lds32(tab_s + l * kCE + 64));
                 bool ok = true;
                 if constexpr (!INR) {
                     ok = n != (int)kNearestInvalid;
-                    const int w0 = __float_as_int(lds32(tab_s + l * 64 + 36));
-                    const int w1m1 = __float_as_int(lds32(tab_s + l * 64 + 40)) + 1;
+                    const int w0 = __float_as_int(lds32(tab_s + l * kCE + 68));
+                    const int w1m1 = __float_as_int(lds32(tab_s + l * kCE + 72)) + 1;
                     n = min(max(n, w0), w1m1);
                 }
                 const uint32_t a = (uint32_t)base + n * BPS;

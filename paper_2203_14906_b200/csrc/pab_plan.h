@@ -10,7 +10,8 @@ namespace pab {
 constexpr int kSmemOptin = 232448;      // sm_100 opt-in dynamic shared memory per block
 constexpr int kStagedTileZ = 64;        // rows per tile of the staged kernel (2 warps deep)
 constexpr int kStagedTileX = 8;         // columns per tile
-constexpr int kStagedMaxChunk = 32;     // channels per stage <= one producer lane per channel
+constexpr int kStagedMaxChunk = 32;
+constexpr int kChanEntryBytes = 80;     // per staged channel: 8 x (xs hi, 2 lo) + window base and bounds     // channels per stage <= one producer lane per channel
 
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
@@ -50,10 +51,10 @@ inline bool plan_geometry(int n_elem, int n_samp, double fs, double c, double pi
     double w = (p.tile_z - 1) * p.zs_per_row + (p.tile_x - 1) * p.xs_per_col;
     p.window_samples = w < 1e6 ? window_bound(p.tile_z, p.tile_x, p.zs_per_row, p.xs_per_col) : 1 << 20;
     if (p.window_samples > round_up(n_samp, 4)) p.window_samples = round_up(n_samp, 4);
-    // bytes of one channel slot: window x (frames_per_thread / 4) quads x 16 B, + its 64-byte table entry;
+    // bytes of one channel slot: window x (frames_per_thread / 4) quads x 16 B, + its 80-byte table entry;
     // 64 bytes of barriers and up to 128 bytes of table padding on top
     const int nq = p.frames_per_thread / 4;
-    const long long slot = (long long)p.window_samples * 16 * nq + 64;
+    const long long slot = (long long)p.window_samples * 16 * nq + kChanEntryBytes;
     const int overhead = 64 + 128;
     p.stages = tune.stages ? tune.stages : 3;
     auto fit = [&](int stages) {
@@ -67,7 +68,7 @@ inline bool plan_geometry(int n_elem, int n_samp, double fs, double c, double pi
     if (chunk < 4 && !tune.stages) { p.stages = 2; chunk = fit(p.stages); }
     if (chunk >= 1) {
         p.chunk_channels = chunk;
-        p.smem_bytes = 64 + round_up(p.stages * chunk * 64, 128) + p.stages * chunk * p.window_samples * 16 * nq;
+        p.smem_bytes = 64 + round_up(p.stages * chunk * kChanEntryBytes, 128) + p.stages * chunk * p.window_samples * 16 * nq;
     } else {
         p.chunk_channels = 0; p.stages = 0; p.smem_bytes = 0;   // staged kernel does not fit: direct only
     }
@@ -99,7 +100,7 @@ inline bool plan_geometry(int n_elem, int n_samp, double fs, double c, double pi
 struct DelayTables {
     std::vector<float> xj;     // [nx][2]
     std::vector<float> xe;     // [N][2]
-    std::vector<float> zrow;   // [nz][4]: zs, zs^2, zf - 1/2, zi - 0x4B400000 (int bits)
+    std::vector<float> zrow;   // [nz][4]: zs_hi, 2 zs_lo, zf - 1/2, zi - 2 * 0x4B400000 (int bits)
 };
 
 inline void split_hi_lo(double v, float* hi, float* lo) { *hi = (float)v; *lo = (float)(v - (double)*hi); }
@@ -117,12 +118,13 @@ inline DelayTables make_tables(int n_elem, double fs, double c, double pitch, co
         const double zs = ((double)g.z0 + m * (double)g.dz) * k;
         double zi = std::floor(zs);
         if (zi > 1.0e9) zi = 1.0e9;
-        const int32_t zii = (int32_t)zi - 0x4B400000;       // pre-biased: i0 = zii + bits(fl + 1.5 * 2^23)
+        // pre-biased for two magic-number roundings; the sum zii + bits(t0) + bits(t1) is taken modulo 2^32
+        const uint32_t zii = (uint32_t)(int64_t)zi - 2u * 0x4B400000u;
         float zib;
         static_assert(sizeof(float) == sizeof(int32_t), "");
         __builtin_memcpy(&zib, &zii, 4);
         t.zrow[4 * m + 0] = (float)zs;
-        t.zrow[4 * m + 1] = (float)(zs * zs);
+        t.zrow[4 * m + 1] = (float)(2.0 * (zs - (double)(float)zs));
         t.zrow[4 * m + 2] = (float)((zs - zi) - 0.5);
         t.zrow[4 * m + 3] = zib;
     }

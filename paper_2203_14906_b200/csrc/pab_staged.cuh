@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 #include "../../include/pab.h"
 #include "pab_kernels.cuh"
+#include "pab_plan.h"
 
 namespace pab {
 
@@ -18,15 +19,22 @@ constexpr int kStgRows = 64, kStgCols = 8, kStgConsumerWarps = 16;
 constexpr int kStgThreads = (kStgConsumerWarps + 1) * 32;
 constexpr int kStgMaxStages = 4;
 
-// per staged channel: what a consumer needs besides the samples (64 bytes; every read is a warp broadcast)
+// per staged channel: what a consumer needs besides the samples (80 bytes; every read is a warp broadcast)
 struct __align__(16) ChanEntry {
-    float xs[8];            // pixel column c of the tile minus the element, in samples (hi + lo difference)
+    float2 xs[8];           // pixel column c of the tile minus the element, in samples: (hi, 2 lo)
     int base;               // shared-space address such that sample i of the first quad lives at base + i * BPS
     int w0;                 // first staged sample
     int w1m2;               // last valid i0 (staged end - 2)
-    int pad[5];
+    int pad;
 };
-static_assert(sizeof(ChanEntry) == 64, "ChanEntry is 64 bytes");
+static_assert(sizeof(ChanEntry) == kChanEntryBytes, "ChanEntry size is part of the shared-memory plan");
+constexpr int kCE = (int)sizeof(ChanEntry);
+
+__device__ __forceinline__ float2 lds64(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -130,12 +138,16 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
                     const float2 xe = __ldg(P.xe + ch);
                     ChanEntry e;
 #pragma unroll
-                    for (int c = 0; c < kStgCols; ++c) e.xs[c] = (xj[c].x - xe.x) + (xj[c].y - xe.y);
-                    const float xlo = e.xs[0], xhi = e.xs[kStgCols - 1];
+                    for (int c = 0; c < kStgCols; ++c) {            // fp64: hi + lo of the exact table difference
+                        const double d = ((double)xj[c].x + (double)xj[c].y) - ((double)xe.x + (double)xe.y);
+                        const float hi = (float)d;
+                        e.xs[c] = make_float2(hi, (float)(2.0 * (d - (double)hi)));
+                    }
+                    const float xlo = e.xs[0].x, xhi = e.xs[kStgCols - 1].x;
                     const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
                     const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
-                    const float imin = fminf(sqrtf(fmaf(amin, amin, zf.y)), 2.0e6f);
-                    const float imax = fminf(sqrtf(fmaf(amax, amax, zl.y)), 2.0e6f);
+                    const float imin = fminf(sqrtf(fmaf(amin, amin, zf.x * zf.x)), 2.0e6f);
+                    const float imax = fminf(sqrtf(fmaf(amax, amax, zl.x * zl.x)), 2.0e6f);
                     int w0 = max((int)floorf(imin) - 1, 0) & ~3;
                     int w1 = (int)floorf(imax) + 3;
                     if (NQ == 0) {
@@ -149,9 +161,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
                     w1 = min(w1, w0 + C.window);
                     const int len = w1 - w0;
                     const int slot = s * stage_bytes + lane * slot_bytes;
-                    e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2;
-#pragma unroll
-                    for (int k = 0; k < 5; ++k) e.pad[k] = 0;
+                    e.base = (int)data0 + slot - w0 * BPS; e.w0 = w0; e.w1m2 = w1 - 2; e.pad = 0;
                     tab[s * C.chunk + lane] = e;
                     const uint32_t bytes = (uint32_t)len * BPS;
                     mbar_arrive_expect_tx(full, bytes * NCOPY);
@@ -186,16 +196,16 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
         for (int ck = 0; ck < n_chunks; ++ck) {
             mbar_wait(bar0 + 8 * s, ph);
             const int nch = min(C.chunk, P.N - ck * C.chunk);
-            const uint32_t tab_s = smem_u32(tab + s * C.chunk) + col * 4;
+            const uint32_t tab_s = smem_u32(tab + s * C.chunk);
 #pragma unroll 2
             for (int l = 0; l < nch; ++l) {
-                const float xs = lds32(tab_s + l * 64);
-                const int base = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 32));
-                const Tap t = delay_tap<INR>(xs, xs * xs, row, P.S);
+                const float2 xs = lds64(tab_s + l * kCE + col * 8);
+                const int base = __float_as_int(lds32(tab_s + l * kCE + 64));
+                const Tap t = delay_tap<INR>(xs.x, xs.y, row, P.S);
                 int i0 = t.i0;
                 if constexpr (!INR) {
-                    const int w0 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 36));
-                    const int w1m2 = __float_as_int(lds32(tab_s - col * 4 + l * 64 + 40));
+                    const int w0 = __float_as_int(lds32(tab_s + l * kCE + 68));
+                    const int w1m2 = __float_as_int(lds32(tab_s + l * kCE + 72));
                     i0 = min(max(i0, w0), w1m2);
                 }
                 const uint32_t a = (uint32_t)base + i0 * BPS;

@@ -50,6 +50,19 @@ def check_raw(gpu, ref, order, mask=None):
     return rel_l2
 
 
+def test_margin_on_fresh_seeds(pab, orc):
+    """The tolerance must not hinge on the seeds of the named configs: other seeds of the headline workload, with
+    a bound 4x tighter than north_star's.  (With the index carried to fp32 ulps of the index instead of ~1e-6
+    samples, 3 % of such frames exceeded 1e-4: the signed root is not Lipschitz at 0.)"""
+    for seed in (9001, 9005):
+        w = synth.make_config("C2b", seed=seed, n_frames=16)
+        for order in (1, 3):
+            gpu, _ = run_gpu(pab, w.geom, w.rf, order)
+            ref = orc.beamform(w.rf, w.geom, order)
+            for f in range(16):
+                assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
+
+
 def edge_mask(orc, g):
     idx = orc.delays(g)                                   # [nz][nx][N]
     return np.any(np.abs(idx - (g.n_samp - 1)) < 1e-2, axis=-1)
