@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll 4
         for (int i = 0; i < P.N; ++i, chan += P.Sp) {
             const float2 xe = __ldg(P.xe + i);
-            const float2 xs = lateral_offset(xj, xe);
+            const float2 xs = lateral_square(xj, xe);
             const Tap t = delay_tap<false>(xs.x, xs.y, row, P.S);
             const float s0 = __ldg(chan + t.i0), s1 = __ldg(chan + t.i0 + 1);
             accumulate_w<K, W>(interp<false>(t, s0, s1), p[0]);
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) bf_direct_kernel(const BfParams P) {
 #pragma unroll 2
         for (int i = 0; i < P.N; ++i, chan += P.S) {
             const float2 xe = __ldg(P.xe + i);
-            const float2 xs = lateral_offset(xj, xe);
+            const float2 xs = lateral_square(xj, xe);
             const Tap t = delay_tap<false>(xs.x, xs.y, row, P.S);
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {

@@ -133,7 +133,9 @@ __device__ __forceinline__ float combine_w(const float (&p)[kAcc<K, W>], float i
 }
 
 // Step a2 + the index half of a3, once per (pixel, element), shared by every frame a thread carries.
-//   xs, xs_lo2   lateral offset pixel - element in samples as hi + lo, lo passed doubled (2 lo)
+//   xs2, c0      the lateral offset xs = pixel - element (samples) enters only through its square, passed as
+//                xs2 = fl(xs_hi^2) and c0 = xs2 - xs^2 (the rounding error of the square plus the low part of xs),
+//                both uniform over a warp and computed once per (tile, element) by the producer
 //   row  (zs_hi, 2 zs_lo, zf - 1/2, zi - 2 * 0x4B400000 as int bits): zs = z fs / c = zs_hi + zs_lo = zi + zf,
 //        zi = floor(zs), all from an fp64 host computation
 //   idx = fs sqrt(dx^2 + z^2) / c = zs + delta, where delta >= 0 solves
@@ -152,9 +154,8 @@ __device__ __forceinline__ float combine_w(const float (&p)[kAcc<K, W>], float i
 struct Tap { int i0; float wa, wb; };
 
 template <bool INR>
-__device__ __forceinline__ Tap delay_tap(float xs, float xs_lo2, const float4 row, int S) {
+__device__ __forceinline__ Tap delay_tap(float xs2, float c0, const float4 row, int S) {
     const float kMagic = 12582912.0f;                           // 1.5 * 2^23: adding it rounds to an integer
-    const float xs2 = xs * xs;
     float q = fmaf(row.x, row.x, xs2);
     if constexpr (!INR) q = fmaxf(q, 1e-30f);
     const float r = rsqrt_approx(q);
@@ -164,15 +165,13 @@ __device__ __forceinline__ Tap delay_tap(float xs, float xs_lo2, const float4 ro
     const float z2 = row.x + row.x;
     const float t_hi = z2 + delta0;                             // delta0 + 2 zs_hi = t_hi + t_lo exactly
     const float t_lo = delta0 - (t_hi - z2);
-    const float xs2_lo = fmaf(xs, xs, -xs2);                    // xs^2 = xs2 + xs2_lo exactly
-    float g = fmaf(delta0, t_lo, -xs2_lo);
-    g = fmaf(delta0, row.y, g);                                 // + delta0 * 2 zs_lo
-    g = fmaf(-xs, xs_lo2, g);                                   // - 2 xs xs_lo
+    float g = fmaf(delta0, t_lo, c0);                           // low-order part of f: delta0 t_lo - (xs^2 - xs2)
+    g = fmaf(delta0, row.y, g);                                 //                      + delta0 * 2 zs_lo
     const float f = fmaf(delta0, t_hi, -xs2) + g;
-    const float corr = -(f * (0.5f * r));                       // Newton step, kept apart from delta0
     const float t0 = delta0 + kMagic;
     const float n0 = t0 - kMagic;                               // nearest integer to delta0 (exact)
-    const float w = (row.z + (delta0 - n0)) + corr;             // idx - zi - n0 - 1/2, |w| <= ~1
+    // Newton step -f r / 2, kept apart from delta0: idx - zi - n0 - 1/2 = frac parts + step, |w| <= ~1
+    const float w = fmaf(f * r, -0.5f, row.z + (delta0 - n0));
     const float t1 = w + kMagic;
     const float fl = t1 - kMagic;
     const int i0 = __float_as_int(row.w) + __float_as_int(t0) + __float_as_int(t1);   // zi + n0 + floor part
@@ -189,15 +188,17 @@ __device__ __forceinline__ Tap delay_tap(float xs, float xs_lo2, const float4 ro
     return o;
 }
 
-// pixel column minus element, in samples, as hi + 2 lo from the two hi + lo table entries (error-free differences)
-__device__ __forceinline__ float2 lateral_offset(float2 xj, float2 xe) {
+// (xs2, c0) of delay_tap from the hi + lo table entries of a pixel column and an element, in fp32 with
+// error-free differences (the direct kernel; the staged kernel's producer does this in fp64)
+__device__ __forceinline__ float2 lateral_square(float2 xj, float2 xe) {
     const float a = xj.x - xe.x;
     const float bv = a - xj.x;
     const float ea = (xj.x - (a - bv)) - (xe.x + bv);           // a + ea = xj.x - xe.x exactly
     const float l = ea + (xj.y - xe.y);
     const float hi = a + l;
     const float lo = l - (hi - a);
-    return make_float2(hi, lo + lo);
+    const float xs2 = hi * hi;
+    return make_float2(xs2, -fmaf(hi, lo + lo, fmaf(hi, hi, -xs2)));
 }
 
 // Step a3: the interpolated sample from its two neighbours.

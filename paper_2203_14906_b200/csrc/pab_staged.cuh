@@ -21,7 +21,7 @@ constexpr int kStgMaxStages = 4;
 
 // per staged channel: what a consumer needs besides the samples (80 bytes; every read is a warp broadcast)
 struct __align__(16) ChanEntry {
-    float2 xs[8];           // pixel column c of the tile minus the element, in samples: (hi, 2 lo)
+    float2 xs[8];           // per pixel column c of the tile: (xs2, c0) of delay_tap, xs = column - element in samples
     int base;               // shared-space address such that sample i of the first quad lives at base + i * BPS
     int w0;                 // first staged sample
     int w1m2;               // last valid i0 (staged end - 2)
@@ -137,13 +137,16 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
                 if (ch < P.N) {
                     const float2 xe = __ldg(P.xe + ch);
                     ChanEntry e;
+                    float xlo = 0.0f, xhi = 0.0f;
 #pragma unroll
-                    for (int c = 0; c < kStgCols; ++c) {            // fp64: hi + lo of the exact table difference
+                    for (int c = 0; c < kStgCols; ++c) {            // fp64: the exact table difference and its square
                         const double d = ((double)xj[c].x + (double)xj[c].y) - ((double)xe.x + (double)xe.y);
                         const float hi = (float)d;
-                        e.xs[c] = make_float2(hi, (float)(2.0 * (d - (double)hi)));
+                        const float xs2 = hi * hi;
+                        e.xs[c] = make_float2(xs2, (float)((double)xs2 - d * d));
+                        if (c == 0) xlo = hi;
+                        if (c == kStgCols - 1) xhi = hi;
                     }
-                    const float xlo = e.xs[0].x, xhi = e.xs[kStgCols - 1].x;
                     const float amax = fmaxf(fabsf(xlo), fabsf(xhi));
                     const float amin = (xlo <= 0.0f && xhi >= 0.0f) ? 0.0f : fminf(fabsf(xlo), fabsf(xhi));
                     const float imin = fminf(sqrtf(fmaf(amin, amin, zf.x * zf.x)), 2.0e6f);
