@@ -200,7 +200,9 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
             mbar_wait(bar0 + 8 * s, ph);
             const int nch = min(C.chunk, P.N - ck * C.chunk);
             const uint32_t tab_s = smem_u32(tab + s * C.chunk);
-#pragma unroll 2
+            // elements in flight per thread: measured best 3 with 16 frames per thread, 2 otherwise
+            constexpr int kElemUnroll = NQ >= 4 ? 3 : 2;
+#pragma unroll (kElemUnroll)
             for (int l = 0; l < nch; ++l) {
                 const float2 xs = lds64(tab_s + l * kCE + col * 8);
                 const int base = __float_as_int(lds32(tab_s + l * kCE + 64));
