@@ -41,11 +41,14 @@ N_SETS = 4          # rotating input/output buffer sets: 4 x (64 MiB RF + 64 MiB
 METRIC = "beamformed frames/s, order-3 DMAS, 128ch (C2b: 128 el x 2048 samp x 1024x256 px, 64-frame batches, " \
          "band-pass + envelope + log)"
 
-# Algorithmic work per item (pixel x element x frame) of the fused beamforming kernel at order 3, DESIGN.md
-# "Roofline": XU (MUFU) lane-ops = 2 (lg2 + ex2 of the cube root) + 1/64 (the delay sqrt, shared by the 64
-# frames of a batch); FP32-pipe slots = 6 + 3/64; HBM bytes = RF in + image out, once.
-XU_PER_ITEM = 2.0 + 1.0 / FRAMES
-FP32_PER_ITEM = 6.0 + 3.0 / FRAMES
+# Work per item (pixel x element x frame) of the fused beamforming kernel at order 3 as this build runs it (cached
+# interpolation taps: no delay square root in the kernel): XU (MUFU) lane-ops = 2 (lg2 + ex2
+# of the cube root); FP32-pipe slots = 6 (interpolation 2, x 1/3, three accumulations); HBM bytes = RF in + image
+# out + the 4-byte tap table of the geometry, once per launch.  (With in-kernel delays the algorithmic figures are
+# 2 + 1/64 and 6 + 3/64: one square root and three FP32 slots per (pixel, element), shared by the 64 frames.)
+XU_PER_ITEM = 2.0
+FP32_PER_ITEM = 6.0
+DELAY_CACHE = "all"
 SM_COUNT = 148
 NCU_TRAFFIC_BYTES = 47_247_872 + 20_565_504   # per 64-frame launch; profiles/r1_beamform_ncu_b.md
 XU_LANES_PER_CLK_SM = 16
@@ -192,7 +195,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     rf_sets = [torch.roll(rf_host, r, 0).to(dev) for r in range(N_SETS)]
     out_sets = [torch.empty((FRAMES, g.nz, g.nx), dtype=torch.float32, device=dev) for _ in range(N_SETS)]
     out_host = torch.empty((FRAMES, g.nz, g.nx), dtype=torch.float32).pin_memory()
-    bf = binding.Beamformer(g, post=POST)
+    bf = binding.Beamformer(g, post=POST, delay_cache=DELAY_CACHE)
     stream = torch.cuda.current_stream(dev)
     items_per_frame = g.nz * g.nx * g.n_elem
     K, W = args.steps, max(args.warmup, 3)
@@ -236,7 +239,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     checksum = float(out_host[0, 512, 128])
 
     # ---- beamform-only (raw output) throughput, for the stage breakdown ----
-    bf_raw = binding.Beamformer(g)
+    bf_raw = binding.Beamformer(g, delay_cache=DELAY_CACHE)
     for i in range(3):
         bf_raw.beamform(rf_sets[i % N_SETS], ORDER, out=out_sets[i % N_SETS], stream=stream)
     torch.cuda.synchronize()
@@ -261,12 +264,13 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         f_hz = peaks["sm_max_mhz"] * 1e6
         xu_peak = SM_COUNT * XU_LANES_PER_CLK_SM * f_hz
         fp32_peak = SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz
-        hbm_bytes = frames_per_launch * (g.n_elem * g.n_samp * 4 + g.nz * g.nx * 4)
+        hbm_bytes = frames_per_launch * (g.n_elem * g.n_samp * 4 + g.nz * g.nx * 4) + g.nz * g.nx * g.n_elem * 4
         t_xu = items_per_launch * XU_PER_ITEM / xu_peak
         t_fp32 = items_per_launch * FP32_PER_ITEM / fp32_peak
         t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
         achieved = items_per_launch * XU_PER_ITEM / (bf_launch_ms * 1e-3)
-        roofline = {"bound": "alu", "kernel": "bf_staged_kernel<3,4,true> (fused delay+interp+root+power sums+Newton, 16 frames per thread)",
+        roofline = {"bound": "alu", "kernel": "bf_cached_kernel<3,4> (fused tap fetch + interpolation + root + power sums + Newton, 16 frames "
+                              "per thread, cached interpolation taps)",
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
                     "frac": achieved / xu_peak, "traffic": NCU_TRAFFIC_BYTES,
                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
@@ -285,6 +289,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                 "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOAD + "+post", "order": ORDER, "frames_per_step": FRAMES,
                            "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx, "post": "log",
+                           "delay_cache": DELAY_CACHE,
                            "parallelism": f"replicas x{world}, no collective",
                            "l2": f"inputs/outputs rotate over {N_SETS} buffer sets (512 MiB) > 126 MB L2"},
                 "items_per_s": fps * items_per_frame,
@@ -327,9 +332,12 @@ def run_sweep(args):
              ("C2b", 64, (1, 2, 3), False, "none"), ("C2b", 64, (3,), False, "cf"), ("C3", 256, (3,), True, "none"),
              ("C4", 1, (4, 5), False, "none"), ("C4", 16, (4, 5), False, "none"), ("C4", 16, (5,), False, "cf"),
              ("C5", 1024, (3,), True, "none"), ("C2b", 64, (6, 8), False, "none"), ("C2b", 64, (1, 2, 3), False, "nearest"), ("C4", 16, (4, 5), False, "nearest")]
+    cases += [("C2", 1, (1, 2, 3), False, "cache-single"), ("C4", 1, (4, 5), False, "cache-single"),
+              ("C2b", 64, (1, 2, 3), False, "cache-all"), ("C4", 16, (4, 5), False, "cache-all")]
     for cfg, F, orders, post, weight in cases:
         interp = "nearest" if weight == "nearest" else "linear"
-        weight = "none" if weight == "nearest" else weight
+        cache = weight[6:] if weight.startswith("cache-") else "off"
+        weight = "cf" if weight == "cf" else "none"
         gen = min(F, 64)
         w = synth.make_config(cfg, n_frames=gen)
         g = w.geom
@@ -338,7 +346,8 @@ def run_sweep(args):
         rf = torch.from_numpy(np.concatenate([w.rf] * (call_frames // gen), axis=0)).cuda()
         dtype = "int16" if w.rf.dtype == np.int16 else "float32"
         out = torch.empty((call_frames, g.nz, g.nx), dtype=torch.float32, device="cuda")
-        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None, weight=weight, interp=interp)
+        bf = binding.Beamformer(g, dtype=dtype, post=dict(w.post) if post else None, weight=weight, interp=interp,
+                                delay_cache=cache)
         items = g.nz * g.nx * g.n_elem
         for order in orders:
             reps = max(3, min(50, int(0.2 / max(1e-5, items * F * 1e-12))))
@@ -367,6 +376,8 @@ def run_sweep(args):
             xu = _XU[order][0] + _XU[order][1] / batch
             if interp == "nearest":          # no MUFU and no delay arithmetic in the hot loop; u, u^2.. accumulation only
                 xu = 0.0
+            if cache != "off" and (F < 4 or cache == "all"):
+                xu = _XU[order][0]            # taps come from the table: no delay square root in the kernel
             fp = _FP32[order][0] + _FP32[order][1] / batch + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
             if interp == "nearest":
                 fp = {1: 1.0, 2: 3.0, 3: 4.0, 4: 5.0, 5: 7.0}[order]
@@ -378,7 +389,7 @@ def run_sweep(args):
             # interpolated path gathers 2 x 4 bytes per item, the nearest-sample path 4
             t_sm = items * F * (4.0 if interp == "nearest" else 8.0) / (SM_COUNT * 128.0 * f_hz) * 1e3
             bf_ms = prof["beamform"][0] / reps
-            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw", "weight": weight, "interp": interp,
+            print(json.dumps({"sweep": cfg, "order": order, "frames": F, "post": "log" if post else "raw", "weight": weight, "interp": interp, "delay_cache": cache,
                               "dtype_in": dtype, "n_elem": g.n_elem, "n_samp": g.n_samp, "nz": g.nz, "nx": g.nx,
                               "ms_per_stream": round(ms, 5), "frames_per_s": round(F / (ms * 1e-3), 1),
                               "items_per_s": round(items * F / (ms * 1e-3), 0),

@@ -48,6 +48,11 @@ extern "C" {
 #define PAB_INTERP_LINEAR  0   /* s_i = linear interpolation at the fractional delay index (A4); default           */
 #define PAB_INTERP_NEAREST 1   /* s_i = rf_i[floor(idx_i + 1/2)]: the literal integer-delay eq. (1) (A21)           */
 
+/* cached interpolation taps (pab_set_delay_cache) */
+#define PAB_CACHE_OFF    0   /* delays computed in-kernel on every call; default                                   */
+#define PAB_CACHE_SINGLE 1   /* calls of 1..3 frames read their taps from the cached table                         */
+#define PAB_CACHE_ALL    2   /* ... and so do the 16-frame (orders 1..3) / 8-frame (orders 4, 5) groups of longer calls */
+
 /* pixel weighting (pab_set_weight) */
 #define PAB_WEIGHT_NONE 0   /* out = e_k                                                                          */
 #define PAB_WEIGHT_CF   1   /* out = CF e_k, CF = (sum_i s_i)^2 / (N sum_i s_i^2), 0 when every s_i = 0             */
@@ -127,6 +132,15 @@ int pab_set_weight(pab_ctx* ctx, int weight);
  * expression: n_elem * nx * nz uint16 entries.  Synchronises the device on the first call.
  * Errors: PAB_ERR_INVALID (n_samp > 65534, or combined with PAB_WEIGHT_CF), PAB_ERR_ALLOC, PAB_ERR_CUDA. */
 int pab_set_interp(pab_ctx* ctx, int interp);
+
+/* pab_set_delay_cache -- keep the interpolation tap (integer sample + fraction) of every (pixel, element) pair in
+ * device memory, computed once in fp64, instead of recomputing the delay in every call (PAPER.md:190 keeps its
+ * delays in GPU global memory; BASELINE.json north_star allows a cached table "where it wins").  It wins for calls
+ * of 1..3 frames, where the in-kernel delay cannot be shared between frames.  4 bytes per (pixel, element):
+ * 134 MB at 128 elements x 1024 x 256 pixels.  Linear interpolation, no weighting, orders 1..5 (other settings
+ * fall back to the in-kernel delay).  In-range geometries only (pab_plan_info.in_range), staged variant.
+ * Synchronises the device on the first call.  Errors: PAB_ERR_INVALID, PAB_ERR_ALLOC, PAB_ERR_CUDA. */
+int pab_set_delay_cache(pab_ctx* ctx, int mode);
 
 /* pab_set_tuning -- override the plan's blocking (autotuning / experiments); 0 keeps the default of a field.
  *   frames_per_thread 4, 8 or 16;  stages 2..4;  chunk_channels 1..32 (clamped to what fits in shared memory);

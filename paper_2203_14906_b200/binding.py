@@ -23,7 +23,7 @@ _MODES = {"raw": RAW, "bandpass": BANDPASS, "envelope": ENVELOPE, "log": LOG}
 _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_STAGED}
 
 # every symbol include/pab.h declares
-SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
+SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_delay_cache", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
            "pab_launch_count", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
@@ -76,6 +76,7 @@ def load(build_if_missing: bool = False):
     L.pab_set_variant.argtypes = [vp, ip]
     L.pab_set_weight.argtypes = [vp, ip]
     L.pab_set_interp.argtypes = [vp, ip]
+    L.pab_set_delay_cache.argtypes = [vp, ip]
     L.pab_set_tuning.argtypes = [vp, ip, ip, ip, ip]
     L.pab_beamform.argtypes = [vp, vp, ip, ip, vp, vp]
     L.pab_beamform_host.argtypes = [vp, vp, ip, ip, vp]
@@ -143,7 +144,7 @@ class Beamformer:
     """pab_create / pab_set_* / pab_beamform / pab_destroy for one geometry on the current CUDA device."""
 
     def __init__(self, g, dtype: str = "float32", scale: float = 1.0, post: dict | None = None,
-                 variant: str = "auto", weight: str = "none", interp: str = "linear"):
+                 variant: str = "auto", weight: str = "none", interp: str = "linear", delay_cache: str = "off"):
         self._L = load()
         self._h = C.c_void_p()
         self.geom = g
@@ -160,6 +161,8 @@ class Beamformer:
             self.set_weight(weight)
         if interp != "linear":
             self.set_interp(interp)
+        if delay_cache != "off":
+            self.set_delay_cache(delay_cache)
 
     def _check(self, rc, what):
         if rc != OK:
@@ -177,6 +180,9 @@ class Beamformer:
     def set_interp(self, interp: str):
         self._check(self._L.pab_set_interp(self._h, {"linear": INTERP_LINEAR, "nearest": INTERP_NEAREST}[interp]),
                     "pab_set_interp")
+
+    def set_delay_cache(self, mode: str):
+        self._check(self._L.pab_set_delay_cache(self._h, {"off": 0, "single": 1, "all": 2}[mode]), "pab_set_delay_cache")
 
     def set_variant(self, variant: str):
         self._check(self._L.pab_set_variant(self._h, _VARIANTS[variant]), "pab_set_variant")

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpab.so")
 SOURCES = ["pab_api.cu"]
-DEPS = ["pab_api.cu", "pab_run.inl", "pab_kernels.cuh", "pab_staged.cuh", "pab_post.cuh", "pab_nearest.cuh", "pab_metrics.cuh", "pab_math.cuh", "pab_plan.h",
+DEPS = ["pab_api.cu", "pab_run.inl", "pab_kernels.cuh", "pab_staged.cuh", "pab_post.cuh", "pab_nearest.cuh", "pab_metrics.cuh", "pab_cache.cuh", "pab_math.cuh", "pab_plan.h",
         os.path.join("..", "..", "include", "pab.h")]
 
 

@@ -12,6 +12,7 @@
 #include "pab_post.cuh"
 #include "pab_nearest.cuh"
 #include "pab_metrics.cuh"
+#include "pab_cache.cuh"
 
 using namespace pab;
 
@@ -30,6 +31,9 @@ struct pab_ctx {
     int variant = PAB_VARIANT_AUTO;
     int weight = PAB_WEIGHT_NONE;
     int interp = PAB_INTERP_LINEAR;
+    int cache_mode = PAB_CACHE_OFF;
+    uint32_t* d_taps = nullptr;          // cached interpolation taps, tile-major (pab_set_delay_cache)
+    int* d_w0s = nullptr;                // window start of every (tile, element)
     void* d_metric = nullptr;            // MetricAcc + double[1] + 2 x 4096 histogram bins (row f3), lazy
     unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
@@ -76,7 +80,7 @@ size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
 
 void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
-    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric);
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s);
     for (int b = 0; b < 2; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -237,6 +241,34 @@ int pab_set_weight(pab_ctx* ctx, int weight) {
     if (!ctx || (weight != PAB_WEIGHT_NONE && weight != PAB_WEIGHT_CF)) return PAB_ERR_INVALID;
     if (weight == PAB_WEIGHT_CF && ctx->interp == PAB_INTERP_NEAREST) return PAB_ERR_INVALID;
     ctx->weight = weight;
+    return PAB_OK;
+}
+
+int pab_set_delay_cache(pab_ctx* ctx, int mode) {
+    if (!ctx || mode < PAB_CACHE_OFF || mode > PAB_CACHE_ALL) return PAB_ERR_INVALID;
+    if (mode != PAB_CACHE_OFF) {
+        if (!ctx->plan.in_range || ctx->plan.smem_bytes == 0 || ctx->plan.window_samples > kCacheMaxWindow) return PAB_ERR_INVALID;
+        if (!ctx->d_taps) {
+            const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z = (ctx->grid.nz + kStgRows - 1) / kStgRows;
+            if (tiles_z > 65535 || ctx->N > 65535) return PAB_ERR_INVALID;
+            const size_t blocks = (size_t)tiles_x * tiles_z * ctx->N;
+            PAB_CUDA(ctx, cached_configure(ctx->smem_optin));
+            PAB_CUDA(ctx, cudaMalloc(&ctx->d_taps, blocks * kCacheBlockBytes));
+            cudaError_t e = cudaMalloc(&ctx->d_w0s, blocks * sizeof(int));
+            if (e == cudaSuccess) {
+                CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
+                            (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x};
+                delay_cache_kernel<<<dim3(tiles_x, tiles_z, ctx->N), kStgRows * kStgCols>>>(G, ctx->d_taps, ctx->d_w0s);
+                ctx->launches++;
+                e = cudaDeviceSynchronize();
+            }
+            if (e != cudaSuccess) {
+                cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); ctx->d_taps = nullptr; ctx->d_w0s = nullptr;
+                return cuda_fail(ctx, e, "delay cache");
+            }
+        }
+    }
+    ctx->cache_mode = mode;
     return PAB_OK;
 }
 

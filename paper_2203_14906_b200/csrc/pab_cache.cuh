@@ -1,0 +1,249 @@
+// pab_cache.cuh -- the cached-delay variant of the fused beamforming kernel (BASELINE.json north_star: "Per-pixel
+// delays are computed in-kernel, with no delay table, or from a cached ... table where ncu shows it wins").
+//
+// The delay of a (pixel, element) pair does not depend on the frame.  With many frames per thread its cost is
+// amortised (bf_staged_kernel); with one frame per thread (calls of 1..3 frames) the ~35 instructions of
+// delay_tap dominate the ~9 of the rest.  Here the interpolation tap of every (pixel, element) is computed ONCE
+// per geometry, in fp64, and kept in device memory as one 32-bit word: 12 bits of integer sample offset from
+// the staged window's start and 20 bits of fraction (2^-21 samples worst-case rounding).  It is the paper's own
+// arrangement (delays "calculated and stored in the GPU (global) memory") with the table laid out
+// tile-major, [tile row][tile col][element][8 cols][64 rows], so the 2 KB block of one (tile, element) is
+// contiguous and the producer warp stages it by one bulk copy beside that element's RF window.  In-range
+// geometries only (no out-of-record pixels); the window start of every (tile, element) is stored beside it so
+// that the table and the staged window agree exactly.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "pab_kernels.cuh"
+#include "pab_staged.cuh"
+
+namespace pab {
+
+constexpr int kCacheBlockBytes = kStgRows * kStgCols * 4;
+constexpr int kCacheFracBits = 20;
+constexpr int kCacheMaxWindow = 4000;        // the integer part must fit 12 bits
+
+struct CacheGeom {
+    double fs, c, pitch, x0, dx, z0, dz;
+    int N, S, nx, nz, tiles_x;
+};
+
+// grid: (tiles_x, tiles_z, N), 512 threads = one tile.  taps[((tile * N + i) * 8 + col) * 64 + row], w0s[tile * N + i]
+__global__ void __launch_bounds__(kStgRows * kStgCols) delay_cache_kernel(const CacheGeom G, uint32_t* __restrict__ taps,
+                                                                           int* __restrict__ w0s) {
+    __shared__ int s_min;
+    const int col = threadIdx.x / kStgRows, row = threadIdx.x % kStgRows;
+    const int j = min((int)blockIdx.x * kStgCols + col, G.nx - 1), m = min((int)blockIdx.y * kStgRows + row, G.nz - 1);
+    const int i = blockIdx.z;
+    // the definition, every operation individually rounded in fp64 (readings A5)
+    const double x = __dadd_rn(G.x0, __dmul_rn((double)j, G.dx));
+    const double z = __dadd_rn(G.z0, __dmul_rn((double)m, G.dz));
+    const double xe = __dmul_rn(__dsub_rn((double)i, __ddiv_rn(__dsub_rn((double)G.N, 1.0), 2.0)), G.pitch);
+    const double ddx = __dsub_rn(x, xe);
+    const double idx = __ddiv_rn(__dmul_rn(G.fs, __dsqrt_rn(__dadd_rn(__dmul_rn(ddx, ddx), __dmul_rn(z, z)))), G.c);
+    if (threadIdx.x == 0) s_min = 0x7fffffff;
+    __syncthreads();
+    atomicMin(&s_min, (int)floor(idx));
+    __syncthreads();
+    const int w0 = max(s_min - 1, 0) & ~3;
+    const size_t blk = ((size_t)blockIdx.y * G.tiles_x + blockIdx.x) * G.N + i;
+    if (threadIdx.x == 0) w0s[blk] = w0;
+    const double rel = idx - (double)w0;                                 // >= 0, < window
+    taps[blk * (kStgRows * kStgCols) + threadIdx.x] = (uint32_t)llrint(rel * (double)(1u << kCacheFracBits));
+}
+
+__device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+// NQ = 0: lin layout, one frame per thread; NQ = 4 (orders 1..3) / NQ = 2 (orders 4, 5): quad layout, 16 / 8 frames
+// per thread.  In-range geometries.
+template <int K, int NQ>
+__global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParams P, const StagedCfg C,
+                                                                    const uint32_t* __restrict__ taps,
+                                                                    const int* __restrict__ w0s) {
+    constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
+    constexpr int BPS = NQ == 0 ? 4 : 16;
+    constexpr int NCOPY = NQ == 0 ? 1 : NQ;
+    extern __shared__ __align__(128) unsigned char stg_smem[];
+    unsigned char* smem = stg_smem;
+    const uint32_t bar0 = smem_u32(smem);
+    const uint32_t ctab0 = bar0 + 64;                                    // [stages][chunk][512] uint32
+    const uint32_t data0 = ctab0 + C.stages * C.chunk * kCacheBlockBytes;
+    const int quad_bytes = C.window * BPS;
+    const int slot_bytes = quad_bytes * NCOPY;
+    const int stage_bytes = C.chunk * slot_bytes;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_chunks = (P.N + C.chunk - 1) / C.chunk;
+    const int n_tiles = C.tiles_x * C.tiles_z * C.groups;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C.stages; ++s) {
+            mbar_init(bar0 + 8 * s, C.chunk);
+            mbar_init(bar0 + 8 * (C.stages + s), kStgConsumerWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == kStgConsumerWarps) {
+        if (lane >= C.chunk) return;
+        const size_t chan_stride = NQ == 0 ? (size_t)P.Sp * 4 : (size_t)P.S * 16;
+        const size_t grp_stride = (size_t)P.N * chan_stride;
+        const int row_len = NQ == 0 ? P.Sp : P.S;
+        int s = 0;
+        uint32_t ph = 1;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            const int bz = tile % C.groups, txy = tile / C.groups;       // frame groups innermost: table blocks reused from L2
+            const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)bz * (NQ == 0 ? 1 : NQ) * grp_stride;
+            const size_t blk0 = (size_t)txy * P.N;
+            for (int ck = 0; ck < n_chunks; ++ck) {
+                const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
+                mbar_wait(empty, ph);
+                const int ch = ck * C.chunk + lane;
+                if (ch < P.N) {
+                    const int w0 = __ldg(w0s + blk0 + ch);
+                    const int len = min(C.window, row_len - w0);
+                    const uint32_t bytes = (uint32_t)len * BPS;
+                    const int slot = s * stage_bytes + lane * slot_bytes;
+                    mbar_arrive_expect_tx(full, bytes * NCOPY + kCacheBlockBytes);
+                    bulk_g2s(ctab0 + (s * C.chunk + lane) * kCacheBlockBytes,
+                             taps + (blk0 + ch) * (size_t)(kStgRows * kStgCols), kCacheBlockBytes, full);
+                    const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
+#pragma unroll
+                    for (int q = 0; q < NCOPY; ++q)
+                        bulk_g2s(data0 + slot + q * quad_bytes, src + q * grp_stride, bytes, full);
+                } else {
+                    mbar_arrive(full);
+                }
+                if (++s == C.stages) { s = 0; ph ^= 1; }
+            }
+        }
+        return;
+    }
+
+    const int col = warp & 7;
+    const uint32_t my = (uint32_t)((col * kStgRows + (warp >> 3) * 32 + lane) * 4);
+    int s = 0;
+    uint32_t ph = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int bz = tile % C.groups, txy = tile / C.groups;
+        const int bx = txy % C.tiles_x, by = txy / C.tiles_x;
+        const int j = bx * kStgCols + col;
+        const int m = by * kStgRows + (warp >> 3) * 32 + lane;
+        float p[NF][K];
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+#pragma unroll
+            for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+
+        for (int ck = 0; ck < n_chunks; ++ck) {
+            mbar_wait(bar0 + 8 * s, ph);
+            const int nch = min(C.chunk, P.N - ck * C.chunk);
+            const uint32_t ctab_s = ctab0 + s * C.chunk * kCacheBlockBytes + my;
+            const uint32_t data_s = data0 + s * stage_bytes;
+            constexpr int kElemUnroll = NQ >= 4 ? 2 : 4;
+#pragma unroll (kElemUnroll)
+            for (int l = 0; l < nch; ++l) {
+                const uint32_t e = lds32u(ctab_s + l * kCacheBlockBytes);
+                const float a = __uint_as_float(0x3F800000u | ((e << (32 - kCacheFracBits)) >> 9)) - 1.0f;   // fraction, exact
+                const uint32_t addr = data_s + l * slot_bytes + (e >> kCacheFracBits) * BPS;
+                if constexpr (NQ == 0) {
+                    const float s0 = lds32(addr), s1 = lds32(addr + 4);
+                    accumulate<K>(fmaf(a, s1 - s0, s0), p[0]);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) {
+                        const float4 s0 = lds128(addr + q * quad_bytes);
+                        const float4 s1 = lds128(addr + q * quad_bytes + 16);
+                        accumulate<K>(fmaf(a, s1.x - s0.x, s0.x), p[4 * q + 0]);
+                        accumulate<K>(fmaf(a, s1.y - s0.y, s0.y), p[4 * q + 1]);
+                        accumulate<K>(fmaf(a, s1.z - s0.z, s0.z), p[4 * q + 2]);
+                        accumulate<K>(fmaf(a, s1.w - s0.w, s0.w), p[4 * q + 3]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar0 + 8 * (C.stages + s));
+            if (++s == C.stages) { s = 0; ph ^= 1; }
+        }
+
+        if (j < P.nx && m < P.nz) {
+            const size_t img = (size_t)P.nz * P.nx;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                const int frame = bz * NF + f;
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+            }
+        }
+    }
+}
+
+// ---- host side ----
+inline size_t cached_smem_bytes(const StagedCfg& c, int nq) {
+    const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
+    return 64 + (size_t)c.stages * c.chunk * ((size_t)kCacheBlockBytes + (size_t)c.window * bps * ncopy);
+}
+template <int K, int NQ>
+inline cudaError_t cached_set_attr(int smem_optin) {
+    return cudaFuncSetAttribute(bf_cached_kernel<K, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+}
+inline cudaError_t cached_configure(int smem_optin) {
+    cudaError_t e;
+    if ((e = cached_set_attr<1, 0>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<2, 0>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<3, 0>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<4, 0>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<5, 0>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<1, 4>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<2, 4>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<4, 2>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<5, 2>(smem_optin)) != cudaSuccess) return e;
+    return cached_set_attr<3, 4>(smem_optin);
+}
+template <int K, int NQ>
+inline void launch_cached_k(const BfParams& P, const StagedCfg& c, const uint32_t* taps, const int* w0s, int sm_count,
+                            cudaStream_t st) {
+    const size_t smem = cached_smem_bytes(c, NQ);
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_cached_kernel<K, NQ>, kStgThreads, smem) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
+    bf_cached_kernel<K, NQ><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(P, c, taps, w0s);
+}
+// nq = 0 (orders 1..5), 4 (orders 1..3) or 2 (orders 4, 5)
+inline void launch_cached(int order, int nq, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
+                          int smem_limit, int sm_count, const uint32_t* taps, const int* w0s, cudaStream_t st) {
+    const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + kCacheBlockBytes;
+    long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
+    if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
+    if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
+    if (chunk > P.N) chunk = P.N;
+    if (chunk < 1) chunk = 1;
+    StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
+                (P.nz + kStgRows - 1) / kStgRows, groups};
+    if (nq == 0) {
+        switch (order) {
+        case 1: launch_cached_k<1, 0>(P, c, taps, w0s, sm_count, st); break;
+        case 2: launch_cached_k<2, 0>(P, c, taps, w0s, sm_count, st); break;
+        case 3: launch_cached_k<3, 0>(P, c, taps, w0s, sm_count, st); break;
+        case 4: launch_cached_k<4, 0>(P, c, taps, w0s, sm_count, st); break;
+        default: launch_cached_k<5, 0>(P, c, taps, w0s, sm_count, st); break;
+        }
+    } else if (nq == 2) {
+        if (order == 4) launch_cached_k<4, 2>(P, c, taps, w0s, sm_count, st);
+        else launch_cached_k<5, 2>(P, c, taps, w0s, sm_count, st);
+    } else {
+        switch (order) {
+        case 1: launch_cached_k<1, 4>(P, c, taps, w0s, sm_count, st); break;
+        case 2: launch_cached_k<2, 4>(P, c, taps, w0s, sm_count, st); break;
+        default: launch_cached_k<3, 4>(P, c, taps, w0s, sm_count, st); break;
+        }
+    }
+}
+
+}  // namespace pab

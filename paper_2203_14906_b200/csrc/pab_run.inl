@@ -108,6 +108,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             nq -= groups * g;
         }
     } else if (F < 4) {
+        const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5;
         // lin layout, one frame per thread.  fp32 input with unit scale and 16-byte rows is read in place.
         const bool in_place = ctx->dtype == PAB_F32 && ctx->scale == 1.0f && (S % 4) == 0 &&
                               ((uintptr_t)rf % 16) == 0;
@@ -124,7 +125,9 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         P.n_frames = F;
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
+            if (cached) launch_cached(order, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
+                                      ctx->d_taps, ctx->d_w0s, st);
+            else if (use_staged) launch_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, 0, weight, P, F, st);
         }
     } else {
@@ -148,7 +151,11 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
+            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 &&
+                ((g == 4 && order <= 3) || (g == 2 && (order == 4 || order == 5))))
+                launch_cached(order, g, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
+                              ctx->d_taps, ctx->d_w0s, st);
+            else if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, g, weight, R, groups, st);
             q0 += groups * g;
             nq -= groups * g;

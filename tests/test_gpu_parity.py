@@ -26,8 +26,10 @@ def pab():
     return binding
 
 
-def run_gpu(pab, g, rf, order, variant="auto", dtype="float32", scale=1.0, post=None, weight="none", interp="linear"):
-    bf = pab.Beamformer(g, dtype=dtype, scale=scale, post=post, variant=variant, weight=weight, interp=interp)
+def run_gpu(pab, g, rf, order, variant="auto", dtype="float32", scale=1.0, post=None, weight="none", interp="linear",
+            delay_cache="off"):
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, post=post, variant=variant, weight=weight, interp=interp,
+                        delay_cache=delay_cache)
     try:
         out = bf.beamform(torch.from_numpy(rf).cuda(), order)
         torch.cuda.synchronize()
@@ -127,11 +129,13 @@ def test_c2_full_size_single_frame(pab, orc, variant, order):
     check_raw(gpu[0], orc.beamform(w.rf, w.geom, order)[0], order)
 
 
-def test_c2b_headline_batch_sampled_pixels(pab, orc):
-    """The launch configuration bench.py times (64 frames, order 3, auto variant) on sampled pixels."""
+@pytest.mark.parametrize("delay_cache", ["all", "off"])
+def test_c2b_headline_batch_sampled_pixels(pab, orc, delay_cache):
+    """The launch configuration bench.py times (64 frames, order 3, auto variant, cached taps) on sampled pixels,
+    and the same with in-kernel delays."""
     w = synth.make_config("C2b", n_frames=64)
     g = w.geom
-    gpu, launches = run_gpu(pab, g, w.rf, 3)
+    gpu, launches = run_gpu(pab, g, w.rf, 3, delay_cache=delay_cache)
     assert launches >= 2
     rng = np.random.default_rng(7)
     pix = np.stack([rng.integers(0, g.nz, 1500), rng.integers(0, g.nx, 1500)], axis=1)
@@ -155,7 +159,7 @@ def test_c2b_headline_batch_sampled_pixels(pab, orc):
 def test_c4_large_aperture(pab, orc, variant, order):
     w = synth.make_config("C4")
     g = w.geom
-    gpu, _ = run_gpu(pab, g, w.rf, order, variant)
+    gpu, _ = run_gpu(pab, g, w.rf, order, variant, delay_cache="single" if variant == "staged" else "off")
     rng = np.random.default_rng(11)
     rows = np.unique(np.concatenate([[0, g.nz - 1], rng.integers(0, g.nz, 62)]))
     sub = synth.Geometry(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, g.nx, 1, g.x0, g.dx, g.z0, g.dz)
@@ -481,5 +485,45 @@ def test_beamform_is_cuda_graph_capturable(pab, orc):
         ref = bf.beamform(rf, 3)
         torch.cuda.synchronize()
         assert torch.equal(out, ref)
+    finally:
+        bf.close()
+
+
+# ---- cached interpolation taps (pab_set_delay_cache): the paper's delay table where it wins ----
+@pytest.mark.parametrize("order", [1, 2, 3, 4, 5])
+def test_delay_cache_single_frames_c2(pab, orc, order):
+    w = synth.make_config("C2b", n_frames=3)
+    ref = orc.beamform(w.rf, w.geom, order)
+    for frames in (1, 3):
+        gpu, _ = run_gpu(pab, w.geom, w.rf[:frames], order, delay_cache="single")
+        for f in range(frames):
+            assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
+
+
+def test_delay_cache_ragged_int16_and_batches(pab, orc):
+    rng = np.random.default_rng(41)
+    g = synth.random_geometry(rng, 24, 514, 37, 129, in_range=True)
+    g = synth.Geometry(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, g.nx, g.nz, g.x0, g.dx, max(g.z0, 2e-4), g.dz).f32()
+    rf = rng.integers(-2000, 2000, (21, 24, 514)).astype(np.int16)
+    for mode, frames in (("single", 2), ("all", 21), ("all", 16)):
+        for order in (2, 3):
+            gpu, _ = run_gpu(pab, g, rf[:frames], order, dtype="int16", scale=0.5, delay_cache=mode)
+            ref = orc.beamform(rf[:frames], g, order, scale=0.5)
+            for f in range(frames):
+                check_raw(gpu[f], ref[f], order)
+
+
+def test_delay_cache_c2b_groups_and_fallbacks(pab, orc):
+    w = synth.make_config("C2b", n_frames=20)
+    gpu, _ = run_gpu(pab, w.geom, w.rf, 3, delay_cache="all")                 # one 16-frame group cached + 4 frames not
+    for f in (0, 15, 19):
+        assert check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, 3)[0], 3) <= 2.5e-5
+    gpu, _ = run_gpu(pab, w.geom, w.rf[:1], 3, delay_cache="single", weight="cf")     # weighting: in-kernel delay
+    check_raw(gpu[0], orc.beamform_ex(w.rf[:1], w.geom, 3, weight="cf")[0], 3)
+    c1 = synth.make_config("C1")                                                      # z starts at 0: not in range
+    bf = pab.Beamformer(c1.geom)
+    try:
+        with pytest.raises(pab.PabError):
+            bf.set_delay_cache("single")
     finally:
         bf.close()
