@@ -412,7 +412,8 @@ _TABLE2_MS = {512: (2.912, 3.028, 3.309, 4.4, 5.133), 1024: (11.051, 11.6, 12.71
 def run_table2(args):
     """--table2: square pixel grids shaped like the paper's Table II (512^2, 1024^2, 2048^2), orders 1..5, 128
     elements x 4096 samples, single frames and 16-frame batches, in both delay modes (nearest = the paper's own
-    integer-delay formulation with a delay table, linear = the interpolated path).  One JSON line per case."""
+    integer-delay formulation with a delay table, linear = the interpolated path with cached interpolation taps).
+    One JSON line per case."""
     import torch
     from paper_2203_14906_b200 import binding, synth
     torch.cuda.set_device(0)
@@ -424,7 +425,7 @@ def run_table2(args):
         g = synth.Geometry(N, S, fs, c, pitch, side, side, -19.0e-3, 38.0e-3 / (side - 1), 5e-3, 60e-3 / (side - 1)).f32()
         out = torch.empty((16, side, side), dtype=torch.float32, device="cuda")
         for interp in ("nearest", "linear"):
-            bf = binding.Beamformer(g, interp=interp)
+            bf = binding.Beamformer(g, interp=interp, delay_cache="all" if interp == "linear" else "off")
             for F in (1, 16):
                 for order in (1, 2, 3, 4, 5):
                     rf = rf16[:F]
