@@ -527,3 +527,31 @@ def test_delay_cache_c2b_groups_and_fallbacks(pab, orc):
             bf.set_delay_cache("single")
     finally:
         bf.close()
+
+
+def test_more_frames_than_one_internal_batch(pab, orc):
+    """300 frames of C1: the device entry point loops over internal batches of 256, the host entry point pipelines
+    64-frame pieces (>= 256 frames) -- both must equal the per-frame oracle and each other; repeated create /
+    destroy must give the memory back."""
+    w = synth.make_config("C1", n_frames=300)
+    assert pab.plan(w.geom)["batch_frames"] == 256
+    free0 = torch.cuda.mem_get_info()[0]
+    bf = pab.Beamformer(w.geom)
+    try:
+        dev = bf.beamform(torch.from_numpy(w.rf).cuda(), 3)
+        torch.cuda.synchronize()
+        host = bf.beamform_host(w.rf, 3)
+        assert np.array_equal(dev.cpu().numpy(), host)
+        for f in (0, 255, 256, 299):
+            check_raw(host[f].astype(np.float64), orc.beamform(w.rf[f:f + 1], w.geom, 3)[0], 3)
+    finally:
+        bf.close()
+    del dev
+    torch.cuda.empty_cache()
+    for _ in range(20):
+        b = pab.Beamformer(synth.geometry("C3"), post=dict(mode="log"), interp="linear", delay_cache="single")
+        b.close()
+        b = pab.Beamformer(synth.geometry("C3"), interp="nearest")
+        b.close()
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] >= free0 - 64 * 2 ** 20          # nothing leaked beyond allocator slack
