@@ -101,7 +101,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.chunk_channels,
+            if (use_staged) launch_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.stages, ctx->tuning.chunk_channels,
                                                   ctx->smem_optin, ctx->sm_count, ctx->d_near, st);
             else launch_nearest_direct(order, g, R, groups, ctx->d_near, st);
             q0 += groups * g;
