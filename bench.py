@@ -303,7 +303,13 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         if not args.no_cpu_baseline:
             n_cpu = 16
             cfps, cms, cores = time_oracle(n_cpu, 2, 0)
+            import oracle as _orc
+            _g1, _rf1 = make_inputs(1)
+            _t0 = time.perf_counter()
+            oracle_step(_orc, _rf1, _g1, nthreads=1)
+            single = 1.0 / (time.perf_counter() - _t0)
             line["cpu_baseline"] = {"value": cfps, "unit": "frames/s", "cores": cores, "kind": "oracle",
+                                    "single_thread_value": single,
                                     "sample": f"2 passes over the first {n_cpu} frames of the step's 64-frame C2b batch, "
                                               "fp64 route B + post chain"}
         print(json.dumps(line), flush=True)

@@ -555,3 +555,30 @@ def test_more_frames_than_one_internal_batch(pab, orc):
         b.close()
     torch.cuda.synchronize()
     assert torch.cuda.mem_get_info()[0] >= free0 - 64 * 2 ** 20          # nothing leaked beyond allocator slack
+
+
+def test_constant_rf_closed_form_on_gpu(pab):
+    """Pin P4 on the CUDA path, no oracle involved: constant RF a on every channel gives C(N, k) a (odd k) or
+    C(N, k) |a| (even k) on every in-range pixel (eqs. 1, 2, 4-6: every k-subset product is a^k)."""
+    import math
+    for cfg, orders in (("C1", (1, 2, 3, 4, 5, 6, 7, 8)), ("C2", (1, 2, 3, 4, 5))):
+        g = synth.geometry(cfg)
+        sub = synth.Geometry(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, 16, 64, g.x0, g.dx * (g.nx // 16),
+                             max(g.z0, 2e-3), g.dz * (g.nz // 64) * 0.8).f32()
+        rf = np.full((5, g.n_elem, g.n_samp), -2.5, dtype=np.float32)
+        for order in orders:
+            for frames in (1, 5):
+                gpu, _ = run_gpu(pab, sub, rf[:frames], order)
+                expect = math.comb(g.n_elem, order) * (-2.5 if order % 2 else 2.5)
+                assert np.allclose(gpu, expect, rtol=2e-4), (cfg, order, frames, gpu.flat[0], expect)
+
+
+def test_channel_reversal_symmetry_on_gpu(pab):
+    """Pin P6 on the CUDA path: mirroring the channels and the pixel columns about x = 0 mirrors the image."""
+    w = synth.make_config("C1", n_frames=4)
+    g = w.geom
+    sym = synth.Geometry(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, g.nx, g.nz, -(g.nx - 1) * g.dx / 2, g.dx, 1e-3, g.dz).f32()
+    for order in (2, 3):
+        a, _ = run_gpu(pab, sym, w.rf, order)
+        b, _ = run_gpu(pab, sym, np.ascontiguousarray(w.rf[:, ::-1, :]), order)
+        assert np.max(np.abs(a - b[:, :, ::-1])) <= 2e-5 * np.max(np.abs(a))
