@@ -428,7 +428,8 @@ def run_table2(args):
     N, S, fs, c, pitch = 128, 4096, 40e6, 1540.0, 0.3e-3
     rf16 = torch.from_numpy((rng.standard_normal((16, N, S)) * 0.3).astype(np.float32)).cuda()
     for side in (512, 1024, 2048):
-        g = synth.Geometry(N, S, fs, c, pitch, side, side, -19.0e-3, 38.0e-3 / (side - 1), 5e-3, 60e-3 / (side - 1)).f32()
+        dx = pitch / (side // 128)            # columns on a sub-multiple of the pitch (38.4 mm wide): the taps are then
+        g = synth.Geometry(N, S, fs, c, pitch, side, side, -(side - 1) / 2 * dx, dx, 5e-3, 60e-3 / (side - 1)).f32()   # translation invariant
         out = torch.empty((16, side, side), dtype=torch.float32, device="cuda")
         for interp in ("nearest", "linear"):
             bf = binding.Beamformer(g, interp=interp, delay_cache="all" if interp == "linear" else "off")

@@ -137,7 +137,8 @@ int pab_set_interp(pab_ctx* ctx, int interp);
  * device memory, computed once in fp64, instead of recomputing the delay in every call (PAPER.md:190 keeps its
  * delays in GPU global memory; BASELINE.json north_star allows a cached table "where it wins").  It wins for calls
  * of 1..3 frames, where the in-kernel delay cannot be shared between frames.  4 bytes per (pixel, element):
- * 134 MB at 128 elements x 1024 x 256 pixels.  Linear interpolation, no weighting, orders 1..5 (other settings
+ * 134 MB at 128 elements x 1024 x 256 pixels; when pitch_m is an exact integer multiple q of grid.dx the tap depends
+ * on (column - q * element, row) only and the table shrinks to (nx + q (N-1)) * nz * 8 bytes (2 MB there).  Linear interpolation, no weighting, orders 1..5 (other settings
  * fall back to the in-kernel delay).  In-range geometries only (pab_plan_info.in_range), staged variant.
  * Synchronises the device on the first call.  Errors: PAB_ERR_INVALID, PAB_ERR_ALLOC, PAB_ERR_CUDA. */
 int pab_set_delay_cache(pab_ctx* ctx, int mode);

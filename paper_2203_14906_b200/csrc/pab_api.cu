@@ -34,6 +34,8 @@ struct pab_ctx {
     int cache_mode = PAB_CACHE_OFF;
     uint32_t* d_taps = nullptr;          // cached interpolation taps, tile-major (pab_set_delay_cache)
     int* d_w0s = nullptr;                // window start of every (tile, element)
+    uint2* d_compact = nullptr;          // (d, row) tap table when pitch = q dx exactly (translation invariance)
+    int cache_q = 0;
     void* d_metric = nullptr;            // MetricAcc + double[1] + 2 x 4096 histogram bins (row f3), lazy
     unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
@@ -80,7 +82,7 @@ size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
 
 void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
-    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s);
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact);
     for (int b = 0; b < 2; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -248,22 +250,41 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
     if (!ctx || mode < PAB_CACHE_OFF || mode > PAB_CACHE_ALL) return PAB_ERR_INVALID;
     if (mode != PAB_CACHE_OFF) {
         if (!ctx->plan.in_range || ctx->plan.smem_bytes == 0 || ctx->plan.window_samples > kCacheMaxWindow) return PAB_ERR_INVALID;
-        if (!ctx->d_taps) {
-            const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z = (ctx->grid.nz + kStgRows - 1) / kStgRows;
-            if (tiles_z > 65535 || ctx->N > 65535) return PAB_ERR_INVALID;
-            const size_t blocks = (size_t)tiles_x * tiles_z * ctx->N;
+        const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z = (ctx->grid.nz + kStgRows - 1) / kStgRows;
+        if (tiles_z > 65535 || ctx->N > 65535) return PAB_ERR_INVALID;
+        const size_t blocks = (size_t)tiles_x * tiles_z * ctx->N;
+        // translation invariance: pitch = q dx exactly (both are the floats the ABI carries) -> compact (d, row) table,
+        // used by the one-frame-per-thread kernel (through L1/L2); the frame-group kernels always take the
+        // tile-major table staged by TMA (the compact table's global loads cost them 9 %)
+        const long long q = llround((double)ctx->pitch / (double)ctx->grid.dx);
+        const bool compact = q >= 1 && q <= 64 && (double)ctx->pitch == (double)q * (double)ctx->grid.dx &&
+                             (long long)ctx->grid.nx + q * (ctx->N - 1) <= 65535;
+        const bool need_taps = (mode == PAB_CACHE_ALL || !compact) && !ctx->d_taps;
+        const bool need_w0s = !ctx->d_w0s, need_compact = compact && !ctx->d_compact;
+        if (need_taps || need_w0s || need_compact) {
             PAB_CUDA(ctx, cached_configure(ctx->smem_optin));
-            PAB_CUDA(ctx, cudaMalloc(&ctx->d_taps, blocks * kCacheBlockBytes));
-            cudaError_t e = cudaMalloc(&ctx->d_w0s, blocks * sizeof(int));
+            cudaError_t e = cudaSuccess;
+            if (need_w0s) e = cudaMalloc(&ctx->d_w0s, blocks * sizeof(int));
+            if (e == cudaSuccess && need_taps) e = cudaMalloc(&ctx->d_taps, blocks * kCacheBlockBytes);
+            const int nd = ctx->grid.nx + (int)q * (ctx->N - 1);
+            if (e == cudaSuccess && need_compact) e = cudaMalloc(&ctx->d_compact, (size_t)nd * ctx->grid.nz * sizeof(uint2));
             if (e == cudaSuccess) {
                 CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
                             (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x};
-                delay_cache_kernel<<<dim3(tiles_x, tiles_z, ctx->N), kStgRows * kStgCols>>>(G, ctx->d_taps, ctx->d_w0s);
-                ctx->launches++;
+                if (need_taps || need_w0s) {
+                    delay_cache_kernel<<<dim3(tiles_x, tiles_z, ctx->N), kStgRows * kStgCols>>>(G, ctx->d_taps, ctx->d_w0s);
+                    ctx->launches++;
+                }
+                if (need_compact) {
+                    delay_compact_kernel<<<dim3((ctx->grid.nz + 255) / 256, nd), 256>>>(G, (int)q, ctx->d_compact);
+                    ctx->launches++;
+                    ctx->cache_q = (int)q;
+                }
                 e = cudaDeviceSynchronize();
             }
             if (e != cudaSuccess) {
-                cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); ctx->d_taps = nullptr; ctx->d_w0s = nullptr;
+                cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact);
+                ctx->d_taps = nullptr; ctx->d_w0s = nullptr; ctx->d_compact = nullptr;
                 return cuda_fail(ctx, e, "delay cache");
             }
         }

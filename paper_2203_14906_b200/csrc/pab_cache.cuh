@@ -49,7 +49,21 @@ __global__ void __launch_bounds__(kStgRows * kStgCols) delay_cache_kernel(const 
     const size_t blk = ((size_t)blockIdx.y * G.tiles_x + blockIdx.x) * G.N + i;
     if (threadIdx.x == 0) w0s[blk] = w0;
     const double rel = idx - (double)w0;                                 // >= 0, < window
-    taps[blk * (kStgRows * kStgCols) + threadIdx.x] = (uint32_t)llrint(rel * (double)(1u << kCacheFracBits));
+    if (taps) taps[blk * (kStgRows * kStgCols) + threadIdx.x] = (uint32_t)llrint(rel * (double)(1u << kCacheFracBits));
+}
+
+// Compact table for translation-invariant geometries (pitch = q dx with an integer q, exactly): the lateral offset
+// of (column j, element i) is x0 + (d - q (N-1)/2) dx with d = j - q i + q (N-1), so the tap depends on (d, row)
+// only: nd = nx + q (N-1) columns instead of nx N -- 2 MB instead of 134 MB at C2, resident in L2/L1.
+// compact[d * nz + m] = (floor(idx), fraction as float bits).  grid: (ceil(nz/256), nd)
+__global__ void __launch_bounds__(256) delay_compact_kernel(const CacheGeom G, int q, uint2* __restrict__ compact) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x, d = blockIdx.y;
+    if (m >= G.nz) return;
+    const double z = __dadd_rn(G.z0, __dmul_rn((double)m, G.dz));
+    const double ddx = __dadd_rn(G.x0, __dmul_rn(__dsub_rn((double)d, __dmul_rn((double)q, __ddiv_rn(__dsub_rn((double)G.N, 1.0), 2.0))), G.dx));
+    const double idx = __ddiv_rn(__dmul_rn(G.fs, __dsqrt_rn(__dadd_rn(__dmul_rn(ddx, ddx), __dmul_rn(z, z)))), G.c);
+    const double fl = floor(idx);
+    compact[(size_t)d * G.nz + m] = make_uint2((unsigned)(int)fl, __float_as_uint((float)(idx - fl)));
 }
 
 __device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
@@ -60,18 +74,22 @@ __device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
 
 // NQ = 0: lin layout, one frame per thread; NQ = 4 (orders 1..3) / NQ = 2 (orders 4, 5): quad layout, 16 / 8 frames
 // per thread.  In-range geometries.
-template <int K, int NQ>
+// COMPACT: taps come from the (d, row) table through L1/L2 (q = pitch / dx), only the window starts are staged.
+template <int K, int NQ, bool COMPACT>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParams P, const StagedCfg C,
                                                                     const uint32_t* __restrict__ taps,
-                                                                    const int* __restrict__ w0s) {
+                                                                    const int* __restrict__ w0s,
+                                                                    const uint2* __restrict__ compact, int q) {
     constexpr int NF = NQ == 0 ? 1 : 4 * NQ;
     constexpr int BPS = NQ == 0 ? 4 : 16;
     constexpr int NCOPY = NQ == 0 ? 1 : NQ;
     extern __shared__ __align__(128) unsigned char stg_smem[];
     unsigned char* smem = stg_smem;
     const uint32_t bar0 = smem_u32(smem);
-    const uint32_t ctab0 = bar0 + 64;                                    // [stages][chunk][512] uint32
-    const uint32_t data0 = ctab0 + C.stages * C.chunk * kCacheBlockBytes;
+    // [stages][chunk] blocks of 512 uint32 taps, or (COMPACT) [stages][chunk] window starts
+    constexpr int kBlk = COMPACT ? 4 : kCacheBlockBytes;
+    const uint32_t ctab0 = bar0 + 64;
+    const uint32_t data0 = ctab0 + ((C.stages * C.chunk * kBlk + 127) & ~127);
     const int quad_bytes = C.window * BPS;
     const int slot_bytes = quad_bytes * NCOPY;
     const int stage_bytes = C.chunk * slot_bytes;
@@ -108,9 +126,14 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                     const int len = min(C.window, row_len - w0);
                     const uint32_t bytes = (uint32_t)len * BPS;
                     const int slot = s * stage_bytes + lane * slot_bytes;
-                    mbar_arrive_expect_tx(full, bytes * NCOPY + kCacheBlockBytes);
-                    bulk_g2s(ctab0 + (s * C.chunk + lane) * kCacheBlockBytes,
-                             taps + (blk0 + ch) * (size_t)(kStgRows * kStgCols), kCacheBlockBytes, full);
+                    if constexpr (COMPACT) {
+                        asm volatile("st.shared.u32 [%0], %1;" ::"r"(ctab0 + (s * C.chunk + lane) * 4), "r"(w0) : "memory");
+                        mbar_arrive_expect_tx(full, bytes * NCOPY);
+                    } else {
+                        mbar_arrive_expect_tx(full, bytes * NCOPY + kCacheBlockBytes);
+                        bulk_g2s(ctab0 + (s * C.chunk + lane) * kCacheBlockBytes,
+                                 taps + (blk0 + ch) * (size_t)(kStgRows * kStgCols), kCacheBlockBytes, full);
+                    }
                     const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
 #pragma unroll
                     for (int q = 0; q < NCOPY; ++q)
@@ -138,18 +161,30 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
         for (int f = 0; f < NF; ++f)
 #pragma unroll
             for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+        // COMPACT: this pixel's row of the (d, row) table; d = j - q i + q (N - 1) falls by q per element
+        const uint2* cp = compact + ((size_t)(min(j, P.nx - 1) + q * (P.N - 1)) * P.nz + min(m, P.nz - 1));
+        const size_t cstep = (size_t)q * P.nz;
 
         for (int ck = 0; ck < n_chunks; ++ck) {
-            mbar_wait(bar0 + 8 * s, ph);
             const int nch = min(C.chunk, P.N - ck * C.chunk);
-            const uint32_t ctab_s = ctab0 + s * C.chunk * kCacheBlockBytes + my;
+            const uint2* cpk = cp - (size_t)(ck * C.chunk) * cstep;
+            mbar_wait(bar0 + 8 * s, ph);
+            const uint32_t ctab_s = ctab0 + s * C.chunk * kBlk + (COMPACT ? 0u : my);
             const uint32_t data_s = data0 + s * stage_bytes;
             constexpr int kElemUnroll = NQ >= 4 ? 2 : 4;
 #pragma unroll (kElemUnroll)
             for (int l = 0; l < nch; ++l) {
-                const uint32_t e = lds32u(ctab_s + l * kCacheBlockBytes);
-                const float a = __uint_as_float(0x3F800000u | ((e << (32 - kCacheFracBits)) >> 9)) - 1.0f;   // fraction, exact
-                const uint32_t addr = data_s + l * slot_bytes + (e >> kCacheFracBits) * BPS;
+                float a;
+                uint32_t addr;
+                if constexpr (COMPACT) {
+                    const uint2 e = __ldg(cpk - (size_t)l * cstep);
+                    a = __uint_as_float(e.y);
+                    addr = data_s + l * slot_bytes + ((int)e.x - (int)lds32u(ctab_s + l * 4)) * BPS;
+                } else {
+                    const uint32_t e = lds32u(ctab_s + l * kCacheBlockBytes);
+                    a = __uint_as_float(0x3F800000u | ((e << (32 - kCacheFracBits)) >> 9)) - 1.0f;          // fraction, exact
+                    addr = data_s + l * slot_bytes + (e >> kCacheFracBits) * BPS;
+                }
                 if constexpr (NQ == 0) {
                     const float s0 = lds32(addr), s1 = lds32(addr + 4);
                     accumulate<K>(fmaf(a, s1 - s0, s0), p[0]);
@@ -182,13 +217,16 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 }
 
 // ---- host side ----
-inline size_t cached_smem_bytes(const StagedCfg& c, int nq) {
+inline size_t cached_smem_bytes(const StagedCfg& c, int nq, bool compact) {
     const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
-    return 64 + (size_t)c.stages * c.chunk * ((size_t)kCacheBlockBytes + (size_t)c.window * bps * ncopy);
+    const size_t blk = compact ? 4 : kCacheBlockBytes;
+    return 64 + (((size_t)c.stages * c.chunk * blk + 127) & ~(size_t)127) + (size_t)c.stages * c.chunk * (size_t)c.window * bps * ncopy;
 }
 template <int K, int NQ>
 inline cudaError_t cached_set_attr(int smem_optin) {
-    return cudaFuncSetAttribute(bf_cached_kernel<K, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(bf_cached_kernel<K, NQ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(bf_cached_kernel<K, NQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 inline cudaError_t cached_configure(int smem_optin) {
     cudaError_t e;
@@ -203,22 +241,33 @@ inline cudaError_t cached_configure(int smem_optin) {
     if ((e = cached_set_attr<5, 2>(smem_optin)) != cudaSuccess) return e;
     return cached_set_attr<3, 4>(smem_optin);
 }
-template <int K, int NQ>
-inline void launch_cached_k(const BfParams& P, const StagedCfg& c, const uint32_t* taps, const int* w0s, int sm_count,
-                            cudaStream_t st) {
-    const size_t smem = cached_smem_bytes(c, NQ);
+struct CacheTables {
+    const uint32_t* taps;      // tile-major 12+20-bit taps, or nullptr when the compact table is in use
+    const int* w0s;            // window start of every (tile, element)
+    const uint2* compact;      // (d, row) table of translation-invariant geometries, or nullptr
+    int q;                     // pitch / dx
+};
+template <int K, int NQ, bool COMPACT>
+inline void launch_cached_kc(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    const size_t smem = cached_smem_bytes(c, NQ, COMPACT);
     int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_cached_kernel<K, NQ>, kStgThreads, smem) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_cached_kernel<K, NQ, COMPACT>, kStgThreads, smem) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
         per_sm = 1;
     }
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
-    bf_cached_kernel<K, NQ><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(P, c, taps, w0s);
+    bf_cached_kernel<K, NQ, COMPACT><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
+        P, c, T.taps, T.w0s, T.compact, T.q);
+}
+template <int K, int NQ>
+inline void launch_cached_k(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    if (T.compact) launch_cached_kc<K, NQ, true>(P, c, T, sm_count, st);
+    else launch_cached_kc<K, NQ, false>(P, c, T, sm_count, st);
 }
 // nq = 0 (orders 1..5), 4 (orders 1..3) or 2 (orders 4, 5)
 inline void launch_cached(int order, int nq, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
-                          int smem_limit, int sm_count, const uint32_t* taps, const int* w0s, cudaStream_t st) {
-    const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + kCacheBlockBytes;
+                          int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
+    const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (T.compact ? 4 : kCacheBlockBytes);
     long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
     if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
     if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
@@ -228,20 +277,20 @@ inline void launch_cached(int order, int nq, const BfParams& P, int groups, cons
                 (P.nz + kStgRows - 1) / kStgRows, groups};
     if (nq == 0) {
         switch (order) {
-        case 1: launch_cached_k<1, 0>(P, c, taps, w0s, sm_count, st); break;
-        case 2: launch_cached_k<2, 0>(P, c, taps, w0s, sm_count, st); break;
-        case 3: launch_cached_k<3, 0>(P, c, taps, w0s, sm_count, st); break;
-        case 4: launch_cached_k<4, 0>(P, c, taps, w0s, sm_count, st); break;
-        default: launch_cached_k<5, 0>(P, c, taps, w0s, sm_count, st); break;
+        case 1: launch_cached_k<1, 0>(P, c, T, sm_count, st); break;
+        case 2: launch_cached_k<2, 0>(P, c, T, sm_count, st); break;
+        case 3: launch_cached_k<3, 0>(P, c, T, sm_count, st); break;
+        case 4: launch_cached_k<4, 0>(P, c, T, sm_count, st); break;
+        default: launch_cached_k<5, 0>(P, c, T, sm_count, st); break;
         }
     } else if (nq == 2) {
-        if (order == 4) launch_cached_k<4, 2>(P, c, taps, w0s, sm_count, st);
-        else launch_cached_k<5, 2>(P, c, taps, w0s, sm_count, st);
+        if (order == 4) launch_cached_k<4, 2>(P, c, T, sm_count, st);
+        else launch_cached_k<5, 2>(P, c, T, sm_count, st);
     } else {
         switch (order) {
-        case 1: launch_cached_k<1, 4>(P, c, taps, w0s, sm_count, st); break;
-        case 2: launch_cached_k<2, 4>(P, c, taps, w0s, sm_count, st); break;
-        default: launch_cached_k<3, 4>(P, c, taps, w0s, sm_count, st); break;
+        case 1: launch_cached_k<1, 4>(P, c, T, sm_count, st); break;
+        case 2: launch_cached_k<2, 4>(P, c, T, sm_count, st); break;
+        default: launch_cached_k<3, 4>(P, c, T, sm_count, st); break;
         }
     }
 }

@@ -126,7 +126,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
             if (cached) launch_cached(order, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
-                                      ctx->d_taps, ctx->d_w0s, st);
+                                      CacheTables{ctx->d_taps, ctx->d_w0s, ctx->d_compact, ctx->cache_q}, st);
             else if (use_staged) launch_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, 0, weight, P, F, st);
         }
@@ -154,7 +154,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 &&
                 ((g == 4 && order <= 3) || (g == 2 && (order == 4 || order == 5))))
                 launch_cached(order, g, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
-                              ctx->d_taps, ctx->d_w0s, st);
+                              CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);
             else if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, g, weight, R, groups, st);
             q0 += groups * g;
