@@ -50,7 +50,7 @@ XU_PER_ITEM = 2.0
 FP32_PER_ITEM = 6.0
 DELAY_CACHE = "all"
 SM_COUNT = 148
-NCU_TRAFFIC_BYTES = 184_726_272 + 51_387_904   # per 64-frame launch; profiles/r1_beamform_ncu_c.md
+NCU_TRAFFIC_BYTES = 183_477_760 + 52_702_464   # per 64-frame launch; profiles/r1_beamform_ncu_c.md
 XU_LANES_PER_CLK_SM = 16
 FP32_LANES_PER_CLK_SM = 128
 
@@ -269,7 +269,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         t_fp32 = items_per_launch * FP32_PER_ITEM / fp32_peak
         t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
         achieved = items_per_launch * XU_PER_ITEM / (bf_launch_ms * 1e-3)
-        roofline = {"bound": "alu", "kernel": "bf_cached_kernel<3,4> (fused tap fetch + interpolation + root + power sums + Newton, 16 frames "
+        roofline = {"bound": "alu", "kernel": "bf_cached_kernel<3,4,false> (fused tap fetch + interpolation + root + power sums + Newton, 16 frames "
                               "per thread, cached interpolation taps)",
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
                     "frac": achieved / xu_peak, "traffic": NCU_TRAFFIC_BYTES,
