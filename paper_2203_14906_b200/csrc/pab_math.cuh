@@ -57,18 +57,17 @@ __device__ __forceinline__ void accumulate(float s, float (&p)[K]) {
         p[3] = fmaf(u2, u2, p[3]);
         p[4] += s;
     } else {
-        // Row f2, orders above 5 ("this can be done for higher orders as well"): the same scheme,
-        // p_m += u^m for m < K and p_K += s (odd K) or |s| (even K).
+        // Row f2, orders above 5 ("this can be done for higher orders as well").  The power-sum /
+        // Newton form loses accuracy to cancellation as k grows (fp32, absorber-free noise frames: 1e-4 at k = 5,
+        // 1e-3 at k = 8), so these orders carry the elementary symmetric sums themselves: E_j += u E_(j-1) for
+        // j = K..1 (E_0 = 1), O(N) per pixel like the paper's forms, K FMAs per sample, no cancellation.
+        // p[j-1] holds E_j; combine<K> returns p[K-1].
         static_assert(K >= 6 && K <= 8, "orders 1..8");
         const float r = ex2_approx(lg2_approx(fabsf(s)) * (1.0f / (float)K));
         const float u = copy_sign(r, s);
-        float pw = u;
 #pragma unroll
-        for (int m = 0; m < K - 1; ++m) {
-            p[m] += pw;
-            pw *= u;
-        }
-        p[K - 1] += (K & 1) ? s : fabsf(s);
+        for (int j = K - 1; j >= 1; --j) p[j] = fmaf(u, p[j - 1], p[j]);
+        p[0] += u;
     }
 }
 
@@ -88,19 +87,7 @@ __device__ __forceinline__ float combine(const float (&p)[K]) {
                 const float e4 = 0.25f * ((fmaf(e3, p[0], -e2 * p[1]) + e1 * p[2]) - p[3]);
                 if constexpr (K == 4) return e4;
                 else if constexpr (K == 5) return 0.2f * (((fmaf(e4, p[0], -e3 * p[1]) + e2 * p[2]) - e1 * p[3]) + p[4]);
-                else {
-                    // orders 6..8: the recursion m e_m = sum_{i=1..m} (-1)^(i-1) e_{m-i} p_i written as a loop
-                    float e[K + 1];
-                    e[0] = 1.0f;
-#pragma unroll
-                    for (int m = 1; m <= K; ++m) {
-                        float acc = 0.0f;
-#pragma unroll
-                        for (int i = 1; i <= m; ++i) acc = (i & 1) ? fmaf(e[m - i], p[i - 1], acc) : fmaf(-e[m - i], p[i - 1], acc);
-                        e[m] = acc / (float)m;
-                    }
-                    return e[K];
-                }
+                else return p[K - 1];       // orders 6..8 carry E_1..E_K directly (accumulate<K>)
             }
         }
     }
