@@ -51,7 +51,7 @@ extern "C" {
 /* cached interpolation taps (pab_set_delay_cache) */
 #define PAB_CACHE_OFF    0   /* delays computed in-kernel on every call; default                                   */
 #define PAB_CACHE_SINGLE 1   /* calls of 1..3 frames read their taps from the cached table                         */
-#define PAB_CACHE_ALL    2   /* ... and so do the 16-frame (orders 1..3) / 8-frame (orders 4, 5) groups of longer calls */
+#define PAB_CACHE_ALL    2   /* ... and so do the frame groups of longer calls                                      */
 
 /* pixel weighting (pab_set_weight) */
 #define PAB_WEIGHT_NONE 0   /* out = e_k                                                                          */

@@ -228,18 +228,23 @@ inline cudaError_t cached_set_attr(int smem_optin) {
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(bf_cached_kernel<K, NQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
+// instantiated: NQ = 0 for orders 1..5; NQ = 1, 2 for orders 1..5; NQ = 4 for orders 1..3
+template <int K>
+inline cudaError_t cached_set_attr_k(int smem_optin) {
+    cudaError_t e;
+    if ((e = cached_set_attr<K, 0>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<K, 1>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr<K, 2>(smem_optin)) != cudaSuccess) return e;
+    if constexpr (K <= 3) return cached_set_attr<K, 4>(smem_optin);
+    else return cudaSuccess;
+}
 inline cudaError_t cached_configure(int smem_optin) {
     cudaError_t e;
-    if ((e = cached_set_attr<1, 0>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<2, 0>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<3, 0>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<4, 0>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<5, 0>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<1, 4>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<2, 4>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<4, 2>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cached_set_attr<5, 2>(smem_optin)) != cudaSuccess) return e;
-    return cached_set_attr<3, 4>(smem_optin);
+    if ((e = cached_set_attr_k<1>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr_k<2>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr_k<3>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cached_set_attr_k<4>(smem_optin)) != cudaSuccess) return e;
+    return cached_set_attr_k<5>(smem_optin);
 }
 struct CacheTables {
     const uint32_t* taps;      // tile-major 12+20-bit taps, or nullptr when the compact table is in use
@@ -264,7 +269,14 @@ inline void launch_cached_k(const BfParams& P, const StagedCfg& c, const CacheTa
     if (T.compact) launch_cached_kc<K, NQ, true>(P, c, T, sm_count, st);
     else launch_cached_kc<K, NQ, false>(P, c, T, sm_count, st);
 }
-// nq = 0 (orders 1..5), 4 (orders 1..3) or 2 (orders 4, 5)
+template <int K>
+inline void launch_cached_nq(int nq, const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    if (nq == 0) launch_cached_k<K, 0>(P, c, T, sm_count, st);
+    else if (nq == 1) launch_cached_k<K, 1>(P, c, T, sm_count, st);
+    else if (nq == 2) launch_cached_k<K, 2>(P, c, T, sm_count, st);
+    else if constexpr (K <= 3) launch_cached_k<K, 4>(P, c, T, sm_count, st);
+}
+// nq = 0, 1, 2 (orders 1..5) or 4 (orders 1..3)
 inline void launch_cached(int order, int nq, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
                           int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (T.compact ? 4 : kCacheBlockBytes);
@@ -275,23 +287,12 @@ inline void launch_cached(int order, int nq, const BfParams& P, int groups, cons
     if (chunk < 1) chunk = 1;
     StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
                 (P.nz + kStgRows - 1) / kStgRows, groups};
-    if (nq == 0) {
-        switch (order) {
-        case 1: launch_cached_k<1, 0>(P, c, T, sm_count, st); break;
-        case 2: launch_cached_k<2, 0>(P, c, T, sm_count, st); break;
-        case 3: launch_cached_k<3, 0>(P, c, T, sm_count, st); break;
-        case 4: launch_cached_k<4, 0>(P, c, T, sm_count, st); break;
-        default: launch_cached_k<5, 0>(P, c, T, sm_count, st); break;
-        }
-    } else if (nq == 2) {
-        if (order == 4) launch_cached_k<4, 2>(P, c, T, sm_count, st);
-        else launch_cached_k<5, 2>(P, c, T, sm_count, st);
-    } else {
-        switch (order) {
-        case 1: launch_cached_k<1, 4>(P, c, T, sm_count, st); break;
-        case 2: launch_cached_k<2, 4>(P, c, T, sm_count, st); break;
-        default: launch_cached_k<3, 4>(P, c, T, sm_count, st); break;
-        }
+    switch (order) {
+    case 1: launch_cached_nq<1>(nq, P, c, T, sm_count, st); break;
+    case 2: launch_cached_nq<2>(nq, P, c, T, sm_count, st); break;
+    case 3: launch_cached_nq<3>(nq, P, c, T, sm_count, st); break;
+    case 4: launch_cached_nq<4>(nq, P, c, T, sm_count, st); break;
+    default: launch_cached_nq<5>(nq, P, c, T, sm_count, st); break;
     }
 }
 

@@ -151,8 +151,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 &&
-                ((g == 4 && order <= 3) || (g == 2 && (order == 4 || order == 5))))
+            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 && order <= 5)
                 launch_cached(order, g, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                               CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);
             else if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
