@@ -253,8 +253,12 @@ extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames
     }
     // Double-buffered: H2D of batch b+1 and D2H of batch b-1 overlap the kernels of batch b.
     int it = 0;
-    for (int f0 = 0; f0 < n_frames; f0 += B, ++it) {
-        const int F = n_frames - f0 < B ? n_frames - f0 : B;
+    // The first and the last piece are half pieces (when there are enough frames): the pipeline starts computing and
+    // starts its last device-to-host copy sooner.
+    const bool ramp = B >= 8 && n_frames >= 4 * B;
+    for (int f0 = 0, F = 0; f0 < n_frames; f0 += F, ++it) {
+        F = n_frames - f0 < B ? n_frames - f0 : B;
+        if (ramp && (f0 == 0 || n_frames - f0 <= B)) F = (f0 == 0 || n_frames - f0 > B / 2) ? B / 2 : n_frames - f0;
         const int b = it & 1;
         if (it >= 2) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_run[b], 0));   // d_in[b] consumed
         PAB_CUDA(ctx, cudaMemcpyAsync(ctx->d_in[b], (const char*)rf_host + (size_t)f0 * frame_in, (size_t)F * frame_in,
