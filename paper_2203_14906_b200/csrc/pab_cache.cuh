@@ -269,6 +269,13 @@ inline void launch_cached_k(const BfParams& P, const StagedCfg& c, const CacheTa
     if (T.compact) launch_cached_kc<K, NQ, true>(P, c, T, sm_count, st);
     else launch_cached_kc<K, NQ, false>(P, c, T, sm_count, st);
 }
+// does at least one channel per stage fit in shared memory for this group size?  (the tap block makes the slot larger
+// than the plain staged kernel's, so a geometry whose plan has chunk 1 may not fit here: the caller falls back)
+inline bool cached_fits(const pab_plan_info& plan, int nq, bool compact, int smem_limit) {
+    const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (compact ? 4 : kCacheBlockBytes);
+    return plan.stages > 0 && (long long)(smem_limit - 64 - 128) / (plan.stages * slot) >= 1;
+}
+
 template <int K>
 inline void launch_cached_nq(int nq, const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
     if (nq == 0) launch_cached_k<K, 0>(P, c, T, sm_count, st);

@@ -339,6 +339,12 @@ inline void launch_nearest_staged_inr(int order, int nq, const BfParams& P, cons
     default: launch_nearest_staged_nq<5, INR>(nq, P, c, table, sm_count, smem_optin, st); break;
     }
 }
+inline bool nearest_staged_fits(const pab_plan_info& plan, int nq, int stages, int smem_limit) {
+    if (stages <= 0) stages = 2;
+    const long long slot = (long long)plan.window_samples * 16 * nq + (long long)sizeof(ChanEntry) + kNearBlockBytes;
+    return (long long)(smem_limit - 64 - 128) / (stages * slot) >= 1;
+}
+
 // nq = 1, 2 or 4 quads per thread (4 only for orders <= 3)
 inline void launch_nearest_staged(int order, int nq, bool in_range, const BfParams& P, int groups, const pab_plan_info& plan,
                                   int stages, int chunk_cap, int smem_limit, int sm_count, const unsigned short* table,

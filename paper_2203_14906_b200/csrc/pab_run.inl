@@ -101,14 +101,16 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged) launch_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.stages, ctx->tuning.chunk_channels,
+            if (use_staged && nearest_staged_fits(ctx->plan, g, ctx->tuning.stages, ctx->smem_optin))
+                launch_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.stages, ctx->tuning.chunk_channels,
                                                   ctx->smem_optin, ctx->sm_count, ctx->d_near, st);
             else launch_nearest_direct(order, g, R, groups, ctx->d_near, st);
             q0 += groups * g;
             nq -= groups * g;
         }
     } else if (F < 4) {
-        const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5;
+        const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
+                            cached_fits(ctx->plan, 0, ctx->d_compact != nullptr, ctx->smem_optin);
         // lin layout, one frame per thread.  fp32 input with unit scale and 16-byte rows is read in place.
         const bool in_place = ctx->dtype == PAB_F32 && ctx->scale == 1.0f && (S % 4) == 0 &&
                               ((uintptr_t)rf % 16) == 0;
@@ -151,7 +153,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 && order <= 5)
+            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 && order <= 5 &&
+                cached_fits(ctx->plan, g, false, ctx->smem_optin))
                 launch_cached(order, g, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                               CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);
             else if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);

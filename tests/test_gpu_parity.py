@@ -582,3 +582,26 @@ def test_channel_reversal_symmetry_on_gpu(pab):
         a, _ = run_gpu(pab, sym, w.rf, order)
         b, _ = run_gpu(pab, sym, np.ascontiguousarray(w.rf[:, ::-1, :]), order)
         assert np.max(np.abs(a - b[:, :, ::-1])) <= 2e-5 * np.max(np.abs(a))
+
+
+@pytest.mark.parametrize("mode", ["cache-all", "cache-single", "nearest", "plain"])
+def test_coarse_rows_large_window_fallbacks(pab, orc, mode):
+    """Rows 1.07 mm apart: a tile needs a 1792-sample window per channel, one channel per stage fills shared memory.
+    The cached-tap and nearest kernels need room for their table block on top and must fall back (found by a
+    randomised sweep: the launch used to fail with 'invalid argument')."""
+    g = synth.Geometry(25, 1978, 40e6, 1540.0, 0.0002074896910926327, 79, 46, -0.00404604896903038,
+                       0.00010374484554631636, 0.01058073341846466, 0.0010749740758910775).f32()
+    assert pab.plan(g)["window_samples"] >= 1500 and pab.plan(g)["chunk_channels"] == 1
+    rng = np.random.default_rng(77)
+    base = [(rng.uniform(-3e-3, 3e-3), rng.uniform(0.02, 0.05), 1.0, 0.0) for _ in range(3)]
+    rf, _ = synth._frames(rng, g, base, 5e6, 17, 20.0, True)
+    kw, okw = {}, {}
+    if mode == "nearest":
+        kw["interp"] = okw["interp"] = "nearest"
+    elif mode.startswith("cache"):
+        kw["delay_cache"] = mode[6:]
+    for frames in (1, 17):
+        gpu, _ = run_gpu(pab, g, rf[:frames], 3, **kw)
+        ref = orc.beamform_ex(rf[:frames], g, 3, **okw)
+        for f in range(frames):
+            check_raw(gpu[f], ref[f], 3)
