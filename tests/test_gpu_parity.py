@@ -605,3 +605,49 @@ def test_coarse_rows_large_window_fallbacks(pab, orc, mode):
         ref = orc.beamform_ex(rf[:frames], g, 3, **okw)
         for f in range(frames):
             check_raw(gpu[f], ref[f], 3)
+
+
+def test_randomised_api_sweep(pab, orc):
+    """80 seeded random small cases over every option of the API (a short version of the sweeps DESIGN.md section 11
+    describes): nothing may raise, every output is finite, and every image is grossly right (3 % relative L2 against
+    the oracle; white-noise RF, so the tight tolerances do not apply: see 'Conditioning')."""
+    rng = np.random.default_rng(2024)
+    for case in range(80):
+        n_elem = int(rng.choice([1, 2, 5, 16, 33, 64, 129])); n_samp = int(rng.choice([3, 17, 64, 333, 1024, 2047]))
+        nx = int(rng.choice([1, 2, 7, 8, 9, 31, 64])); nz = int(rng.choice([1, 2, 31, 32, 33, 64, 65, 130]))
+        g = synth.random_geometry(rng, n_elem, max(n_samp, 8), nx, nz, in_range=bool(rng.integers(0, 2)))
+        g = synth.Geometry(g.n_elem, n_samp, g.fs, g.c, g.pitch, g.nx, g.nz, g.x0, g.dx,
+                           g.z0 if rng.integers(0, 4) else 0.0, g.dz).f32()
+        F = int(rng.choice([1, 2, 3, 4, 7, 8, 16, 17, 33]))
+        order = int(rng.integers(1, 9))
+        dtype = str(rng.choice(["float32", "int16"]))
+        rf = ((rng.standard_normal((F, n_elem, n_samp)) * 300).astype(np.int16) if dtype == "int16"
+              else rng.standard_normal((F, n_elem, n_samp)).astype(np.float32))
+        mode = "plain" if order > 5 else str(rng.choice(["plain", "cf", "nearest", "cache-single", "cache-all"]))
+        kw, okw = dict(dtype=dtype), {}
+        if mode == "cf":
+            kw["weight"] = okw["weight"] = "cf"
+        if mode == "nearest":
+            kw["interp"] = okw["interp"] = "nearest"
+        bf = pab.Beamformer(g, **kw)
+        try:
+            try:
+                bf.set_variant(str(rng.choice(["auto", "direct", "staged"])))
+            except pab.PabError:
+                pass                                      # staged not available for this geometry
+            if mode.startswith("cache"):
+                try:
+                    bf.set_delay_cache(mode[6:])
+                except pab.PabError:
+                    pass                                  # not an in-range geometry
+            if rng.integers(0, 4) == 0:
+                out = np.asarray(bf.beamform_host(rf, order)).astype(np.float64)
+            else:
+                out = bf.beamform(torch.from_numpy(rf).cuda(), order).cpu().numpy().astype(np.float64)
+        finally:
+            bf.close()
+        assert np.all(np.isfinite(out)), (case, mode, order)
+        ref = orc.beamform_ex(rf, g, order, **okw)
+        den = np.sqrt(np.sum(ref ** 2))
+        if den > 0:
+            assert np.sqrt(np.sum((out - ref) ** 2)) / den <= 3e-2, (case, mode, order, F, g)
