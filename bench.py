@@ -181,7 +181,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    binding.load()                                  # raises when libpab.so is missing
+    binding.load(build_if_missing=True)             # nvcc-builds libpab.so if absent; raises when it cannot (no fallback)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
@@ -331,7 +331,7 @@ def run_sweep(args):
     import torch
     from paper_2203_14906_b200 import binding, synth
     torch.cuda.set_device(0)
-    binding.load()
+    binding.load(build_if_missing=True)
     peaks = read_peaks()
     f_hz = peaks["sm_max_mhz"] * 1e6
     cases = [("C1", 1, (1, 2, 3, 4, 5), False, "none"), ("C2", 1, (1, 2, 3), False, "none"),
@@ -423,7 +423,7 @@ def run_table2(args):
     import torch
     from paper_2203_14906_b200 import binding, synth
     torch.cuda.set_device(0)
-    binding.load()
+    binding.load(build_if_missing=True)
     rng = np.random.default_rng(1020)
     N, S, fs, c, pitch = 128, 4096, 40e6, 1540.0, 0.3e-3
     rf16 = torch.from_numpy((rng.standard_normal((16, N, S)) * 0.3).astype(np.float32)).cuda()

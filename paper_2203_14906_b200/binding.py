@@ -62,7 +62,7 @@ def load(build_if_missing: bool = False):
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_missing:
+    if build_if_missing and not os.path.exists(LIB_PATH):
         from . import build as _b
         _b.build_lib()
     if not os.path.exists(LIB_PATH):

@@ -34,6 +34,15 @@ def is_stale() -> bool:
 def build_lib(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
+    import fcntl
+    with open(LIB + ".lock", "w") as lock:            # several ranks may get here at once: one builds, the rest wait
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and not is_stale():
+            return LIB
+        return _build_locked(verbose)
+
+
+def _build_locked(verbose: bool) -> str:
     cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
            "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
     if verbose:

@@ -22,7 +22,7 @@ def pab():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     from paper_2203_14906_b200 import binding
-    binding.load()          # raises if libpab.so is missing: no fallback
+    binding.load(build_if_missing=True)     # compiles libpab.so with nvcc if it is not there; raises if it cannot: no fallback
     return binding
 
 
