@@ -15,17 +15,18 @@ struct PostTaps64 {
     float hh[64];   // Hilbert taps g[t' ] = g(t' - L), zero-padded
 };
 
-// 8 consecutive output rows m0..m0+7 of one column: out[m] = sum_t taps[t] in[m + shift - t], t < 64.
+// R (8 or 16) consecutive output rows m0..m0+R-1 of one column: out[m] = sum_t taps[t] in[m + shift - t], t < 64, from
+// an (R + 7)-row register window that slides 8 rows per block of 8 taps: 8 R FMAs per 8 shared loads.
 // PAR = 0 / 1: only taps of that index parity are non-zero; PAR = 2: dense.
-template <int PAR>
-__device__ __forceinline__ void fir8_c64(const float* in_col, int in_r0, const float (&taps)[64], int shift, int m0,
-                                         float (&acc)[8]) {
+template <int R, int PAR>
+__device__ __forceinline__ void fir_c64(const float* in_col, int in_r0, const float (&taps)[64], int shift, int m0,
+                                        float (&acc)[R]) {
     const float* base = in_col + (m0 + shift - in_r0) * 32;
-    float w[15];
+    float w[R + 7];
 #pragma unroll
-    for (int e = 0; e < 7; ++e) w[8 + e] = base[(1 + e) * 32];
+    for (int e = 0; e < R - 1; ++e) w[8 + e] = base[(1 + e) * 32];
 #pragma unroll
-    for (int r = 0; r < 8; ++r) acc[r] = 0.0f;
+    for (int r = 0; r < R; ++r) acc[r] = 0.0f;
 #pragma unroll
     for (int tb = 0; tb < 64; tb += 8) {
 #pragma unroll
@@ -35,11 +36,11 @@ __device__ __forceinline__ void fir8_c64(const float* in_col, int in_r0, const f
             if (PAR == 2 || ((tb + tt) & 1) == PAR) {
                 const float h = taps[tb + tt];
 #pragma unroll
-                for (int r = 0; r < 8; ++r) acc[r] = fmaf(h, w[r - tt + 7], acc[r]);
+                for (int r = 0; r < R; ++r) acc[r] = fmaf(h, w[r - tt + 7], acc[r]);
             }
         }
 #pragma unroll
-        for (int d = 6; d >= 0; --d) w[d + 8] = w[d];
+        for (int d = R - 2; d >= 0; --d) w[d + 8] = w[d];
     }
 }
 
@@ -76,31 +77,45 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
         }
     }
     __syncthreads();
-    float acc[8];
+    // every warp owns a slab of consecutive rows: 32 output rows (two 16-row groups), and with the envelope 40 rows of
+    // the band-pass intermediate (16 + 16 + 8): the same work for all 8 warps
+    static_assert(TZ == 256, "the row slabs below assume 256-row tiles and 8 warps");
+    float a16[16], a8[8];
     if constexpr (!ENV) {
-        for (int g = warp; g < TZ / 8; g += 8) {
-            const int m0 = r0 + g * 8;
-            fir8_c64<2>(xs + lane, xr0, T.hb, P.shiftB, m0, acc);
+#pragma unroll 1
+        for (int g = 0; g < 2; ++g) {
+            const int m0 = r0 + warp * 32 + g * 16;
+            fir_c64<16, 2>(xs + lane, xr0, T.hb, P.shiftB, m0, a16);
 #pragma unroll
-            for (int r = 0; r < 8; ++r)
-                if (m0 + r < P.nz && col < P.nx) P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = acc[r];
+            for (int r = 0; r < 16; ++r)
+                if (m0 + r < P.nz && col < P.nx) P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = a16[r];
         }
     } else {
-        for (int g = warp; g < YR / 8; g += 8) {
-            const int m0 = yr0 + g * 8;
-            fir8_c64<2>(xs + lane, xr0, T.hb, P.shiftB, m0, acc);
+        static_assert(!ENV || YR == 320, "band-pass intermediate: 8 slabs of 40 rows");
+        const int y0 = warp * 40;                                  // first row of this warp's slab, relative to yr0
+#pragma unroll 1
+        for (int g = 0; g < 2; ++g) {
+            const int m0 = yr0 + y0 + g * 16;
+            fir_c64<16, 2>(xs + lane, xr0, T.hb, P.shiftB, m0, a16);
 #pragma unroll
-            for (int r = 0; r < 8; ++r) ys[(g * 8 + r) * 32 + lane] = (m0 + r >= 0 && m0 + r < P.nz) ? acc[r] : 0.0f;
+            for (int r = 0; r < 16; ++r) ys[(y0 + g * 16 + r) * 32 + lane] = (m0 + r >= 0 && m0 + r < P.nz) ? a16[r] : 0.0f;
+        }
+        {
+            const int m0 = yr0 + y0 + 32;
+            fir_c64<8, 2>(xs + lane, xr0, T.hb, P.shiftB, m0, a8);
+#pragma unroll
+            for (int r = 0; r < 8; ++r) ys[(y0 + 32 + r) * 32 + lane] = (m0 + r >= 0 && m0 + r < P.nz) ? a8[r] : 0.0f;
         }
         __syncthreads();
         float vmax = 0.0f;
-        for (int g = warp; g < TZ / 8; g += 8) {
-            const int m0 = r0 + g * 8;
-            fir8_c64<HPAR>(ys + lane, yr0, T.hh, P.shiftH, m0, acc);
+#pragma unroll 1
+        for (int g = 0; g < 2; ++g) {
+            const int m0 = r0 + warp * 32 + g * 16;
+            fir_c64<16, HPAR>(ys + lane, yr0, T.hh, P.shiftH, m0, a16);
 #pragma unroll
-            for (int r = 0; r < 8; ++r) {
+            for (int r = 0; r < 16; ++r) {
                 const float y = ys[(m0 + r - yr0) * 32 + lane];
-                const float env = sqrtf(fmaf(y, y, acc[r] * acc[r]));
+                const float env = sqrtf(fmaf(y, y, a16[r] * a16[r]));
                 if (m0 + r < P.nz && col < P.nx) {
                     P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = env;
                     vmax = fmaxf(vmax, env);
