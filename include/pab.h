@@ -135,11 +135,13 @@ int pab_set_interp(pab_ctx* ctx, int interp);
 
 /* pab_set_delay_cache -- keep the interpolation tap (integer sample + fraction) of every (pixel, element) pair in
  * device memory, computed once in fp64, instead of recomputing the delay in every call (PAPER.md:190 keeps its
- * delays in GPU global memory; BASELINE.json north_star allows a cached table "where it wins").  It wins for calls
- * of 1..3 frames, where the in-kernel delay cannot be shared between frames.  4 bytes per (pixel, element):
- * 134 MB at 128 elements x 1024 x 256 pixels; when pitch_m is an exact integer multiple q of grid.dx the tap depends
- * on (column - q * element, row) only and the table shrinks to (nx + q (N-1)) * nz * 8 bytes (2 MB there).  Linear interpolation, no weighting, orders 1..5 (other settings
- * fall back to the in-kernel delay).  In-range geometries only (pab_plan_info.in_range), staged variant.
+ * delays in GPU global memory; BASELINE.json north_star allows a cached table "where it wins").  It wins most for
+ * calls of 1..3 frames, where the in-kernel delay cannot be shared between frames, and by ~7 % for 16-frame groups.
+ * 4 bytes per (pixel, element): 134 MB at 128 elements x 1024 x 256 pixels; when pitch_m is an exact integer
+ * multiple q of grid.dx the tap depends on (column - q * element, row) only, and calls of 1..3 frames use a compact
+ * table of (nx + q (N-1)) * nz * 8 bytes (2 MB there) instead.  Linear interpolation, no weighting, orders 1..5
+ * (other settings, and geometries whose table block does not fit in shared memory, fall back to the in-kernel
+ * delay).  In-range geometries only (pab_plan_info.in_range), staged variant.
  * Synchronises the device on the first call.  Errors: PAB_ERR_INVALID, PAB_ERR_ALLOC, PAB_ERR_CUDA. */
 int pab_set_delay_cache(pab_ctx* ctx, int mode);
 
@@ -160,8 +162,8 @@ int pab_set_variant(pab_ctx* ctx, int variant);
  *              pab_set_input; aligned to its element size; read only; caller keeps it alive until the
  *              stream work finishes
  *   n_frames   >= 1; frames are independent; the library batches them internally
- *   order      k = 1..5 (1 = DAS eq. 1, 2 = DMAS eq. 3, 3..5 = eqs. 7, 8, 9); k = 6..8 (row f2: the same power-sum
- *              scheme continued) with linear interpolation and no weighting only
+ *   order      k = 1..5 (1 = DAS eq. 1, 2 = DMAS eq. 3, 3..5 = eqs. 7, 8, 9); k = 6..8 (row f2: the same
+ *              O(N) evaluation of e_k, by its recurrence) with linear interpolation and no weighting only
  *   out_dev    device pointer, [n_frames][nz][nx], x fastest, fp32, 4-byte aligned; fully overwritten
  *   cuda_stream a cudaStream_t passed as void*; NULL = the legacy default stream
  * One context must not be used from two streams at once (shared scratch).
@@ -170,9 +172,10 @@ int pab_set_variant(pab_ctx* ctx, int variant);
 int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int order, float* out_dev, void* cuda_stream);
 
 /*
- * pab_beamform_host -- the same path from HOST buffers: copies rf_host to the device in frame batches
- * through pinned staging buffers (copies overlapped with compute on two internal streams), runs the
- * kernels, copies the images back to out_host, and returns after everything has finished.
+ * pab_beamform_host -- the same path from HOST buffers: copies rf_host to the device in pieces of a few frames,
+ * runs the kernels and copies the images back on three internal streams with two device buffer sets, so that the
+ * copies of successive pieces overlap the kernels; returns after everything has finished.  Pinned host memory
+ * is what makes the copies asynchronous; pageable buffers work but serialise.
  *   rf_host   host pointer, same layout and type as rf_dev above (pageable or pinned)
  *   out_host  host pointer, [n_frames][nz][nx] fp32
  */
