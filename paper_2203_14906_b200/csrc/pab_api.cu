@@ -258,7 +258,8 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
         // tile-major table staged by TMA (the compact table's global loads cost them 9 %)
         const long long q = llround((double)ctx->pitch / (double)ctx->grid.dx);
         const bool compact = q >= 1 && q <= 64 && (double)ctx->pitch == (double)q * (double)ctx->grid.dx &&
-                             (long long)ctx->grid.nx + q * (ctx->N - 1) <= 65535;
+                             (long long)ctx->grid.nx + q * (ctx->N - 1) <= 65535 &&
+                             ((long long)ctx->grid.nx + q * (ctx->N - 1)) * ctx->grid.nz < (1LL << 31);
         const bool need_taps = (mode == PAB_CACHE_ALL || !compact) && !ctx->d_taps;
         const bool need_w0s = !ctx->d_w0s, need_compact = compact && !ctx->d_compact;
         if (need_taps || need_w0s || need_compact) {

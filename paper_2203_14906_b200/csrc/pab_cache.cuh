@@ -126,8 +126,9 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                     const int len = min(C.window, row_len - w0);
                     const uint32_t bytes = (uint32_t)len * BPS;
                     const int slot = s * stage_bytes + lane * slot_bytes;
-                    if constexpr (COMPACT) {
-                        asm volatile("st.shared.u32 [%0], %1;" ::"r"(ctab0 + (s * C.chunk + lane) * 4), "r"(w0) : "memory");
+                    if constexpr (COMPACT) {          // the shared address sample 0 of this channel would have
+                        asm volatile("st.shared.u32 [%0], %1;" ::"r"(ctab0 + (s * C.chunk + lane) * 4),
+                                     "r"(data0 + slot - (uint32_t)w0 * BPS) : "memory");
                         mbar_arrive_expect_tx(full, bytes * NCOPY);
                     } else {
                         mbar_arrive_expect_tx(full, bytes * NCOPY + kCacheBlockBytes);
@@ -162,12 +163,13 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 #pragma unroll
             for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
         // COMPACT: this pixel's row of the (d, row) table; d = j - q i + q (N - 1) falls by q per element
-        const uint2* cp = compact + ((size_t)(min(j, P.nx - 1) + q * (P.N - 1)) * P.nz + min(m, P.nz - 1));
-        const size_t cstep = (size_t)q * P.nz;
+        // (32-bit entry index: pab_set_delay_cache builds the compact table only below 2^31 entries)
+        const uint32_t ci0 = (uint32_t)(min(j, P.nx - 1) + q * (P.N - 1)) * (uint32_t)P.nz + (uint32_t)min(m, P.nz - 1);
+        const uint32_t cstep = (uint32_t)q * (uint32_t)P.nz;
 
         for (int ck = 0; ck < n_chunks; ++ck) {
             const int nch = min(C.chunk, P.N - ck * C.chunk);
-            const uint2* cpk = cp - (size_t)(ck * C.chunk) * cstep;
+            const uint32_t cik = ci0 - (uint32_t)(ck * C.chunk) * cstep;
             mbar_wait(bar0 + 8 * s, ph);
             const uint32_t ctab_s = ctab0 + s * C.chunk * kBlk + (COMPACT ? 0u : my);
             const uint32_t data_s = data0 + s * stage_bytes;
@@ -177,9 +179,9 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                 float a;
                 uint32_t addr;
                 if constexpr (COMPACT) {
-                    const uint2 e = __ldg(cpk - (size_t)l * cstep);
+                    const uint2 e = __ldg(compact + (cik - (uint32_t)l * cstep));
                     a = __uint_as_float(e.y);
-                    addr = data_s + l * slot_bytes + ((int)e.x - (int)lds32u(ctab_s + l * 4)) * BPS;
+                    addr = lds32u(ctab_s + l * 4) + e.x * BPS;
                 } else {
                     const uint32_t e = lds32u(ctab_s + l * kCacheBlockBytes);
                     a = __uint_as_float(0x3F800000u | ((e << (32 - kCacheFracBits)) >> 9)) - 1.0f;          // fraction, exact
