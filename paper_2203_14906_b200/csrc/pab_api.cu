@@ -351,13 +351,19 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
     ctx->post_fast = TpB > 32 && TpB <= 64 && (mode < PAB_ENVELOPE || (TpH > 32 && TpH <= 64));
     if (ctx->post_fast) {
         memset(&ctx->taps64, 0, sizeof ctx->taps64);
-        for (int t = 0; t < TpB; ++t) ctx->taps64.hb[t] = hb[t];
+        PostTaps64& T = ctx->taps64;
+        for (int t = 0; t < TpB; ++t) T.hbr[63 - t] = hb[t];
+        for (int j = 1; j < 64; ++j) T.hbs[j] = T.hbr[j - 1];
         bool even_zero = true, odd_zero = true;
         if (mode >= PAB_ENVELOPE)
             for (int t = 0; t < TpH; ++t) {
-                ctx->taps64.hh[t] = hh[t];
+                T.hhr[63 - t] = hh[t];
                 if (hh[t] != 0.0f) { if (t & 1) odd_zero = false; else even_zero = false; }
             }
+        for (int j = 1; j < 64; ++j) T.hhs[j] = T.hhr[j - 1];
+        // type III: the non-zero original parity p sits at reversed parity 1 - p
+        const int q = odd_zero ? 1 : 0;
+        for (int i = 0; i < 32; ++i) T.hhd[2 * i] = T.hhd[2 * i + 1] = T.hhr[q + 2 * i];
         ctx->hilbert_parity = odd_zero ? 0 : (even_zero ? 1 : 2);
     }
     ctx->post_mode = mode; ctx->n_taps_bp = n_taps_bp; ctx->n_taps_h = n_taps_hilbert;

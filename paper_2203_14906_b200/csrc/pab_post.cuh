@@ -7,49 +7,92 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "pab_kernels.cuh"
+#include "pab_staged.cuh"   // mbarrier / bulk-copy helpers
 
 namespace pab {
 
-struct PostTaps64 {
-    float hb[64];   // band-pass taps, zero-padded
-    float hh[64];   // Hilbert taps g[t' ] = g(t' - L), zero-padded
+// Taps as the kernels read them (correlation form): out[m] = sum_j hr[j] in[m + shift - 63 + j], hr[j] = h[63 - j].
+struct alignas(16) PostTaps64 {
+    float hbr[64];   // band-pass taps, zero-padded to 64, reversed
+    float hbs[64];   // the same one place on: hbs[j] = hbr[j - 1] (pairs for odd output rows)
+    float hhr[64];   // Hilbert taps g[t'] = g(t' - L), zero-padded to 64, reversed (dense case)
+    float hhs[64];   // hhs[j] = hhr[j - 1]
+    float hhd[64];   // type-III case: the 32 reversed taps of the non-zero parity, each stored twice
 };
 
-// R (8 or 16) consecutive output rows m0..m0+R-1 of one column: out[m] = sum_t taps[t] in[m + shift - t], t < 64, from
-// an (R + 7)-row register window that slides 8 rows per block of 8 taps: 8 R FMAs per 8 shared loads.
-// PAR = 0 / 1: only taps of that index parity are non-zero; PAR = 2: dense.
-template <int R, int PAR>
-__device__ __forceinline__ void fir_c64(const float* in_col, int in_r0, const float (&taps)[64], int shift, int m0,
-                                        float (&acc)[R]) {
-    const float* base = in_col + (m0 + shift - in_r0) * 32;
-    float w[R + 7];
+// Blackwell packed fp32 FMA (FFMA2): two independent fp32 FMAs, each rounded as fmaf, in one issue slot.
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;"
+        : "=l"(r)
+        : "l"(reinterpret_cast<unsigned long long&>(a)), "l"(reinterpret_cast<unsigned long long&>(b)),
+          "l"(reinterpret_cast<unsigned long long&>(c)));
+    return reinterpret_cast<float2&>(r);
+}
+
+// R consecutive output rows of one column, dense taps; base = in_col + (m0 + shift - 63 - in_r0) * 32 is window row 0.
+// The two FMAs of an FFMA2 take neighbouring taps and neighbouring window rows (an aligned register pair), so even
+// output rows pair taps (0,1),(2,3).. and odd rows (1,2),(3,4).. from the shifted copy, with taps 0 and 63 on their
+// own; the two partial sums of a row are added at the end: 33.5 instructions per row for 64 taps.
+template <int R>
+__device__ __forceinline__ void fir_dense64(const float* base, const float (&hr)[64], const float (&hs)[64],
+                                            float (&out)[R]) {
+    static_assert(R % 2 == 0, "rows are produced in pairs");
+    float w[R + 63];
 #pragma unroll
-    for (int e = 0; e < R - 1; ++e) w[8 + e] = base[(1 + e) * 32];
+    for (int a = 0; a < R + 63; ++a) w[a] = base[a * 32];
 #pragma unroll
-    for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+    for (int r = 0; r < R; r += 2) {
+        float2 e = make_float2(0.0f, 0.0f);
+        float2 o = make_float2(hr[0] * w[r + 1], hr[63] * w[r + 64]);
 #pragma unroll
-    for (int tb = 0; tb < 64; tb += 8) {
-#pragma unroll
-        for (int d = 0; d < 8; ++d) w[d] = base[(d - 7 - tb) * 32];
-#pragma unroll
-        for (int tt = 0; tt < 8; ++tt) {
-            if (PAR == 2 || ((tb + tt) & 1) == PAR) {
-                const float h = taps[tb + tt];
-#pragma unroll
-                for (int r = 0; r < R; ++r) acc[r] = fmaf(h, w[r - tt + 7], acc[r]);
-            }
+        for (int j = 0; j < 64; j += 2) {
+            const float2 x = make_float2(w[r + j], w[r + j + 1]);
+            e = ffma2(make_float2(hr[j], hr[j + 1]), x, e);
+            if (j >= 2) o = ffma2(make_float2(hs[j], hs[j + 1]), x, o);
         }
-#pragma unroll
-        for (int d = R - 2; d >= 0; --d) w[d + 8] = w[d];
+        out[r] = e.x + e.y;
+        out[r + 1] = o.x + o.y;
     }
+}
+
+// The same for taps that are non-zero only at reversed index parity Q (type-III Hilbert FIR, reading A9): every tap
+// serves two neighbouring output rows in one FFMA2 (tap stored twice in hd), the window pairs all start at parity Q:
+// 16 instructions per row for the 32 taps.
+template <int R, int Q>
+__device__ __forceinline__ void fir_parity64(const float* base, const float (&hd)[64], float (&out)[R]) {
+    static_assert(R % 2 == 0, "rows are produced in pairs");
+    float w[R + 63];
+#pragma unroll
+    for (int a = Q; a < R + 62 + Q; ++a) w[a] = base[a * 32];
+    float2 acc[R / 2];
+#pragma unroll
+    for (int r = 0; r < R / 2; ++r) acc[r] = make_float2(0.0f, 0.0f);
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        const float2 h = make_float2(hd[2 * i], hd[2 * i + 1]);
+#pragma unroll
+        for (int r = 0; r < R; r += 2) acc[r / 2] = ffma2(h, make_float2(w[r + Q + 2 * i], w[r + Q + 2 * i + 1]), acc[r / 2]);
+    }
+#pragma unroll
+    for (int r = 0; r < R; r += 2) { out[r] = acc[r / 2].x; out[r + 1] = acc[r / 2].y; }
+}
+
+// HPAR = parity of the non-zero ORIGINAL Hilbert taps (0 / 1), 2 = dense
+template <int R, int HPAR>
+__device__ __forceinline__ void fir_hilbert64(const float* base, const PostTaps64& T, float (&out)[R]) {
+    if constexpr (HPAR == 2) fir_dense64<R>(base, T.hhr, T.hhs, out);
+    else fir_parity64<R, 1 - HPAR>(base, T.hhd, out);
 }
 
 constexpr int kPostFastTZ = 256;
 
 // grid: (ceil(nx/32), ceil(nz/TZ), F), 256 threads; lanes own columns.
-template <int TZ, bool ENV, int HPAR>
+// BULK (nx a multiple of 32): the tile rows (128 B each) come in as 1-D TMA bulk copies on one mbarrier, rows outside
+// the image are zero-filled by hand; otherwise plain predicated loads.
+template <int TZ, bool ENV, int HPAR, bool BULK>
 __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, const __grid_constant__ PostTaps64 T) {
-    extern __shared__ float post64_smem[];
+    extern __shared__ __align__(128) float post64_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int col0 = blockIdx.x * 32, r0 = blockIdx.y * TZ, f = blockIdx.z;
     const int col = col0 + lane;
@@ -60,6 +103,26 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
     float* xs = post64_smem;            // [XR][32]
     float* ys = xs + XR * 32;           // [YR][32]   (ENV only)
     const float* img = P.x + (size_t)f * P.nz * P.nx;
+    if constexpr (BULK) {
+        __shared__ __align__(8) unsigned long long bar;
+        const uint32_t barA = smem_u32(&bar);
+        const int lo = max(0, -xr0), hi = min(XR, P.nz - xr0);           // tile rows [lo, hi) lie inside the image
+        if (threadIdx.x == 0) {
+            mbar_init(barA, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            mbar_arrive_expect_tx(barA, (uint32_t)(hi - lo) * 128u);
+        }
+        __syncthreads();
+        const uint32_t xsA = smem_u32(xs);
+        for (int r = threadIdx.x; r < XR; r += 256) {
+            if (r >= lo && r < hi) bulk_g2s(xsA + r * 128, img + (size_t)(xr0 + r) * P.nx + col0, 128u, barA);
+            else {
+#pragma unroll
+                for (int c = 0; c < 32; c += 4) *reinterpret_cast<float4*>(xs + r * 32 + c) = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+        mbar_wait(barA, 0);
+    } else {
     // tile load: 16 rows per warp in flight at a time (the loop is latency-bound otherwise)
     constexpr int kRowsPerWarp = (XR + 7) / 8;
 #pragma unroll 1
@@ -76,6 +139,7 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
             if (r < XR) xs[r * 32 + lane] = v[k];
         }
     }
+    }
     __syncthreads();
     // every warp owns a slab of consecutive rows: 32 output rows (two 16-row groups), and with the envelope 40 rows of
     // the band-pass intermediate (16 + 16 + 8): the same work for all 8 warps
@@ -85,7 +149,7 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
 #pragma unroll 1
         for (int g = 0; g < 2; ++g) {
             const int m0 = r0 + warp * 32 + g * 16;
-            fir_c64<16, 2>(xs + lane, xr0, T.hb, P.shiftB, m0, a16);
+            fir_dense64<16>(xs + lane + (m0 + P.shiftB - 63 - xr0) * 32, T.hbr, T.hbs, a16);
 #pragma unroll
             for (int r = 0; r < 16; ++r)
                 if (m0 + r < P.nz && col < P.nx) P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = a16[r];
@@ -96,13 +160,13 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
 #pragma unroll 1
         for (int g = 0; g < 2; ++g) {
             const int m0 = yr0 + y0 + g * 16;
-            fir_c64<16, 2>(xs + lane, xr0, T.hb, P.shiftB, m0, a16);
+            fir_dense64<16>(xs + lane + (m0 + P.shiftB - 63 - xr0) * 32, T.hbr, T.hbs, a16);
 #pragma unroll
             for (int r = 0; r < 16; ++r) ys[(y0 + g * 16 + r) * 32 + lane] = (m0 + r >= 0 && m0 + r < P.nz) ? a16[r] : 0.0f;
         }
         {
             const int m0 = yr0 + y0 + 32;
-            fir_c64<8, 2>(xs + lane, xr0, T.hb, P.shiftB, m0, a8);
+            fir_dense64<8>(xs + lane + (m0 + P.shiftB - 63 - xr0) * 32, T.hbr, T.hbs, a8);
 #pragma unroll
             for (int r = 0; r < 8; ++r) ys[(y0 + 32 + r) * 32 + lane] = (m0 + r >= 0 && m0 + r < P.nz) ? a8[r] : 0.0f;
         }
@@ -111,11 +175,11 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
 #pragma unroll 1
         for (int g = 0; g < 2; ++g) {
             const int m0 = r0 + warp * 32 + g * 16;
-            fir_c64<16, HPAR>(ys + lane, yr0, T.hh, P.shiftH, m0, a16);
+            fir_hilbert64<16, HPAR>(ys + lane + (m0 + P.shiftH - 63 - yr0) * 32, T, a16);
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
                 const float y = ys[(m0 + r - yr0) * 32 + lane];
-                const float env = sqrtf(fmaf(y, y, a16[r] * a16[r]));
+                const float env = sqrt_approx(fmaf(y, y, a16[r] * a16[r]));
                 if (m0 + r < P.nz && col < P.nx) {
                     P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = env;
                     vmax = fmaxf(vmax, env);
@@ -133,21 +197,36 @@ inline size_t post64_smem_bytes(bool env) {
     return ((size_t)(YR + 63) * 32 + (env ? (size_t)YR * 32 : 0)) * 4;
 }
 
-inline cudaError_t post64_configure(int smem_optin) {
+template <bool BULK>
+inline cudaError_t post64_configure_b(int smem_optin) {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
-    return cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    smem_optin = (int)post64_smem_bytes(true);   // what the kernels use (the bulk variant adds a static mbarrier)
+    if ((e = cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, false, 2, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, true, 0, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, true, 1, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(post_fir64_kernel<kPostFastTZ, true, 2, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 
-inline void launch_post64(const PostParams& Q, const PostTaps64& T, bool env, int hpar, int F, cudaStream_t st) {
+inline cudaError_t post64_configure(int smem_optin) {
+    cudaError_t e = post64_configure_b<false>(smem_optin);
+    return e != cudaSuccess ? e : post64_configure_b<true>(smem_optin);
+}
+
+template <bool BULK>
+inline void launch_post64_b(const PostParams& Q, const PostTaps64& T, bool env, int hpar, int F, cudaStream_t st) {
     dim3 grid((Q.nx + 31) / 32, (Q.nz + kPostFastTZ - 1) / kPostFastTZ, F);
     const size_t sm = post64_smem_bytes(env);
-    if (!env) post_fir64_kernel<kPostFastTZ, false, 2><<<grid, 256, sm, st>>>(Q, T);
-    else if (hpar == 0) post_fir64_kernel<kPostFastTZ, true, 0><<<grid, 256, sm, st>>>(Q, T);
-    else if (hpar == 1) post_fir64_kernel<kPostFastTZ, true, 1><<<grid, 256, sm, st>>>(Q, T);
-    else post_fir64_kernel<kPostFastTZ, true, 2><<<grid, 256, sm, st>>>(Q, T);
+    if (!env) post_fir64_kernel<kPostFastTZ, false, 2, BULK><<<grid, 256, sm, st>>>(Q, T);
+    else if (hpar == 0) post_fir64_kernel<kPostFastTZ, true, 0, BULK><<<grid, 256, sm, st>>>(Q, T);
+    else if (hpar == 1) post_fir64_kernel<kPostFastTZ, true, 1, BULK><<<grid, 256, sm, st>>>(Q, T);
+    else post_fir64_kernel<kPostFastTZ, true, 2, BULK><<<grid, 256, sm, st>>>(Q, T);
+}
+
+// bulk row copies need 128-byte rows of whole tiles at 16-byte aligned addresses
+inline void launch_post64(const PostParams& Q, const PostTaps64& T, bool env, int hpar, int F, cudaStream_t st) {
+    const bool bulk = Q.nx % 32 == 0 && (reinterpret_cast<uintptr_t>(Q.x) & 15) == 0;
+    if (bulk) launch_post64_b<true>(Q, T, env, hpar, F, st);
+    else launch_post64_b<false>(Q, T, env, hpar, F, st);
 }
 
 }  // namespace pab
