@@ -3,6 +3,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <vector>
 #include <cuda_runtime.h>
 #include "../../include/pab.h"

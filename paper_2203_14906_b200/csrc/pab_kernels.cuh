@@ -55,6 +55,25 @@ __global__ void __launch_bounds__(256) ingest_quad_kernel(const T* __restrict__ 
         if (s4 + k < S) dst[k] = make_float4(v[0][k], v[1][k], v[2][k], v[3][k]);
 }
 
+// The same for fp32 records with S a multiple of 4 at a 16-byte aligned address: 128-bit loads, all 4 frames in flight.
+__global__ void __launch_bounds__(256) ingest_quad_vec_kernel(const float4* __restrict__ rf, float4* __restrict__ quad,
+                                                               int F, int N, int S4, float scale) {
+    const int n = blockIdx.y, q = blockIdx.z;
+    const int s4 = blockIdx.x * blockDim.x + threadIdx.x;     // in units of 4 samples
+    if (s4 >= S4) return;
+    float4 v[4];
+#pragma unroll
+    for (int fr = 0; fr < 4; ++fr) {
+        const int f = q * 4 + fr;
+        v[fr] = f < F ? __ldcs(rf + ((size_t)f * N + n) * (size_t)S4 + s4) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    float4* dst = quad + (((size_t)q * N + n) * (size_t)S4 + s4) * 4;
+    dst[0] = make_float4(scale * v[0].x, scale * v[1].x, scale * v[2].x, scale * v[3].x);
+    dst[1] = make_float4(scale * v[0].y, scale * v[1].y, scale * v[2].y, scale * v[3].y);
+    dst[2] = make_float4(scale * v[0].z, scale * v[1].z, scale * v[2].z, scale * v[3].z);
+    dst[3] = make_float4(scale * v[0].w, scale * v[1].w, scale * v[2].w, scale * v[3].w);
+}
+
 // rf[F][N][S] -> lin[F][N][Sp], Sp >= S multiple of 4, pad written as zeros.  grid: (ceil(Sp/blockDim.x), N, F)
 template <typename T>
 __global__ void __launch_bounds__(256) ingest_lin_kernel(const T* __restrict__ rf, float* __restrict__ lin,
@@ -255,6 +274,40 @@ __global__ void __launch_bounds__(256) post_log_kernel(float* __restrict__ img, 
             p[i] = v;
         }
     }
+}
+
+__device__ __forceinline__ float log_db(float e, float M, float lgM, float dr) {
+    const float k = 6.02059991327962f;   // 20 log10(2)
+    return (M > 0.0f && e > 0.0f) ? fmaxf(k * (lg2_approx(e) - lgM), -dr) : -dr;
+}
+
+// The same for npix a multiple of 4 at a 16-byte aligned address.  grid: (ceil(npix / 4096), F), 256 threads x 4 x 128 bit.
+__global__ void __launch_bounds__(256) post_log_vec_kernel(float4* __restrict__ img, const unsigned int* __restrict__ frame_max,
+                                                            int npix4, float dyn_range_db) {
+    const int f = blockIdx.y;
+    const float M = __uint_as_float(frame_max[f]);
+    const float lgM = lg2_approx(M);
+    float4* p = img + (size_t)f * npix4;
+    float4 e[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int i = (blockIdx.x * 4 + u) * 256 + threadIdx.x;
+        e[u] = i < npix4 ? p[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int i = (blockIdx.x * 4 + u) * 256 + threadIdx.x;
+        if (i < npix4)
+            __stcs(p + i, make_float4(log_db(e[u].x, M, lgM, dyn_range_db), log_db(e[u].y, M, lgM, dyn_range_db),
+                                      log_db(e[u].z, M, lgM, dyn_range_db), log_db(e[u].w, M, lgM, dyn_range_db)));
+    }
+}
+
+inline void launch_post_log(float* out, const unsigned int* frame_max, int npix, int F, float dr, cudaStream_t st) {
+    if (npix % 4 == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0)
+        post_log_vec_kernel<<<dim3((npix / 4 + 1023) / 1024, F), 256, 0, st>>>((float4*)out, frame_max, npix / 4, dr);
+    else
+        post_log_kernel<<<dim3((npix + 1023) / 1024, F), 256, 0, st>>>(out, frame_max, npix, dr);
 }
 
 }  // namespace pab

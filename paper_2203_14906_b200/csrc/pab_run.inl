@@ -22,6 +22,12 @@ template <typename T>
 void launch_ingest_quad(const void* rf, float* stage, int F, int N, int S, float scale, cudaStream_t st) {
     const int nq = (F + 3) / 4;
     dim3 grid((S + 1023) / 1024, N, nq);
+    if constexpr (std::is_same<T, float>::value) {
+        if (S % 4 == 0 && (reinterpret_cast<uintptr_t>(rf) & 15) == 0) {
+            ingest_quad_vec_kernel<<<dim3((S / 4 + 255) / 256, N, nq), 256, 0, st>>>((const float4*)rf, (float4*)stage, F, N, S / 4, scale);
+            return;
+        }
+    }
     ingest_quad_kernel<T><<<grid, 256, 0, st>>>((const T*)rf, (float4*)stage, F, N, S, scale);
 }
 template <typename T>
@@ -180,9 +186,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
                 launch_post64(Q, ctx->taps64, env, ctx->hilbert_parity, F, st);
             }
             if (ctx->post_mode == PAB_LOG) {
-                dim3 g2((nx * nz + 1023) / 1024, F);
                 Span sp(ctx, PAB_STAGE_POST_LOG, st);
-                post_log_kernel<<<g2, 256, 0, st>>>(out, ctx->d_max, nx * nz, ctx->dyn_range_db);
+                launch_post_log(out, ctx->d_max, nx * nz, F, ctx->dyn_range_db, st);
             }
         } else if (ctx->post_mode == PAB_BANDPASS) {
             const size_t sm = ((size_t)(TZ + Q.TpB - 1) * 32 + Q.TpB + Q.TpH) * 4;
@@ -197,9 +202,8 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
                 post_fir_kernel<TZ, true><<<grid, 256, sm, st>>>(Q);
             }
             if (ctx->post_mode == PAB_LOG) {
-                dim3 g2((nx * nz + 1023) / 1024, F);
                 Span sp(ctx, PAB_STAGE_POST_LOG, st);
-                post_log_kernel<<<g2, 256, 0, st>>>(out, ctx->d_max, nx * nz, ctx->dyn_range_db);
+                launch_post_log(out, ctx->d_max, nx * nz, F, ctx->dyn_range_db, st);
             }
         }
     }
