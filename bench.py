@@ -50,7 +50,7 @@ XU_PER_ITEM = 2.0
 FP32_PER_ITEM = 6.0
 DELAY_CACHE = "all"
 SM_COUNT = 148
-NCU_TRAFFIC_BYTES = 183_477_760 + 52_702_464   # per 64-frame launch; profiles/r1_beamform_ncu_c.md
+NCU_TRAFFIC_BYTES = 185_511_680 + 51_419_136   # per 64-frame launch; profiles/r1_step_ncu_f.md
 XU_LANES_PER_CLK_SM = 16
 FP32_LANES_PER_CLK_SM = 128
 
@@ -274,7 +274,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
                     "frac": achieved / xu_peak, "traffic": NCU_TRAFFIC_BYTES,
                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
-                                      "kernel at this workload: profiles/r1_beamform_ncu_c.md",
+                                      "kernel at this workload: profiles/r1_step_ncu_f.md",
                     "peak_source": f"148 SM x 16 XU lanes/clk x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, "
                                    f"{peaks['source']}); DESIGN.md Roofline",
                     "launch_ms": bf_launch_ms, "launches_timed": bf_n,
