@@ -75,7 +75,8 @@ __device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
 // NQ = 0: lin layout, one frame per thread; NQ = 4 (orders 1..3) / NQ = 2 (orders 4, 5): quad layout, 16 / 8 frames
 // per thread.  In-range geometries.
 // COMPACT: taps come from the (d, row) table through L1/L2 (q = pitch / dx), only the window starts are staged.
-template <int K, int NQ, bool COMPACT>
+// W = 1: coherence-factor weighting (row f1), frame groups with the tile-major table only (NQ = 1, 2; orders 4, 5: NQ = 1).
+template <int K, int NQ, bool COMPACT, int W = 0>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParams P, const StagedCfg C,
                                                                     const uint32_t* __restrict__ taps,
                                                                     const int* __restrict__ w0s,
@@ -157,11 +158,11 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
         const int bx = txy % C.tiles_x, by = txy / C.tiles_x;
         const int j = bx * kStgCols + col;
         const int m = by * kStgRows + (warp >> 3) * 32 + lane;
-        float p[NF][K];
+        float p[NF][kAcc<K, W>];
 #pragma unroll
         for (int f = 0; f < NF; ++f)
 #pragma unroll
-            for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+            for (int k = 0; k < kAcc<K, W>; ++k) p[f][k] = 0.0f;
         // COMPACT: this pixel's row of the (d, row) table; d = j - q i + q (N - 1) falls by q per element
         // (32-bit entry index: pab_set_delay_cache builds the compact table only below 2^31 entries)
         const uint32_t ci0 = (uint32_t)(min(j, P.nx - 1) + q * (P.N - 1)) * (uint32_t)P.nz + (uint32_t)min(m, P.nz - 1);
@@ -189,16 +190,16 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                 }
                 if constexpr (NQ == 0) {
                     const float s0 = lds32(addr), s1 = lds32(addr + 4);
-                    accumulate<K>(fmaf(a, s1 - s0, s0), p[0]);
+                    accumulate_w<K, W>(fmaf(a, s1 - s0, s0), p[0]);
                 } else {
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
                         const float4 s0 = lds128(addr + q * quad_bytes);
                         const float4 s1 = lds128(addr + q * quad_bytes + 16);
-                        accumulate<K>(fmaf(a, s1.x - s0.x, s0.x), p[4 * q + 0]);
-                        accumulate<K>(fmaf(a, s1.y - s0.y, s0.y), p[4 * q + 1]);
-                        accumulate<K>(fmaf(a, s1.z - s0.z, s0.z), p[4 * q + 2]);
-                        accumulate<K>(fmaf(a, s1.w - s0.w, s0.w), p[4 * q + 3]);
+                        accumulate_w<K, W>(fmaf(a, s1.x - s0.x, s0.x), p[4 * q + 0]);
+                        accumulate_w<K, W>(fmaf(a, s1.y - s0.y, s0.y), p[4 * q + 1]);
+                        accumulate_w<K, W>(fmaf(a, s1.z - s0.z, s0.z), p[4 * q + 2]);
+                        accumulate_w<K, W>(fmaf(a, s1.w - s0.w, s0.w), p[4 * q + 3]);
                     }
                 }
             }
@@ -212,7 +213,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
-                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[f], P.inv_n);
             }
         }
     }
@@ -237,8 +238,11 @@ inline cudaError_t cached_set_attr_k(int smem_optin) {
     if ((e = cached_set_attr<K, 0>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr<K, 1>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr<K, 2>(smem_optin)) != cudaSuccess) return e;
-    if constexpr (K <= 3) return cached_set_attr<K, 4>(smem_optin);
-    else return cudaSuccess;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<K, 1, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if constexpr (K <= 3) {
+        if ((e = cudaFuncSetAttribute(bf_cached_kernel<K, 2, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+        return cached_set_attr<K, 4>(smem_optin);
+    } else return cudaSuccess;
 }
 inline cudaError_t cached_configure(int smem_optin) {
     cudaError_t e;
@@ -254,16 +258,16 @@ struct CacheTables {
     const uint2* compact;      // (d, row) table of translation-invariant geometries, or nullptr
     int q;                     // pitch / dx
 };
-template <int K, int NQ, bool COMPACT>
+template <int K, int NQ, bool COMPACT, int W = 0>
 inline void launch_cached_kc(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
     const size_t smem = cached_smem_bytes(c, NQ, COMPACT);
     int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_cached_kernel<K, NQ, COMPACT>, kStgThreads, smem) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_cached_kernel<K, NQ, COMPACT, W>, kStgThreads, smem) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
         per_sm = 1;
     }
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
-    bf_cached_kernel<K, NQ, COMPACT><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
+    bf_cached_kernel<K, NQ, COMPACT, W><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
         P, c, T.taps, T.w0s, T.compact, T.q);
 }
 template <int K, int NQ>
@@ -279,14 +283,23 @@ inline bool cached_fits(const pab_plan_info& plan, int nq, bool compact, int sme
 }
 
 template <int K>
-inline void launch_cached_nq(int nq, const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+inline void launch_cached_nq(int nq, int weight, const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    if (weight != 0) {          // cached_weight_ok(order, nq, compact) held
+        if (nq == 1) launch_cached_kc<K, 1, false, 1>(P, c, T, sm_count, st);
+        else if constexpr (K <= 3) launch_cached_kc<K, 2, false, 1>(P, c, T, sm_count, st);
+        return;
+    }
     if (nq == 0) launch_cached_k<K, 0>(P, c, T, sm_count, st);
     else if (nq == 1) launch_cached_k<K, 1>(P, c, T, sm_count, st);
     else if (nq == 2) launch_cached_k<K, 2>(P, c, T, sm_count, st);
     else if constexpr (K <= 3) launch_cached_k<K, 4>(P, c, T, sm_count, st);
 }
-// nq = 0, 1, 2 (orders 1..5) or 4 (orders 1..3)
-inline void launch_cached(int order, int nq, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
+// which (order, frame group, table) combinations have a coherence-factor instantiation
+inline bool cached_weight_ok(int order, int nq, bool compact) {
+    return !compact && (nq == 1 || (nq == 2 && order <= 3));
+}
+// nq = 0, 1, 2 (orders 1..5) or 4 (orders 1..3); weight != 0 only where cached_weight_ok
+inline void launch_cached(int order, int nq, int weight, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
                           int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (T.compact ? 4 : kCacheBlockBytes);
     long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
@@ -297,11 +310,11 @@ inline void launch_cached(int order, int nq, const BfParams& P, int groups, cons
     StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
                 (P.nz + kStgRows - 1) / kStgRows, groups};
     switch (order) {
-    case 1: launch_cached_nq<1>(nq, P, c, T, sm_count, st); break;
-    case 2: launch_cached_nq<2>(nq, P, c, T, sm_count, st); break;
-    case 3: launch_cached_nq<3>(nq, P, c, T, sm_count, st); break;
-    case 4: launch_cached_nq<4>(nq, P, c, T, sm_count, st); break;
-    default: launch_cached_nq<5>(nq, P, c, T, sm_count, st); break;
+    case 1: launch_cached_nq<1>(nq, weight, P, c, T, sm_count, st); break;
+    case 2: launch_cached_nq<2>(nq, weight, P, c, T, sm_count, st); break;
+    case 3: launch_cached_nq<3>(nq, weight, P, c, T, sm_count, st); break;
+    case 4: launch_cached_nq<4>(nq, weight, P, c, T, sm_count, st); break;
+    default: launch_cached_nq<5>(nq, weight, P, c, T, sm_count, st); break;
     }
 }
 

@@ -133,7 +133,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         P.n_frames = F;
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (cached) launch_cached(order, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
+            if (cached) launch_cached(order, 0, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                                       CacheTables{ctx->d_taps, ctx->d_w0s, ctx->d_compact, ctx->cache_q}, st);
             else if (use_staged) launch_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, 0, weight, P, F, st);
@@ -159,9 +159,9 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && weight == 0 && order <= 5 &&
-                cached_fits(ctx->plan, g, false, ctx->smem_optin))
-                launch_cached(order, g, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
+            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && order <= 5 &&
+                (weight == 0 || cached_weight_ok(order, g, false)) && cached_fits(ctx->plan, g, false, ctx->smem_optin))
+                launch_cached(order, g, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                               CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);
             else if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else launch_direct_nq(order, g, weight, R, groups, st);

@@ -500,6 +500,21 @@ def test_delay_cache_single_frames_c2(pab, orc, order):
             assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
 
 
+@pytest.mark.parametrize("order", [1, 2, 3, 4, 5])
+def test_delay_cache_cf_weighting_ragged(pab, orc, order):
+    # row f1 on the cached-tap kernel: 8-frame (orders 1..3) and 4-frame groups, ragged grid, every order
+    rng = np.random.default_rng(43)
+    g = synth.random_geometry(rng, 24, 514, 37, 129, in_range=True)
+    g = synth.Geometry(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, g.nx, g.nz, g.x0, g.dx, max(g.z0, 2e-4), g.dz).f32()
+    rf = rng.standard_normal((13, 24, 514)).astype(np.float32)
+    gpu, _ = run_gpu(pab, g, rf, order, delay_cache="all", weight="cf")
+    ref = orc.beamform_ex(rf, g, order, weight="cf")
+    off, _ = run_gpu(pab, g, rf, order, weight="cf")
+    for f in range(13):
+        check_raw(gpu[f], ref[f], order)
+        check_raw(off[f], ref[f], order)
+
+
 def test_delay_cache_ragged_int16_and_batches(pab, orc):
     rng = np.random.default_rng(41)
     g = synth.random_geometry(rng, 24, 514, 37, 129, in_range=True)
@@ -520,6 +535,9 @@ def test_delay_cache_c2b_groups_and_fallbacks(pab, orc):
         assert check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, 3)[0], 3) <= 2.5e-5
     gpu, _ = run_gpu(pab, w.geom, w.rf[:1], 3, delay_cache="single", weight="cf")     # weighting: in-kernel delay
     check_raw(gpu[0], orc.beamform_ex(w.rf[:1], w.geom, 3, weight="cf")[0], 3)
+    gpu, _ = run_gpu(pab, w.geom, w.rf[:13], 3, delay_cache="all", weight="cf")       # CF: 8 cached + 4 cached + 1 not
+    for f in (0, 7, 11, 12):
+        check_raw(gpu[f], orc.beamform_ex(w.rf[f:f + 1], w.geom, 3, weight="cf")[0], 3)
     c1 = synth.make_config("C1")                                                      # z starts at 0: not in range
     bf = pab.Beamformer(c1.geom)
     try:
