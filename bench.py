@@ -340,7 +340,8 @@ def run_sweep(args):
              ("C5", 1024, (3,), True, "none"), ("C2b", 64, (6, 8), False, "none"), ("C2b", 64, (1, 2, 3), False, "nearest"), ("C4", 16, (4, 5), False, "nearest")]
     cases += [("C2", 1, (1, 2, 3), False, "cache-single"), ("C4", 1, (4, 5), False, "cache-single"),
               ("C2b", 64, (1, 2, 3), False, "cache-all"), ("C4", 16, (4, 5), False, "cache-all"),
-              ("C2b", 64, (3,), False, "cf-cache-all"), ("C4", 16, (5,), False, "cf-cache-all")]
+              ("C2b", 64, (3,), False, "cf-cache-all"), ("C4", 16, (5,), False, "cf-cache-all"),
+              ("C2b", 64, (6, 8), False, "cache-all")]
     for cfg, F, orders, post, weight in cases:
         interp = "nearest" if weight == "nearest" else "linear"
         cache = weight.split("cache-")[1] if "cache-" in weight else "off"

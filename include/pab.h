@@ -139,9 +139,10 @@ int pab_set_interp(pab_ctx* ctx, int interp);
  * calls of 1..3 frames, where the in-kernel delay cannot be shared between frames, and by ~7 % for 16-frame groups.
  * 4 bytes per (pixel, element): 134 MB at 128 elements x 1024 x 256 pixels; when pitch_m is an exact integer
  * multiple q of grid.dx the tap depends on (column - q * element, row) only, and calls of 1..3 frames use a compact
- * table of (nx + q (N-1)) * nz * 8 bytes (2 MB there) instead.  Linear interpolation, orders 1..5; coherence-factor
- * weighting reads the table in its 8-frame (orders 1..3) and 4-frame groups under PAB_CACHE_ALL only (other
- * settings, and geometries whose table block does not fit in shared memory, fall back to the in-kernel delay).  In-range geometries only (pab_plan_info.in_range), staged variant.
+ * table of (nx + q (N-1)) * nz * 8 bytes (2 MB there) instead.  Linear interpolation; coherence-factor weighting
+ * (8- and 4-frame groups) and orders 6..8 (4-frame groups) read the table under PAB_CACHE_ALL only (other
+ * settings, and geometries whose table block does not fit in shared memory, fall back to the in-kernel delay).
+ * In-range geometries only (pab_plan_info.in_range), staged variant.
  * Synchronises the device on the first call.  Errors: PAB_ERR_INVALID, PAB_ERR_ALLOC, PAB_ERR_CUDA. */
 int pab_set_delay_cache(pab_ctx* ctx, int mode);
 

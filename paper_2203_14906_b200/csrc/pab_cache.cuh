@@ -250,7 +250,11 @@ inline cudaError_t cached_configure(int smem_optin) {
     if ((e = cached_set_attr_k<2>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr_k<3>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr_k<4>(smem_optin)) != cudaSuccess) return e;
-    return cached_set_attr_k<5>(smem_optin);
+    if ((e = cached_set_attr_k<5>(smem_optin)) != cudaSuccess) return e;
+    // orders 6..8 (row f2): 4-frame groups with the tile-major table only
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<6, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<7, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(bf_cached_kernel<8, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 struct CacheTables {
     const uint32_t* taps;      // tile-major 12+20-bit taps, or nullptr when the compact table is in use
@@ -298,7 +302,7 @@ inline void launch_cached_nq(int nq, int weight, const BfParams& P, const Staged
 inline bool cached_weight_ok(int order, int nq, bool compact) {
     return !compact && (nq == 1 || (nq == 2 && order <= 3));
 }
-// nq = 0, 1, 2 (orders 1..5) or 4 (orders 1..3); weight != 0 only where cached_weight_ok
+// nq = 0, 1, 2 (orders 1..5), 4 (orders 1..3) or 1 (orders 6..8, tile-major table); weight != 0 only where cached_weight_ok
 inline void launch_cached(int order, int nq, int weight, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
                           int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (T.compact ? 4 : kCacheBlockBytes);
@@ -314,7 +318,10 @@ inline void launch_cached(int order, int nq, int weight, const BfParams& P, int 
     case 2: launch_cached_nq<2>(nq, weight, P, c, T, sm_count, st); break;
     case 3: launch_cached_nq<3>(nq, weight, P, c, T, sm_count, st); break;
     case 4: launch_cached_nq<4>(nq, weight, P, c, T, sm_count, st); break;
-    default: launch_cached_nq<5>(nq, weight, P, c, T, sm_count, st); break;
+    case 5: launch_cached_nq<5>(nq, weight, P, c, T, sm_count, st); break;
+    case 6: launch_cached_kc<6, 1, false>(P, c, T, sm_count, st); break;          // orders 6..8: nq == 1, no weighting
+    case 7: launch_cached_kc<7, 1, false>(P, c, T, sm_count, st); break;
+    default: launch_cached_kc<8, 1, false>(P, c, T, sm_count, st); break;
     }
 }
 

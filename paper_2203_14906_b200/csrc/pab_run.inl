@@ -159,7 +159,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && order <= 5 &&
+            if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && (order <= 5 || g == 1) &&
                 (weight == 0 || cached_weight_ok(order, g, false)) && cached_fits(ctx->plan, g, false, ctx->smem_optin))
                 launch_cached(order, g, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                               CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);

@@ -389,6 +389,15 @@ def test_high_orders_c2_full_size(pab, orc, order):
         check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, order)[0], order)
 
 
+@pytest.mark.parametrize("order", [6, 7, 8])
+def test_high_orders_cached_taps(pab, orc, order):
+    """Row f2 on the cached-tap kernel (4-frame groups under PAB_CACHE_ALL): C2b frames, 4 cached + 1 not."""
+    w = synth.make_config("C2b", n_frames=5)
+    gpu, _ = run_gpu(pab, w.geom, w.rf, order, delay_cache="all")
+    for f in (0, 3, 4):
+        check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, order)[0], order)
+
+
 def test_high_orders_reject_weight_and_nearest(pab):
     w = synth.make_config("C1")
     rf = torch.from_numpy(w.rf).cuda()
