@@ -167,7 +167,8 @@ int pab_set_variant(pab_ctx* ctx, int variant);
  *              O(N) evaluation of e_k, by its recurrence) with linear interpolation and no weighting only
  *   out_dev    device pointer, [n_frames][nz][nx], x fastest, fp32, 4-byte aligned; fully overwritten
  *   cuda_stream a cudaStream_t passed as void*; NULL = the legacy default stream
- * One context must not be used from two streams at once (shared scratch).
+ * One context must not be used from two streams at once (shared scratch).  The CUDA device that was current at
+ * pab_create must be current at the call (PAB_ERR_INVALID otherwise).
  * Errors: PAB_ERR_INVALID (nothing launched), PAB_ERR_CUDA.
  */
 int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int order, float* out_dev, void* cuda_stream);

@@ -62,9 +62,10 @@ def load(build_if_missing: bool = False):
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_missing and not os.path.exists(LIB_PATH):
+    if build_if_missing:
         from . import build as _b
-        _b.build_lib()
+        if _b.is_stale():                       # absent, or older than a source file
+            _b.build_lib()
     if not os.path.exists(LIB_PATH):
         raise PabError(f"{LIB_PATH} is missing: build it with `python -m paper_2203_14906_b200.build` "
                        "(there is no CPU fallback)")
@@ -247,15 +248,21 @@ class Beamformer:
         g = self.geom
         is_torch = isinstance(rf, torch.Tensor)
         F = rf.shape[0]
+        assert tuple(rf.shape) == (F, g.n_elem, g.n_samp), rf.shape
         if is_torch:
             assert not rf.is_cuda and rf.is_contiguous()
+            assert rf.dtype == (torch.int16 if self.dtype == "int16" else torch.float32), rf.dtype
             if out is None:
                 out = torch.empty((F, g.nz, g.nx), dtype=torch.float32, pin_memory=rf.is_pinned())
+            assert not out.is_cuda and out.is_contiguous() and out.dtype == torch.float32
+            assert tuple(out.shape) == (F, g.nz, g.nx), out.shape
             src, dst = rf.data_ptr(), out.data_ptr()
         else:
             rf = np.ascontiguousarray(rf)
+            assert rf.dtype == (np.int16 if self.dtype == "int16" else np.float32), rf.dtype
             if out is None:
                 out = np.empty((F, g.nz, g.nx), dtype=np.float32)
+            assert out.dtype == np.float32 and out.flags["C_CONTIGUOUS"] and out.shape == (F, g.nz, g.nx), out.shape
             src, dst = rf.ctypes.data, out.ctypes.data
         self._check(self._L.pab_beamform_host(self._h, src, F, order, dst), "pab_beamform_host")
         return out

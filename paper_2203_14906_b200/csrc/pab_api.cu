@@ -1,6 +1,7 @@
 // pab_api.cu -- the C ABI of libpab.so (include/pab.h): context, host logic, kernel launches.
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <type_traits>
@@ -8,12 +9,8 @@
 #include <cuda_runtime.h>
 #include "../../include/pab.h"
 #include "pab_plan.h"
-#include "pab_kernels.cuh"
-#include "pab_staged.cuh"
-#include "pab_post.cuh"
-#include "pab_nearest.cuh"
-#include "pab_metrics.cuh"
-#include "pab_cache.cuh"
+#include "pab_types.h"
+#include "pab_launch.h"
 
 using namespace pab;
 
@@ -175,12 +172,8 @@ int pab_create(pab_ctx** out, int n_elem, int n_samp, float fs_hz, float c_m_s, 
     else if ((e = cudaMemcpy(ctx->d_xj, t.xj.data(), t.xj.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) fail(e, "copy xj");
     else if ((e = cudaMemcpy(ctx->d_xe, t.xe.data(), t.xe.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) fail(e, "copy xe");
     else if ((e = cudaMemcpy(ctx->d_zrow, t.zrow.data(), t.zrow.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) fail(e, "copy zrow");
-    if (rc == PAB_OK) rc = staged_configure(ctx->smem_optin);
-    if (rc == PAB_OK &&
-        (cudaFuncSetAttribute(post_fir_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin) != cudaSuccess ||
-         cudaFuncSetAttribute(post_fir_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin) != cudaSuccess))
-        rc = PAB_ERR_CUDA;
-    if (rc == PAB_OK && post64_configure(ctx->smem_optin) != cudaSuccess) rc = PAB_ERR_CUDA;
+    if (rc == PAB_OK) rc = xl_staged_configure(ctx->smem_optin);
+    if (rc == PAB_OK && xl_post_configure(ctx->smem_optin) != cudaSuccess) rc = PAB_ERR_CUDA;
     if (rc != PAB_OK) { free_all(ctx); delete ctx; return rc; }
     *out = ctx;
     return PAB_OK;
@@ -264,7 +257,7 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
         const bool need_taps = (mode == PAB_CACHE_ALL || !compact) && !ctx->d_taps;
         const bool need_w0s = !ctx->d_w0s, need_compact = compact && !ctx->d_compact;
         if (need_taps || need_w0s || need_compact) {
-            PAB_CUDA(ctx, cached_configure(ctx->smem_optin));
+            PAB_CUDA(ctx, xl_cached_configure(ctx->smem_optin));
             cudaError_t e = cudaSuccess;
             if (need_w0s) e = cudaMalloc(&ctx->d_w0s, blocks * sizeof(int));
             if (e == cudaSuccess && need_taps) e = cudaMalloc(&ctx->d_taps, blocks * kCacheBlockBytes);
@@ -274,11 +267,11 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
                 CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
                             (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x};
                 if (need_taps || need_w0s) {
-                    delay_cache_kernel<<<dim3(tiles_x, tiles_z, ctx->N), kStgRows * kStgCols>>>(G, ctx->d_taps, ctx->d_w0s);
+                    xl_build_delay_cache(G, tiles_z, ctx->d_taps, ctx->d_w0s);
                     ctx->launches++;
                 }
                 if (need_compact) {
-                    delay_compact_kernel<<<dim3((ctx->grid.nz + 255) / 256, nd), 256>>>(G, (int)q, ctx->d_compact);
+                    xl_build_delay_compact(G, (int)q, nd, ctx->d_compact);
                     ctx->launches++;
                     ctx->cache_q = (int)q;
                 }
@@ -299,16 +292,14 @@ int pab_set_interp(pab_ctx* ctx, int interp) {
     if (!ctx || (interp != PAB_INTERP_LINEAR && interp != PAB_INTERP_NEAREST)) return PAB_ERR_INVALID;
     if (interp == PAB_INTERP_NEAREST) {
         if (ctx->weight != PAB_WEIGHT_NONE || ctx->S > 65534) return PAB_ERR_INVALID;
-        PAB_CUDA(ctx, nearest_configure(ctx->smem_optin));
+        PAB_CUDA(ctx, xl_nearest_configure(ctx->smem_optin));
         if (!ctx->d_near) {
             const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z = (ctx->grid.nz + kStgRows - 1) / kStgRows;
             const size_t n = (size_t)ctx->N * tiles_x * kStgCols * (size_t)tiles_z * kStgRows;
             PAB_CUDA(ctx, cudaMalloc(&ctx->d_near, n * sizeof(unsigned short)));
             NearestGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
                           (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz};
-            dim3 grid((tiles_z * kStgRows + 255) / 256, tiles_x * kStgCols, ctx->N);
-            if (grid.y > 65535u || grid.z > 65535u) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return PAB_ERR_INVALID; }
-            nearest_table_kernel<<<grid, 256>>>(G, ctx->d_near);
+            if (!xl_nearest_table(G, ctx->d_near)) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return PAB_ERR_INVALID; }
             ctx->launches++;
             cudaError_t e = cudaDeviceSynchronize();
             if (e != cudaSuccess) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return cuda_fail(ctx, e, "nearest table"); }
@@ -341,13 +332,20 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
     design_bandpass(n_taps_bp, f_lo, f_hi, hb.data());
     if (mode >= PAB_ENVELOPE) design_hilbert((n_taps_hilbert - 1) / 2, hh.data());
     PAB_CUDA(ctx, cudaDeviceSynchronize());
-    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); ctx->d_taps_bp = ctx->d_taps_h = nullptr;
-    PAB_CUDA(ctx, cudaMalloc(&ctx->d_taps_bp, TpB * 4));
-    PAB_CUDA(ctx, cudaMalloc(&ctx->d_taps_h, TpH * 4));
-    PAB_CUDA(ctx, cudaMemcpy(ctx->d_taps_bp, hb.data(), TpB * 4, cudaMemcpyHostToDevice));
-    PAB_CUDA(ctx, cudaMemcpy(ctx->d_taps_h, hh.data(), TpH * 4, cudaMemcpyHostToDevice));
-    if (!ctx->d_img)
-        PAB_CUDA(ctx, cudaMalloc(&ctx->d_img, (size_t)ctx->plan.batch_frames * ctx->grid.nz * (size_t)ctx->grid.nx * 4));
+    // the new tap buffers are allocated and filled first and swapped in only on success: a failure leaves the
+    // context with its previous post chain intact
+    float *nb = nullptr, *nh = nullptr;
+    cudaError_t e = cudaMalloc(&nb, TpB * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&nh, TpH * 4);
+    if (e == cudaSuccess) e = cudaMemcpy(nb, hb.data(), TpB * 4, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(nh, hh.data(), TpH * 4, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(nb); cudaFree(nh); return cuda_fail(ctx, e, "post taps"); }
+    if (!ctx->d_img) {
+        e = cudaMalloc(&ctx->d_img, (size_t)ctx->plan.batch_frames * ctx->grid.nz * (size_t)ctx->grid.nx * 4);
+        if (e != cudaSuccess) { ctx->d_img = nullptr; cudaFree(nb); cudaFree(nh); return cuda_fail(ctx, e, "post scratch"); }
+    }
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h);
+    ctx->d_taps_bp = nb; ctx->d_taps_h = nh;
     // fast path: both filters fit 64 taps and are long enough for it to pay
     ctx->post_fast = TpB > 32 && TpB <= 64 && (mode < PAB_ENVELOPE || (TpH > 32 && TpH <= 64));
     if (ctx->post_fast) {
@@ -387,11 +385,7 @@ int pab_image_metrics(pab_ctx* ctx, const float* img_dev, const pab_roi* target,
     unsigned int* hist = (unsigned int*)(base + hist_off);
     PAB_CUDA(ctx, cudaMemsetAsync(base, 0, total, st));
     RoiPair R{{target->r0, target->r1, target->c0, target->c1}, {background->r0, background->r1, background->c0, background->c1}};
-    dim3 grid(32, 2);
-    metrics_sum_kernel<<<grid, 256, 0, st>>>(img_dev, nx, R, acc);
-    metrics_hist_kernel<<<grid, 256, 0, st>>>(img_dev, nx, R, acc, hist, n_bins);
-    ctx->launches += 2;
-    if (fwhm_row >= 0) { metrics_fwhm_kernel<<<1, 32, 0, st>>>(img_dev, nx, fwhm_row, target->c0, target->c1, fw); ctx->launches++; }
+    ctx->launches += xl_metrics(img_dev, nx, R, acc, hist, n_bins, fwhm_row, fw, st);
     MetricAcc h{};
     double fwh = 0.0;
     std::vector<unsigned int> hh(2 * (size_t)n_bins);

@@ -14,19 +14,10 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
-#include "pab_kernels.cuh"
-#include "pab_staged.cuh"
+#include "pab_math.cuh"
+#include "pab_pipe.cuh"
 
 namespace pab {
-
-constexpr int kCacheBlockBytes = kStgRows * kStgCols * 4;
-constexpr int kCacheFracBits = 20;
-constexpr int kCacheMaxWindow = 4000;        // the integer part must fit 12 bits
-
-struct CacheGeom {
-    double fs, c, pitch, x0, dx, z0, dz;
-    int N, S, nx, nz, tiles_x;
-};
 
 // grid: (tiles_x, tiles_z, N), 512 threads = one tile.  taps[((tile * N + i) * 8 + col) * 64 + row], w0s[tile * N + i]
 __global__ void __launch_bounds__(kStgRows * kStgCols) delay_cache_kernel(const CacheGeom G, uint32_t* __restrict__ taps,
@@ -256,20 +247,10 @@ inline cudaError_t cached_configure(int smem_optin) {
     if ((e = cudaFuncSetAttribute(bf_cached_kernel<7, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(bf_cached_kernel<8, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
-struct CacheTables {
-    const uint32_t* taps;      // tile-major 12+20-bit taps, or nullptr when the compact table is in use
-    const int* w0s;            // window start of every (tile, element)
-    const uint2* compact;      // (d, row) table of translation-invariant geometries, or nullptr
-    int q;                     // pitch / dx
-};
 template <int K, int NQ, bool COMPACT, int W = 0>
 inline void launch_cached_kc(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
     const size_t smem = cached_smem_bytes(c, NQ, COMPACT);
-    int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_cached_kernel<K, NQ, COMPACT, W>, kStgThreads, smem) != cudaSuccess || per_sm < 1) {
-        cudaGetLastError();
-        per_sm = 1;
-    }
+    const int per_sm = resident_per_sm(bf_cached_kernel<K, NQ, COMPACT, W>, kStgThreads, smem);
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
     bf_cached_kernel<K, NQ, COMPACT, W><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
         P, c, T.taps, T.w0s, T.compact, T.q);

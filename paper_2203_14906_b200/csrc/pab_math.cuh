@@ -131,7 +131,7 @@ __device__ __forceinline__ float combine_w(const float (&p)[kAcc<K, W>], float i
 // therefore carried to ~1e-6 samples, not to an fp32 ulp of the 11-12 bit index (DESIGN.md "Delay index
 // precision").  One MUFU (rsqrt) gives d0 ~ sqrt(xs^2 + zs^2); delta0 = d0 - zs; one Newton step on
 // f(delta) = delta (delta + 2 zs) - xs^2 (f' ~ 2 d0, step -f r / 2) with f evaluated in compensated arithmetic:
-// exact xs^2 = xs2 + xs2_lo (FMA), exact delta0 + 2 zs = t_hi + t_lo (Fast2Sum), and the first-order terms of
+// exact xs^2 = xs2 + xs2_lo (FMA), exact delta0 + 2 zs = t_hi + t_lo (branch-free TwoSum), and the first-order terms of
 // the low parts of xs and zs.  The correction is NOT folded back into delta0: delta0 is split exactly into an
 // integer n0 and a fraction, and the fractions (of zs, of delta0, the correction) are summed at full relative
 // precision; floor(zs) and n0 only ever meet as integers.
@@ -150,8 +150,9 @@ __device__ __forceinline__ Tap delay_tap(float xs2, float c0, const float4 row, 
     float delta0 = d0 - row.x;
     if constexpr (!INR) delta0 = fminf(fmaxf(delta0, 0.0f), 2097152.0f);
     const float z2 = row.x + row.x;
-    const float t_hi = z2 + delta0;                             // delta0 + 2 zs_hi = t_hi + t_lo exactly
-    const float t_lo = delta0 - (t_hi - z2);
+    const float t_hi = z2 + delta0;                             // delta0 + 2 zs_hi = t_hi + t_lo exactly: TwoSum, valid
+    const float bb = t_hi - z2;                                 // for either order of magnitudes (delta0 > 2 zs for
+    const float t_lo = (z2 - (t_hi - bb)) + (delta0 - bb);      // shallow rows seen by far elements)
     float g = fmaf(delta0, t_lo, c0);                           // low-order part of f: delta0 t_lo - (xs^2 - xs2)
     g = fmaf(delta0, row.y, g);                                 //                      + delta0 * 2 zs_lo
     const float f = fmaf(delta0, t_hi, -xs2) + g;

@@ -4,17 +4,9 @@
 // is decided in float32 arithmetic with individually rounded operations.
 #pragma once
 #include <cuda_runtime.h>
+#include "pab_types.h"
 
 namespace pab {
-
-struct RoiPair { int t[4]; int b[4]; };      // target, background: rows [r0, r1), columns [c0, c1)
-
-// acc[0..5]: sum_in, sum_out, sumsq_dev_out (second pass), max bits (as unsigned), unused...
-struct MetricAcc {
-    double sum_in, sum_out, var_out;
-    unsigned int max_bits;          // float bits of the largest amplitude of both regions (amplitudes >= 0)
-    unsigned int pad;
-};
 
 __device__ __forceinline__ double block_sum(double v, double* sh) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -13,19 +13,10 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
-#include "pab_kernels.cuh"
-#include "pab_staged.cuh"
+#include "pab_math.cuh"
+#include "pab_pipe.cuh"
 
 namespace pab {
-
-constexpr unsigned short kNearestInvalid = 0xFFFFu;
-constexpr int kNearBlockBytes = kStgRows * kStgCols * 2;      // one element's delay-table block for one tile
-
-// geometry as the ABI carries it (floats), promoted to double unchanged -- the oracle does the same promotion
-struct NearestGeom {
-    double fs, c, pitch, x0, dx, z0, dz;
-    int N, S, nx, nz;
-};
 
 // table[nearest_index(...)] = floor(idx + 1/2) or 0xFFFF.
 // grid: (ceil(nz_pad/256), nx_pad, N) with nz_pad, nx_pad the grid rounded up to whole tiles.

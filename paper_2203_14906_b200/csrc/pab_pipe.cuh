@@ -1,0 +1,92 @@
+// pab_pipe.cuh -- shared-memory pipeline primitives of the staged kernels: mbarrier full/empty ring, 1-D bulk
+// async copies (TMA engine: cp.async.bulk, SASS UBLKCP) and explicit shared-space loads.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "pab_types.h"
+
+namespace pab {
+
+// per staged channel: what a consumer needs besides the samples (80 bytes; every read is a warp broadcast)
+struct __align__(16) ChanEntry {
+    float2 xs[8];           // per pixel column c of the tile: (xs2, c0) of delay_tap, xs = column - element in samples
+    int base;               // shared-space address such that sample i of the first quad lives at base + i * BPS
+    int w0;                 // first staged sample
+    int w1m2;               // last valid i0 (staged end - 2)
+    int pad;
+};
+static_assert(sizeof(ChanEntry) == kChanEntryBytes, "ChanEntry size is part of the shared-memory plan");
+constexpr int kCE = (int)sizeof(ChanEntry);
+
+__device__ __forceinline__ float2 lds64(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
+// Shared-memory bytes of one launch: the plan's chunk is sized for `frames_per_thread / 4` quads per channel;
+// with fewer bytes per sample the same chunk fits with room to spare.
+inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
+    const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
+    const size_t tab = ((size_t)c.stages * c.chunk * sizeof(ChanEntry) + 127) & ~(size_t)127;
+    return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy;
+}
+
+// Resident CTAs per SM of a kernel instantiation at a given dynamic shared-memory size, asked of the runtime once per
+// (instantiation, device, size) and remembered: the query costs microseconds, which is the whole budget of a
+// launch-bound call (config C1).
+template <typename Kernel>
+inline int resident_per_sm(Kernel kernel, int threads, size_t smem) {
+    struct Memo { const void* fn = nullptr; int dev = -1; size_t smem = 0; int per_sm = 1; };
+    static thread_local Memo memos[64];          // kernels of one signature share this function: keyed by address
+    const void* fn = reinterpret_cast<const void*>(kernel);
+    Memo& memo = memos[(reinterpret_cast<uintptr_t>(fn) >> 4) % 64];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (memo.fn == fn && memo.dev == dev && memo.smem == smem) return memo.per_sm;
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    memo.fn = fn; memo.dev = dev; memo.smem = smem; memo.per_sm = per_sm;
+    return per_sm;
+}
+
+}  // namespace pab

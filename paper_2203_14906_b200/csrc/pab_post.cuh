@@ -6,19 +6,161 @@
 //   env = sqrt(y^2 + q^2), per-frame max by atomicMax on the bit pattern.
 #pragma once
 #include <cuda_runtime.h>
-#include "pab_kernels.cuh"
-#include "pab_staged.cuh"   // mbarrier / bulk-copy helpers
+#include "pab_math.cuh"
+#include "pab_pipe.cuh"   // mbarrier / bulk-copy helpers
 
 namespace pab {
 
-// Taps as the kernels read them (correlation form): out[m] = sum_j hr[j] in[m + shift - 63 + j], hr[j] = h[63 - j].
-struct alignas(16) PostTaps64 {
-    float hbr[64];   // band-pass taps, zero-padded to 64, reversed
-    float hbs[64];   // the same one place on: hbs[j] = hbr[j - 1] (pairs for odd output rows)
-    float hhr[64];   // Hilbert taps g[t'] = g(t' - L), zero-padded to 64, reversed (dense case)
-    float hhs[64];   // hhs[j] = hhr[j - 1]
-    float hhd[64];   // type-III case: the 32 reversed taps of the non-zero parity, each stored twice
-};
+// ------------------------------------------------------------------------------------------------------
+// a7 + a8: axial FIR band-pass and Hilbert-FIR envelope, fused per tile of TZ rows x 32 columns.
+//
+//   y[m] = sum_{t<T} h[t] x[m + T/2 - t]        x = 0 outside [0, nz)      (A11, A12)
+//   q[m] = sum_{t'<2L+1} g[t'] y[m + L - t']    y = 0 outside [0, nz)      (A9)
+//   env  = sqrt(y^2 + q^2); per-frame max of env by atomicMax on the bit pattern (env >= 0)
+//
+// Both filters are "out[m] = sum_t taps[t] in[m + shift - t]" with the tap count padded to a multiple of 8
+// by zeros; fir8 computes 8 consecutive rows of one column with a 15-row register window, 64 FMAs per
+// 8 + 8 shared-memory loads.  Lanes own columns (coalesced image rows).
+// ------------------------------------------------------------------------------------------------------
+// in_col: shared-memory column of this lane, row r of the image stored at in_col[(r - in_r0) * 32]
+__device__ __forceinline__ void fir8(const float* in_col, int in_r0, const float* taps, int Tp, int shift, int m0,
+                                     float (&acc)[8]) {
+    const int c = m0 + shift;
+    const float* base = in_col + (c - in_r0) * 32;
+    float w[15];
+#pragma unroll
+    for (int e = 0; e < 7; ++e) w[8 + e] = base[(1 + e) * 32];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) acc[r] = 0.0f;
+    for (int tb = 0; tb < Tp; tb += 8) {
+#pragma unroll
+        for (int d = 0; d < 8; ++d) w[d] = base[(d - 7 - tb) * 32];
+#pragma unroll
+        for (int tt = 0; tt < 8; ++tt) {
+            const float h = taps[tb + tt];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) acc[r] = fmaf(h, w[r - tt + 7], acc[r]);
+        }
+#pragma unroll
+        for (int d = 6; d >= 0; --d) w[d + 8] = w[d];
+    }
+}
+
+template <int TZ, bool ENV>
+__global__ void __launch_bounds__(256) post_fir_kernel(const PostParams P) {
+    extern __shared__ float post_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int col0 = blockIdx.x * 32, r0 = blockIdx.y * TZ, f = blockIdx.z;
+    const int col = col0 + lane;
+    // y rows this block needs and x rows those need
+    const int yr0 = ENV ? r0 + P.shiftH - P.TpH + 1 : r0;
+    const int YR = ENV ? ((TZ + P.TpH - 1 + 7) & ~7) : TZ;
+    const int xr0 = yr0 + P.shiftB - P.TpB + 1;
+    const int XR = YR + P.TpB - 1;
+    float* xs = post_smem;                    // [XR][32]
+    float* ys = xs + XR * 32;            // [YR][32]   (ENV only)
+    float* hb = ys + (ENV ? YR * 32 : 0);   // [TpB]
+    float* hh = hb + P.TpB;              // [TpH]
+    for (int t = threadIdx.x; t < P.TpB; t += 256) hb[t] = P.taps_bp[t];
+    if (ENV) for (int t = threadIdx.x; t < P.TpH; t += 256) hh[t] = P.taps_h[t];
+    const float* img = P.x + (size_t)f * P.nz * P.nx;
+    for (int r = warp; r < XR; r += 8) {
+        const int gr = xr0 + r;
+        xs[r * 32 + lane] = (gr >= 0 && gr < P.nz && col < P.nx) ? img[(size_t)gr * P.nx + col] : 0.0f;
+    }
+    __syncthreads();
+    float acc[8];
+    if constexpr (!ENV) {
+        for (int g = warp; g < TZ / 8; g += 8) {
+            const int m0 = r0 + g * 8;
+            fir8(xs + lane, xr0, hb, P.TpB, P.shiftB, m0, acc);
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+                if (m0 + r < P.nz && col < P.nx) P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = acc[r];
+        }
+    } else {
+    for (int g = warp; g < YR / 8; g += 8) {
+        const int m0 = yr0 + g * 8;
+        fir8(xs + lane, xr0, hb, P.TpB, P.shiftB, m0, acc);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) ys[(g * 8 + r) * 32 + lane] = (m0 + r >= 0 && m0 + r < P.nz) ? acc[r] : 0.0f;
+    }
+    __syncthreads();
+    float vmax = 0.0f;
+    for (int g = warp; g < TZ / 8; g += 8) {
+        const int m0 = r0 + g * 8;
+        fir8(ys + lane, yr0, hh, P.TpH, P.shiftH, m0, acc);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const float y = ys[(m0 + r - yr0) * 32 + lane];
+            const float env = sqrtf(fmaf(y, y, acc[r] * acc[r]));
+            if (m0 + r < P.nz && col < P.nx) {
+                P.out[((size_t)f * P.nz + m0 + r) * P.nx + col] = env;
+                vmax = fmaxf(vmax, env);
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+    if (lane == 0 && vmax > 0.0f) atomicMax(P.frame_max + f, __float_as_uint(vmax));
+    }
+}
+
+// a9: out = max(20 log10(env / M_frame), -DR); env = 0 or M = 0 gives -DR (A10).  In place.
+// grid: (ceil(npix / 1024), F), 256 threads x 4 pixels.
+__global__ void __launch_bounds__(256) post_log_kernel(float* __restrict__ img, const unsigned int* __restrict__ frame_max,
+                                                        int npix, float dyn_range_db) {
+    const int f = blockIdx.y;
+    const float M = __uint_as_float(frame_max[f]);
+    const float lgM = lg2_approx(M);
+    float* p = img + (size_t)f * npix;
+    const float k = 6.02059991327962f;   // 20 log10(2)
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int i = (blockIdx.x * 4 + u) * 256 + threadIdx.x;
+        if (i < npix) {
+            const float e = p[i];
+            float v = -dyn_range_db;
+            if (M > 0.0f && e > 0.0f) v = fmaxf(k * (lg2_approx(e) - lgM), -dyn_range_db);
+            p[i] = v;
+        }
+    }
+}
+
+__device__ __forceinline__ float log_db(float e, float M, float lgM, float dr) {
+    const float k = 6.02059991327962f;   // 20 log10(2)
+    return (M > 0.0f && e > 0.0f) ? fmaxf(k * (lg2_approx(e) - lgM), -dr) : -dr;
+}
+
+// The same for npix a multiple of 4 at a 16-byte aligned address.  grid: (ceil(npix / 4096), F), 256 threads x 4 x 128 bit.
+__global__ void __launch_bounds__(256) post_log_vec_kernel(float4* __restrict__ img, const unsigned int* __restrict__ frame_max,
+                                                            int npix4, float dyn_range_db) {
+    const int f = blockIdx.y;
+    const float M = __uint_as_float(frame_max[f]);
+    const float lgM = lg2_approx(M);
+    float4* p = img + (size_t)f * npix4;
+    float4 e[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int i = (blockIdx.x * 4 + u) * 256 + threadIdx.x;
+        e[u] = i < npix4 ? p[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int i = (blockIdx.x * 4 + u) * 256 + threadIdx.x;
+        if (i < npix4)
+            __stcs(p + i, make_float4(log_db(e[u].x, M, lgM, dyn_range_db), log_db(e[u].y, M, lgM, dyn_range_db),
+                                      log_db(e[u].z, M, lgM, dyn_range_db), log_db(e[u].w, M, lgM, dyn_range_db)));
+    }
+}
+
+inline void launch_post_log(float* out, const unsigned int* frame_max, int npix, int F, float dr, cudaStream_t st) {
+    if (npix % 4 == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0)
+        post_log_vec_kernel<<<dim3((npix / 4 + 1023) / 1024, F), 256, 0, st>>>((float4*)out, frame_max, npix / 4, dr);
+    else
+        post_log_kernel<<<dim3((npix + 1023) / 1024, F), 256, 0, st>>>(out, frame_max, npix, dr);
+}
+
 
 // Blackwell packed fp32 FMA (FFMA2): two independent fp32 FMAs, each rounded as fmaf, in one issue slot.
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {

@@ -18,62 +18,6 @@ struct Span {
     }
 };
 
-template <typename T>
-void launch_ingest_quad(const void* rf, float* stage, int F, int N, int S, float scale, cudaStream_t st) {
-    const int nq = (F + 3) / 4;
-    dim3 grid((S + 1023) / 1024, N, nq);
-    if constexpr (std::is_same<T, float>::value) {
-        if (S % 4 == 0 && (reinterpret_cast<uintptr_t>(rf) & 15) == 0) {
-            ingest_quad_vec_kernel<<<dim3((S / 4 + 255) / 256, N, nq), 256, 0, st>>>((const float4*)rf, (float4*)stage, F, N, S / 4, scale);
-            return;
-        }
-    }
-    ingest_quad_kernel<T><<<grid, 256, 0, st>>>((const T*)rf, (float4*)stage, F, N, S, scale);
-}
-template <typename T>
-void launch_ingest_lin(const void* rf, float* stage, int F, int N, int S, int Sp, float scale, cudaStream_t st) {
-    dim3 grid((Sp + 255) / 256, N, F);
-    ingest_lin_kernel<T><<<grid, 256, 0, st>>>((const T*)rf, stage, N, S, Sp, scale);
-}
-
-template <int K, int NQ, int W>
-void launch_direct(const BfParams& P, int groups, cudaStream_t st) {
-    dim3 grid((P.nx + kDirectCols - 1) / kDirectCols, (P.nz + kDirectRows - 1) / kDirectRows, groups);
-    bf_direct_kernel<K, NQ, W><<<grid, 256, 0, st>>>(P);
-}
-
-template <int NQ, int W>
-void launch_direct_order_w(int order, const BfParams& P, int groups, cudaStream_t st) {
-    switch (order) {
-    case 1: launch_direct<1, NQ, W>(P, groups, st); break;
-    case 2: launch_direct<2, NQ, W>(P, groups, st); break;
-    case 3: launch_direct<3, NQ, W>(P, groups, st); break;
-    case 4: launch_direct<4, NQ, W>(P, groups, st); break;
-    case 5: launch_direct<5, NQ, W>(P, groups, st); break;
-    default:
-        if constexpr (NQ <= 1 && W == 0) {          // orders 6..8: at most 4 frames per thread, no weighting
-            if (order == 6) launch_direct<6, NQ, W>(P, groups, st);
-            else if (order == 7) launch_direct<7, NQ, W>(P, groups, st);
-            else launch_direct<8, NQ, W>(P, groups, st);
-        }
-        break;
-    }
-}
-
-// nq = 0: lin layout, one frame per thread; 1, 2, 4 quads per thread (4 only without weighting)
-void launch_direct_nq(int order, int nq, int weight, const BfParams& P, int groups, cudaStream_t st) {
-    if (weight == 0) {
-        if (nq == 4) launch_direct_order_w<4, 0>(order, P, groups, st);
-        else if (nq == 2) launch_direct_order_w<2, 0>(order, P, groups, st);
-        else if (nq == 1) launch_direct_order_w<1, 0>(order, P, groups, st);
-        else launch_direct_order_w<0, 0>(order, P, groups, st);
-    } else {
-        if (nq == 2) launch_direct_order_w<2, 1>(order, P, groups, st);
-        else if (nq == 1) launch_direct_order_w<1, 1>(order, P, groups, st);
-        else launch_direct_order_w<0, 1>(order, P, groups, st);
-    }
-}
-
 // One batch (<= plan.batch_frames frames): ingest -> beamform -> post.  rf points at the batch's first frame
 // in the caller's layout, out at the batch's first image.
 int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaStream_t st) {
@@ -87,14 +31,13 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
     P.out = post ? ctx->d_img : out;
     const bool in_range = ctx->plan.in_range != 0;
     const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
-                            (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0 && staged_available());
+                            (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0);
 
     if (ctx->interp == PAB_INTERP_NEAREST) {
         // row f4: rooted quad staging, then the table-driven gather kernel (always the quad layout)
         {
             Span sp(ctx, PAB_STAGE_INGEST, st);
-            if (ctx->dtype == PAB_I16) launch_ingest_root_quad<int16_t>(order, rf, ctx->d_stage, F, N, S, ctx->scale, st);
-            else launch_ingest_root_quad<float>(order, rf, ctx->d_stage, F, N, S, ctx->scale, st);
+            xl_ingest_root_quad(ctx->dtype, order, rf, ctx->d_stage, F, N, S, ctx->scale, st);
         }
         int nq = (F + 3) / 4, q0 = 0;
         int g0 = ctx->plan.frames_per_thread / 4;
@@ -107,16 +50,16 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.out = P.out + (size_t)(4 * q0) * nz * (size_t)nx;
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (use_staged && nearest_staged_fits(ctx->plan, g, ctx->tuning.stages, ctx->smem_optin))
-                launch_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.stages, ctx->tuning.chunk_channels,
+            if (use_staged && xl_nearest_staged_fits(ctx->plan, g, ctx->tuning.stages, ctx->smem_optin))
+                xl_nearest_staged(order, g, in_range, R, groups, ctx->plan, ctx->tuning.stages, ctx->tuning.chunk_channels,
                                                   ctx->smem_optin, ctx->sm_count, ctx->d_near, st);
-            else launch_nearest_direct(order, g, R, groups, ctx->d_near, st);
+            else xl_nearest_direct(order, g, R, groups, ctx->d_near, st);
             q0 += groups * g;
             nq -= groups * g;
         }
     } else if (F < 4) {
         const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
-                            cached_fits(ctx->plan, 0, ctx->d_compact != nullptr, ctx->smem_optin);
+                            xl_cached_fits(ctx->plan, 0, ctx->d_compact != nullptr, ctx->smem_optin);
         // lin layout, one frame per thread.  fp32 input with unit scale and 16-byte rows is read in place.
         const bool in_place = ctx->dtype == PAB_F32 && ctx->scale == 1.0f && (S % 4) == 0 &&
                               ((uintptr_t)rf % 16) == 0;
@@ -125,24 +68,22 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         } else {
             {
                 Span sp(ctx, PAB_STAGE_INGEST, st);
-                if (ctx->dtype == PAB_I16) launch_ingest_lin<int16_t>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
-                else launch_ingest_lin<float>(rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
+                xl_ingest_lin(ctx->dtype, rf, ctx->d_stage, F, N, S, ctx->Sp, ctx->scale, st);
             }
             P.rf = ctx->d_stage;
         }
         P.n_frames = F;
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            if (cached) launch_cached(order, 0, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
+            if (cached) xl_cached(order, 0, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                                       CacheTables{ctx->d_taps, ctx->d_w0s, ctx->d_compact, ctx->cache_q}, st);
-            else if (use_staged) launch_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
-            else launch_direct_nq(order, 0, weight, P, F, st);
+            else if (use_staged) xl_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
+            else xl_direct(order, 0, weight, P, F, st);
         }
     } else {
         {
             Span sp(ctx, PAB_STAGE_INGEST, st);
-            if (ctx->dtype == PAB_I16) launch_ingest_quad<int16_t>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
-            else launch_ingest_quad<float>(rf, ctx->d_stage, F, N, S, ctx->scale, st);
+            xl_ingest_quad(ctx->dtype, rf, ctx->d_stage, F, N, S, ctx->scale, st);
         }
         // quads are consumed in groups of frames_per_thread / 4, then the remainder in halves (4 -> 2 -> 1)
         int nq = (F + 3) / 4, q0 = 0;
@@ -160,11 +101,11 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             R.n_frames = F - 4 * q0;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
             if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && (order <= 5 || g == 1) &&
-                (weight == 0 || cached_weight_ok(order, g, false)) && cached_fits(ctx->plan, g, false, ctx->smem_optin))
-                launch_cached(order, g, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
+                (weight == 0 || xl_cached_weight_ok(order, g, false)) && xl_cached_fits(ctx->plan, g, false, ctx->smem_optin))
+                xl_cached(order, g, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
                               CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);
-            else if (use_staged) launch_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
-            else launch_direct_nq(order, g, weight, R, groups, st);
+            else if (use_staged) xl_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
+            else xl_direct(order, g, weight, R, groups, st);
             q0 += groups * g;
             nq -= groups * g;
         }
@@ -176,35 +117,16 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         Q.TpB = ctx->TpB; Q.shiftB = ctx->n_taps_bp / 2;
         Q.TpH = ctx->TpH; Q.shiftH = (ctx->n_taps_h - 1) / 2;
         Q.nx = nx; Q.nz = nz;
-        constexpr int TZ = 128;
-        dim3 grid((nx + 31) / 32, (nz + TZ - 1) / TZ, F);
-        if (ctx->post_fast) {
-            const bool env = ctx->post_mode >= PAB_ENVELOPE;
-            if (env) cudaMemsetAsync(ctx->d_max, 0, (size_t)F * 4, st);
-            {
-                Span sp(ctx, PAB_STAGE_POST_FIR, st);
-                launch_post64(Q, ctx->taps64, env, ctx->hilbert_parity, F, st);
-            }
-            if (ctx->post_mode == PAB_LOG) {
-                Span sp(ctx, PAB_STAGE_POST_LOG, st);
-                launch_post_log(out, ctx->d_max, nx * nz, F, ctx->dyn_range_db, st);
-            }
-        } else if (ctx->post_mode == PAB_BANDPASS) {
-            const size_t sm = ((size_t)(TZ + Q.TpB - 1) * 32 + Q.TpB + Q.TpH) * 4;
+        const bool env = ctx->post_mode >= PAB_ENVELOPE;
+        if (env) cudaMemsetAsync(ctx->d_max, 0, (size_t)F * 4, st);
+        {
             Span sp(ctx, PAB_STAGE_POST_FIR, st);
-            post_fir_kernel<TZ, false><<<grid, 256, sm, st>>>(Q);
-        } else {
-            const int YR = (TZ + Q.TpH - 1 + 7) & ~7;
-            const size_t sm = ((size_t)(YR + Q.TpB - 1) * 32 + (size_t)YR * 32 + Q.TpB + Q.TpH) * 4;
-            cudaMemsetAsync(ctx->d_max, 0, (size_t)F * 4, st);
-            {
-                Span sp(ctx, PAB_STAGE_POST_FIR, st);
-                post_fir_kernel<TZ, true><<<grid, 256, sm, st>>>(Q);
-            }
-            if (ctx->post_mode == PAB_LOG) {
-                Span sp(ctx, PAB_STAGE_POST_LOG, st);
-                launch_post_log(out, ctx->d_max, nx * nz, F, ctx->dyn_range_db, st);
-            }
+            if (ctx->post_fast) xl_post64(Q, ctx->taps64, env, ctx->hilbert_parity, F, st);
+            else xl_post_generic(Q, env, F, st);
+        }
+        if (ctx->post_mode == PAB_LOG) {
+            Span sp(ctx, PAB_STAGE_POST_LOG, st);
+            xl_post_log(out, ctx->d_max, nx * nz, F, ctx->dyn_range_db, st);
         }
     }
     cudaError_t e = cudaGetLastError();
@@ -216,6 +138,8 @@ int check_args(pab_ctx* ctx, const void* rf, int n_frames, int order, const floa
     if (!ctx || !rf || !out || n_frames < 1 || order < 1 || order > PAB_MAX_ORDER) return PAB_ERR_INVALID;
     if (order > 5 && (ctx->weight != PAB_WEIGHT_NONE || ctx->interp != PAB_INTERP_LINEAR)) return PAB_ERR_INVALID;
     if (((uintptr_t)rf % elem_size(ctx->dtype)) != 0 || ((uintptr_t)out % 4) != 0) return PAB_ERR_INVALID;
+    int dev = -1;                         // the context lives on the device that was current at pab_create
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device) return PAB_ERR_INVALID;
     return PAB_OK;
 }
 

@@ -9,75 +9,10 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
-#include "../../include/pab.h"
-#include "pab_kernels.cuh"
-#include "pab_plan.h"
+#include "pab_math.cuh"
+#include "pab_pipe.cuh"
 
 namespace pab {
-
-constexpr int kStgRows = 64, kStgCols = 8, kStgConsumerWarps = 16;
-constexpr int kStgThreads = (kStgConsumerWarps + 1) * 32;
-constexpr int kStgMaxStages = 4;
-
-// per staged channel: what a consumer needs besides the samples (80 bytes; every read is a warp broadcast)
-struct __align__(16) ChanEntry {
-    float2 xs[8];           // per pixel column c of the tile: (xs2, c0) of delay_tap, xs = column - element in samples
-    int base;               // shared-space address such that sample i of the first quad lives at base + i * BPS
-    int w0;                 // first staged sample
-    int w1m2;               // last valid i0 (staged end - 2)
-    int pad;
-};
-static_assert(sizeof(ChanEntry) == kChanEntryBytes, "ChanEntry size is part of the shared-memory plan");
-constexpr int kCE = (int)sizeof(ChanEntry);
-
-__device__ __forceinline__ float2 lds64(uint32_t addr) {
-    float2 v;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-    return v;
-}
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-__device__ __forceinline__ float4 lds128(uint32_t addr) {
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ float lds32(uint32_t addr) {
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-    return v;
-}
-
-struct StagedCfg {
-    int chunk;          // channels per stage (<= 32)
-    int stages;         // ring depth
-    int window;         // samples per channel slot per quad (multiple of 4)
-    int tiles_x, tiles_z, groups;   // tile grid: columns / 8, rows / 64, frame groups; tile t = (t % tiles_x, ...)
-};
 
 // NQ = 0: lin layout, one frame per thread; NQ = 1, 2, 4: quad layout, 4 NQ frames per thread.
 // INR: every delay index of the geometry lies inside the record (checked on the host): no masks, no clamps.
@@ -272,28 +207,11 @@ inline bool staged_configure_inr(int smem_optin) {
            staged_set_attr_orders<0, INR, 1>(smem_optin) == cudaSuccess && staged_set_attr_orders<1, INR, 1>(smem_optin) == cudaSuccess &&
            staged_set_attr_orders<2, INR, 1>(smem_optin) == cudaSuccess;
 }
-inline int staged_configure(int smem_optin) {
-    return staged_configure_inr<false>(smem_optin) && staged_configure_inr<true>(smem_optin) ? PAB_OK : PAB_ERR_CUDA;
-}
-inline bool staged_available() { return true; }
-
-// Shared-memory bytes of one launch: the plan's chunk is sized for `frames_per_thread / 4` quads per channel;
-// with fewer bytes per sample the same chunk fits with room to spare.
-inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
-    const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
-    const size_t tab = ((size_t)c.stages * c.chunk * sizeof(ChanEntry) + 127) & ~(size_t)127;
-    return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy;
-}
 
 template <int K, int NQ, bool INR, int W>
 inline void launch_staged_k(const BfParams& P, const StagedCfg& c, int sm_count, cudaStream_t st) {
     const size_t smem = staged_smem_bytes(c, NQ);
-    int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf_staged_kernel<K, NQ, INR, W>, kStgThreads, smem) != cudaSuccess ||
-        per_sm < 1) {
-        cudaGetLastError();
-        per_sm = 1;
-    }
+    const int per_sm = resident_per_sm(bf_staged_kernel<K, NQ, INR, W>, kStgThreads, smem);
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups;
     const long long resident = (long long)sm_count * per_sm;
     bf_staged_kernel<K, NQ, INR, W><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(P, c);
@@ -329,8 +247,9 @@ inline void launch_staged_inr(int order, int nq, int weight, const BfParams& P, 
         else launch_staged_nq<2, INR, 1>(order, P, c, sm_count, st);
     }
 }
-inline void launch_staged(int order, int nq, bool in_range, int weight, const BfParams& P, int groups, const pab_plan_info& plan,
-                          int chunk_cap, int smem_limit, int sm_count, cudaStream_t st) {
+template <bool INR>
+inline void launch_staged_t(int order, int nq, int weight, const BfParams& P, int groups, const pab_plan_info& plan,
+                            int chunk_cap, int smem_limit, int sm_count, cudaStream_t st) {
     // the plan's chunk is sized for frames_per_thread / 4 quads per channel; fewer quads -> more channels per stage
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (long long)sizeof(ChanEntry);
     long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
@@ -340,8 +259,7 @@ inline void launch_staged(int order, int nq, bool in_range, int weight, const Bf
     if (chunk < 1) chunk = 1;       // cannot happen: the plan fitted >= 1 channel at the largest nq
     StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
                 (P.nz + kStgRows - 1) / kStgRows, groups};
-    if (in_range) launch_staged_inr<true>(order, nq, weight, P, c, sm_count, st);
-    else launch_staged_inr<false>(order, nq, weight, P, c, sm_count, st);
+    launch_staged_inr<INR>(order, nq, weight, P, c, sm_count, st);
 }
 
 }  // namespace pab
