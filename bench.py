@@ -51,6 +51,7 @@ FP32_PER_ITEM = 6.0
 DELAY_CACHE = "all"
 SM_COUNT = 148
 NCU_TRAFFIC_BYTES = 185_511_680 + 51_419_136   # per 64-frame launch; profiles/r1_step_ncu_f.md
+NCU_TRAFFIC_COMMIT = "17be8fa (round 1)"       # the build that capture was taken on: the constant goes stale silently otherwise
 XU_LANES_PER_CLK_SM = 16
 FP32_LANES_PER_CLK_SM = 128
 
@@ -238,6 +239,23 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     e2e_ms = (time.perf_counter() - t0) * 1e3
     checksum = float(out_host[0, 512, 128])
 
+    # the same with int16 transport (BASELINE.json config C5: the ADC data is int16): the C2b frames quantised to
+    # 15 bits of their peak, scale restored by pab_set_input; half the host-to-device bytes
+    peak_rf = float(np.max(np.abs(rf_np)))
+    q_scale = peak_rf / 32000.0
+    rf16_host = torch.from_numpy(np.rint(rf_np / q_scale).astype(np.int16)).pin_memory()
+    bf16 = binding.Beamformer(g, dtype="int16", scale=q_scale, post=POST, delay_cache=DELAY_CACHE)
+    for _ in range(2):
+        bf16.beamform_host(rf16_host, ORDER, out=out_host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        bf16.beamform_host(rf16_host, ORDER, out=out_host)
+    torch.cuda.synchronize()
+    e2e16_ms = (time.perf_counter() - t0) * 1e3
+    bf16.close()
+    box = binding.measure_peaks() if rank == 0 else None      # bare pinned cudaMemcpyAsync rates of this box, same run
+
     # ---- beamform-only (raw output) throughput, for the stage breakdown ----
     bf_raw = binding.Beamformer(g, delay_cache=DELAY_CACHE)
     for i in range(3):
@@ -252,7 +270,20 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     raw_ms = r0.elapsed_time(r1) / K
     bf_raw.close()
 
-    ms_total, e2e_ms = max_over_ranks([ms_total, e2e_ms], world, dev)
+    # the in-kernel-delay (table-free) headline beside the cached one
+    bf_nc = binding.Beamformer(g, delay_cache="off")
+    for i in range(3):
+        bf_nc.beamform(rf_sets[i % N_SETS], ORDER, out=out_sets[i % N_SETS], stream=stream)
+    torch.cuda.synchronize()
+    bf_nc.set_profile(4 * K + 8)
+    for i in range(K):
+        bf_nc.beamform(rf_sets[i % N_SETS], ORDER, out=out_sets[i % N_SETS], stream=stream)
+    torch.cuda.synchronize()
+    nc_ms, nc_n = bf_nc.get_profile()["beamform"]
+    nc_launch_ms = nc_ms / max(nc_n, 1)
+    bf_nc.close()
+
+    ms_total, e2e_ms, e2e16_ms = max_over_ranks([ms_total, e2e_ms, e2e16_ms], world, dev)
     if rank == 0:
         peaks = read_peaks()
         ms_step = ms_total / K
@@ -272,7 +303,12 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         roofline = {"bound": "alu", "kernel": "bf_cached_kernel<3,4,false> (fused tap fetch + interpolation + root + power sums + Newton, 16 frames "
                               "per thread, cached interpolation taps)",
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
-                    "frac": achieved / xu_peak, "traffic": NCU_TRAFFIC_BYTES,
+                    "frac": achieved / xu_peak, "frac_definition": "XU (MUFU) pipe term of T_roof (DESIGN.md reading B3)",
+                    "frac_xu": t_xu / (bf_launch_ms * 1e-3),
+                    "frac_fp32_hbm": max(t_fp32, t_hbm) / (bf_launch_ms * 1e-3),      # north_star's literal FMA-rate reading
+                    "in_kernel_delays": {"launch_ms": nc_launch_ms,
+                                         "frac_xu": items_per_launch * (XU_PER_ITEM + 1.0 / FRAMES) / xu_peak / (nc_launch_ms * 1e-3)},
+                    "traffic": NCU_TRAFFIC_BYTES, "traffic_commit": NCU_TRAFFIC_COMMIT,
                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
                                       "kernel at this workload: profiles/r1_step_ncu_f.md",
                     "peak_source": f"148 SM x 16 XU lanes/clk x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, "
@@ -296,7 +332,15 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                 "e2e": {"value": world * FRAMES * Ke / (e2e_ms * 1e-3), "unit": "frames/s",
                         "h2d_bytes_per_step": int(rf_host.numel() * 4), "d2h_bytes_per_step": int(out_host.numel() * 4),
                         "ms_per_step": e2e_ms / Ke, "steps": Ke, "api": "pab_beamform_host (pinned host buffers)",
-                        "checksum": checksum},
+                        "checksum": checksum,
+                        "h2d_ceiling_gbs": box["h2d_pinned_gbs"], "d2h_ceiling_gbs": box["d2h_pinned_gbs"],
+                        "copy_bound_ms": max(rf_host.numel() * 4 / box["h2d_pinned_gbs"], out_host.numel() * 4 / box["d2h_pinned_gbs"]) * 1e-6,
+                        "int16_input": {"value": world * FRAMES * Ke / (e2e16_ms * 1e-3), "ms_per_step": e2e16_ms / Ke,
+                                        "h2d_bytes_per_step": int(rf16_host.numel() * 2),
+                                        "note": "same frames quantised to int16 (scale restored by pab_set_input)"}},
+                "timing_note": "per-launch profiling events (pab_set_profile) are recorded inside the timed region: "
+                               "two event records per kernel, a slight downward bias of value",
+                "box_peaks": box,
                 "gpu_launches": int(launches), "clocks": clk, "roofline": roofline, "stages": stages,
                 "raw_only": {"ms_per_step": raw_ms, "frames_per_s": FRAMES / (raw_ms * 1e-3),
                              "items_per_s": FRAMES * items_per_frame / (raw_ms * 1e-3)}}
@@ -467,12 +511,20 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--table2", action="store_true", help="square grids shaped like the paper's Table II; 1 GPU")
     ap.add_argument("--sweep", action="store_true", help="per-config table (C1..C5), one JSON line each; 1 GPU")
+    ap.add_argument("--peaks", action="store_true", help="pab_measure_peaks: MUFU / FFMA / LDS.128 unit rates and pinned "
+                                                         "copy rates of this box, one JSON line; 1 GPU")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.peaks:
+        if rank == 0:
+            from paper_2203_14906_b200 import binding
+            binding.load(build_if_missing=True)
+            print(json.dumps({"peaks": binding.measure_peaks()}), flush=True)
         return
     if args.sweep or args.table2:
         if rank == 0:

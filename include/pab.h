@@ -221,6 +221,14 @@ long long pab_launch_count(const pab_ctx* ctx);
 int pab_set_profile(pab_ctx* ctx, int max_launches);
 int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset);
 
+/* pab_measure_peaks -- the microbenchmarks behind the roofline denominators, run on the
+ * current device: out_host[0] MUFU (lg2/ex2) lanes per clock per SM, [1] FFMA lanes/clk/SM, [2] packed FFMA2 fp32
+ * results/clk/SM, [3] conflict-free LDS.128 bytes/clk/SM (each timed with clock64 inside one 1024-thread CTA per
+ * SM), [4] pinned host->device and [5] device->host GB/s of a 64 MiB cudaMemcpyAsync, [6] the SM clock seen during
+ * the MUFU loop in MHz, [7] the SM count.  n_out >= 8.  Synchronises the device.  Measurement only: nothing on the
+ * hot path calls it.  Errors: PAB_ERR_INVALID, PAB_ERR_DEVICE, PAB_ERR_ALLOC, PAB_ERR_CUDA. */
+int pab_measure_peaks(double* out_host, int n_out);
+
 /* Image-quality metrics of the paper's evaluation (SNR eq. 10, CR eq. 11, gCNR eq. 12, FWHM),
  * SURVEY.md section 8(f) row f3, reading A22.  Regions are pixel rectangles. */
 typedef struct { int r0, r1, c0, c1; } pab_roi;          /* rows [r0, r1), columns [c0, c1), non-empty, inside the grid */

@@ -25,7 +25,7 @@ _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_S
 # every symbol include/pab.h declares
 SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_delay_cache", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
-           "pab_launch_count", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
+           "pab_launch_count", "pab_measure_peaks", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
 
 class Grid(C.Structure):
@@ -90,6 +90,7 @@ def load(build_if_missing: bool = False):
     L.pab_launch_count.argtypes = [vp]
     L.pab_launch_count.restype = C.c_longlong
     L.pab_image_metrics.argtypes = [vp, vp, C.POINTER(Roi), C.POINTER(Roi), ip, ip, C.POINTER(Metrics), vp]
+    L.pab_measure_peaks.argtypes = [C.POINTER(C.c_double), ip]
     L.pab_set_profile.argtypes = [vp, ip]
     L.pab_get_profile.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong), ip]
     L.pab_strerror.argtypes = [ip]
@@ -131,6 +132,17 @@ def design_hilbert(half_len: int):
     if rc != OK:
         raise PabError(f"pab_design_hilbert: {load().pab_strerror(rc).decode()}")
     return g
+
+
+def measure_peaks() -> dict:
+    """pab_measure_peaks on the current device: the measured unit rates behind the roofline denominators."""
+    out = (C.c_double * 8)()
+    rc = load().pab_measure_peaks(out, 8)
+    if rc != OK:
+        raise PabError(f"pab_measure_peaks: {load().pab_strerror(rc).decode()}")
+    keys = ("mufu_lanes_per_clk_sm", "ffma_lanes_per_clk_sm", "ffma2_results_per_clk_sm", "lds128_bytes_per_clk_sm",
+            "h2d_pinned_gbs", "d2h_pinned_gbs", "sm_clock_mhz", "sm_count")
+    return dict(zip(keys, [float(v) for v in out]))
 
 
 def shard_frames(n_frames: int, rank: int, world: int):

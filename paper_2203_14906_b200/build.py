@@ -28,6 +28,7 @@ UNITS = {
     "pab_tu_cached.cu": _KERNEL + ["pab_cache.cuh"],
     "pab_tu_nearest.cu": _KERNEL + ["pab_nearest.cuh"],
     "pab_tu_post.cu": _KERNEL + ["pab_post.cuh", "pab_metrics.cuh"],
+    "pab_tu_peaks.cu": [os.path.join("..", "..", "include", "pab.h")],
 }
 SOURCES = list(UNITS)
 DEPS = sorted({d for u, ds in UNITS.items() for d in [u] + ds})

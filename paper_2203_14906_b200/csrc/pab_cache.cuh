@@ -149,11 +149,15 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
         const int bx = txy % C.tiles_x, by = txy / C.tiles_x;
         const int j = bx * kStgCols + col;
         const int m = by * kStgRows + (warp >> 3) * 32 + lane;
-        float p[NF][kAcc<K, W>];
+        // one frame per thread: scalar accumulators; frame groups: the frames in pairs, packed f32x2 arithmetic
+        float p[1][kAcc<K, W>];
+        float2 pp[NQ == 0 ? 1 : NF / 2][kAcc<K, W>];
 #pragma unroll
-        for (int f = 0; f < NF; ++f)
+        for (int k = 0; k < kAcc<K, W>; ++k) p[0][k] = 0.0f;
 #pragma unroll
-            for (int k = 0; k < kAcc<K, W>; ++k) p[f][k] = 0.0f;
+        for (int f = 0; f < (NQ == 0 ? 1 : NF / 2); ++f)
+#pragma unroll
+            for (int k = 0; k < kAcc<K, W>; ++k) pp[f][k] = make_float2(0.0f, 0.0f);
         // COMPACT: this pixel's row of the (d, row) table; d = j - q i + q (N - 1) falls by q per element
         // (32-bit entry index: pab_set_delay_cache builds the compact table only below 2^31 entries)
         const uint32_t ci0 = (uint32_t)(min(j, P.nx - 1) + q * (P.N - 1)) * (uint32_t)P.nz + (uint32_t)min(m, P.nz - 1);
@@ -187,10 +191,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                     for (int q = 0; q < NQ; ++q) {
                         const float4 s0 = lds128(addr + q * quad_bytes);
                         const float4 s1 = lds128(addr + q * quad_bytes + 16);
-                        accumulate_w<K, W>(fmaf(a, s1.x - s0.x, s0.x), p[4 * q + 0]);
-                        accumulate_w<K, W>(fmaf(a, s1.y - s0.y, s0.y), p[4 * q + 1]);
-                        accumulate_w<K, W>(fmaf(a, s1.z - s0.z, s0.z), p[4 * q + 2]);
-                        accumulate_w<K, W>(fmaf(a, s1.w - s0.w, s0.w), p[4 * q + 3]);
+                        accumulate2_w<K, W>(interp2(a, make_float2(s0.x, s0.y), make_float2(s1.x, s1.y)), pp[2 * q + 0]);
+                        accumulate2_w<K, W>(interp2(a, make_float2(s0.z, s0.w), make_float2(s1.z, s1.w)), pp[2 * q + 1]);
                     }
                 }
             }
@@ -204,7 +206,12 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
-                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[f], P.inv_n);
+                if (frame < P.n_frames) {
+                    float v;
+                    if constexpr (NQ == 0) v = combine_w<K, W>(p[0], P.inv_n);
+                    else v = combine2_w<K, W>(pp[f / 2], f & 1, P.inv_n);
+                    P.out[(size_t)frame * img + (size_t)m * P.nx + j] = v;
+                }
             }
         }
     }

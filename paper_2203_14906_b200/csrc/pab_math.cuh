@@ -119,6 +119,103 @@ __device__ __forceinline__ float combine_w(const float (&p)[kAcc<K, W>], float i
     }
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Packed forms of a3..a5 for the frame-group kernels: Blackwell issues two independent fp32 operations, each rounded
+// as its scalar counterpart, in one slot (PTX add/sub/mul/fma .f32x2, SASS FADD2 / FMUL2 / FFMA2).  The frames a thread
+// carries are natural pairs (the x,y and z,w halves of a 128-bit staged sample), so the interpolation, the scaling of
+// the logarithm and the power-sum updates take one slot per two frames; the MUFU roots and the LOP3 sign copy stay
+// scalar.  Order 3: 6.5 instead of 9 issue slots per item beside the shared loads.
+// ------------------------------------------------------------------------------------------------------
+#define PAB_U64(v) (reinterpret_cast<unsigned long long&>(v))
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(PAB_U64(a)), "l"(PAB_U64(b)));
+    return reinterpret_cast<float2&>(r);
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(PAB_U64(a)), "l"(PAB_U64(b)));
+    return reinterpret_cast<float2&>(r);
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(PAB_U64(a)), "l"(PAB_U64(b)));
+    return reinterpret_cast<float2&>(r);
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(PAB_U64(a)), "l"(PAB_U64(b)), "l"(PAB_U64(c)));
+    return reinterpret_cast<float2&>(r);
+}
+#undef PAB_U64
+__device__ __forceinline__ float2 bcast2(float a) { return make_float2(a, a); }
+
+// a3 for an in-range tap: s = s0 + a (s1 - s0) on two frames
+__device__ __forceinline__ float2 interp2(float a, float2 s0, float2 s1) { return fma2(bcast2(a), sub2(s1, s0), s0); }
+
+// a4 + a5 on two frames: p[m] holds the pair's p_(m+1).  The even powers need no sign, so they are formed from the
+// unsigned root r; p_K = sum s (odd K) is accumulated from s itself; for even K, |s| = r^K to 2^-22 relative.
+template <int K>
+__device__ __forceinline__ void accumulate2(float2 s, float2 (&p)[K]) {
+    if constexpr (K == 1) {
+        p[0] = add2(p[0], s);
+    } else if constexpr (K == 2) {
+        const float2 r = make_float2(sqrt_approx(fabsf(s.x)), sqrt_approx(fabsf(s.y)));
+        p[0] = add2(p[0], make_float2(copy_sign(r.x, s.x), copy_sign(r.y, s.y)));
+        p[1] = fma2(r, r, p[1]);
+    } else if constexpr (K == 3) {
+        const float2 t = mul2(make_float2(lg2_approx(fabsf(s.x)), lg2_approx(fabsf(s.y))), bcast2(1.0f / 3.0f));
+        const float2 r = make_float2(ex2_approx(t.x), ex2_approx(t.y));
+        p[0] = add2(p[0], make_float2(copy_sign(r.x, s.x), copy_sign(r.y, s.y)));
+        p[1] = fma2(r, r, p[1]);
+        p[2] = add2(p[2], s);
+    } else if constexpr (K == 4) {
+        const float2 r = make_float2(rsqrt_approx(rsqrt_approx(fabsf(s.x))), rsqrt_approx(rsqrt_approx(fabsf(s.y))));
+        const float2 u = make_float2(copy_sign(r.x, s.x), copy_sign(r.y, s.y));
+        const float2 u2 = mul2(r, r);
+        p[0] = add2(p[0], u);
+        p[1] = add2(p[1], u2);
+        p[2] = fma2(u2, u, p[2]);
+        p[3] = fma2(u2, u2, p[3]);
+    } else if constexpr (K == 5) {
+        const float2 t = mul2(make_float2(lg2_approx(fabsf(s.x)), lg2_approx(fabsf(s.y))), bcast2(0.2f));
+        const float2 r = make_float2(ex2_approx(t.x), ex2_approx(t.y));
+        const float2 u = make_float2(copy_sign(r.x, s.x), copy_sign(r.y, s.y));
+        const float2 u2 = mul2(r, r);
+        p[0] = add2(p[0], u);
+        p[1] = add2(p[1], u2);
+        p[2] = fma2(u2, u, p[2]);
+        p[3] = fma2(u2, u2, p[3]);
+        p[4] = add2(p[4], s);
+    } else {
+        static_assert(K >= 6 && K <= 8, "orders 1..8");          // row f2: E_j += u E_(j-1), j = K..1
+        const float2 t = mul2(make_float2(lg2_approx(fabsf(s.x)), lg2_approx(fabsf(s.y))), bcast2(1.0f / (float)K));
+        const float2 r = make_float2(ex2_approx(t.x), ex2_approx(t.y));
+        const float2 u = make_float2(copy_sign(r.x, s.x), copy_sign(r.y, s.y));
+#pragma unroll
+        for (int j = K - 1; j >= 1; --j) p[j] = fma2(u, p[j - 1], p[j]);
+        p[0] = add2(p[0], u);
+    }
+}
+
+template <int K, int W>
+__device__ __forceinline__ void accumulate2_w(float2 s, float2 (&p)[kAcc<K, W>]) {
+    accumulate2<K>(s, reinterpret_cast<float2 (&)[K]>(p));
+    if constexpr (W == 1) {
+        p[K] = fma2(s, s, p[K]);
+        if constexpr ((K & 1) == 0) p[K + 1] = add2(p[K + 1], s);
+    }
+}
+
+// the pair's accumulator rows unpacked: half h (0 / 1) of p[0..kAcc) as the scalar row combine_w expects
+template <int K, int W>
+__device__ __forceinline__ float combine2_w(const float2 (&p)[kAcc<K, W>], int h, float inv_n) {
+    float q[kAcc<K, W>];
+#pragma unroll
+    for (int k = 0; k < kAcc<K, W>; ++k) q[k] = h == 0 ? p[k].x : p[k].y;
+    return combine_w<K, W>(q, inv_n);
+}
+
 // Step a2 + the index half of a3, once per (pixel, element), shared by every frame a thread carries.
 //   xs2, c0      the lateral offset xs = pixel - element (samples) enters only through its square, passed as
 //                xs2 = fl(xs_hi^2) and c0 = xs2 - xs^2 (the rounding error of the square plus the low part of xs),
@@ -194,6 +291,12 @@ template <bool INR>
 __device__ __forceinline__ float interp(const Tap& t, float s0, float s1) {
     if constexpr (INR) return fmaf(t.wa, s1 - s0, s0);
     else return fmaf(t.wa, s1, t.wb * s0);
+}
+// the same on two frames (packed)
+template <bool INR>
+__device__ __forceinline__ float2 interp2(const Tap& t, float2 s0, float2 s1) {
+    if constexpr (INR) return interp2(t.wa, s0, s1);
+    else return fma2(bcast2(t.wa), s1, mul2(bcast2(t.wb), s0));
 }
 
 }  // namespace pab

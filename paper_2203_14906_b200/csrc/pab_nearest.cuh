@@ -91,6 +91,26 @@ __device__ __forceinline__ void accumulate_rooted(float u, float (&p)[K]) {
     }
 }
 
+// the same on two frames (packed f32x2, pab_math.cuh)
+template <int K>
+__device__ __forceinline__ void accumulate_rooted2(float2 u, float2 (&p)[K]) {
+    p[0] = add2(p[0], u);
+    if constexpr (K >= 2) {
+        const float2 u2 = mul2(u, u);
+        p[1] = add2(p[1], u2);
+        if constexpr (K >= 3) p[2] = fma2(u2, u, p[2]);
+        if constexpr (K >= 4) p[3] = fma2(u2, u2, p[3]);
+        if constexpr (K >= 5) p[4] = fma2(mul2(u2, u2), u, p[4]);
+    }
+}
+template <int K>
+__device__ __forceinline__ float combine_half(const float2 (&p)[K], int h) {
+    float q[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) q[k] = h == 0 ? p[k].x : p[k].y;
+    return combine<K>(q);
+}
+
 // ------------------------------------------------------------------------------------------------------
 // Staged kernel: same tile, producer warp, bulk-copy ring and persistent tile loop as bf_staged_kernel; the
 // consumer's per-(pixel, element) work is one 16-bit table load, one address, and NQ 128-bit shared loads.
@@ -185,11 +205,11 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
         const int bx = tile % C.tiles_x, by = (tile / C.tiles_x) % C.tiles_z, bz = tile / (C.tiles_x * C.tiles_z);
         const int j = bx * kStgCols + col;
         const int m = by * kStgRows + (warp >> 3) * 32 + lane;
-        float p[NF][K];
+        float2 p[NF / 2][K];
 #pragma unroll
-        for (int f = 0; f < NF; ++f)
+        for (int f = 0; f < NF / 2; ++f)
 #pragma unroll
-            for (int k = 0; k < K; ++k) p[f][k] = 0.0f;
+            for (int k = 0; k < K; ++k) p[f][k] = make_float2(0.0f, 0.0f);
 
         for (int ck = 0; ck < n_chunks; ++ck) {
             const int nch = min(C.chunk, P.N - ck * C.chunk);
@@ -212,10 +232,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
                 for (int q = 0; q < NQ; ++q) {
                     float4 u = lds128(a + q * quad_bytes);
                     if constexpr (!INR) { if (!ok) u = make_float4(0.0f, 0.0f, 0.0f, 0.0f); }
-                    accumulate_rooted<K>(u.x, p[4 * q + 0]);
-                    accumulate_rooted<K>(u.y, p[4 * q + 1]);
-                    accumulate_rooted<K>(u.z, p[4 * q + 2]);
-                    accumulate_rooted<K>(u.w, p[4 * q + 3]);
+                    accumulate_rooted2<K>(make_float2(u.x, u.y), p[2 * q + 0]);
+                    accumulate_rooted2<K>(make_float2(u.z, u.w), p[2 * q + 1]);
                 }
             }
             __syncwarp();
@@ -228,7 +246,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
-                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine<K>(p[f]);
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine_half<K>(p[f / 2], f & 1);
             }
         }
     }

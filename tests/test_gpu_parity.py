@@ -142,15 +142,16 @@ def test_c2b_headline_batch_sampled_pixels(pab, orc, delay_cache):
     pix[:4] = [[0, 0], [g.nz - 1, g.nx - 1], [0, g.nx - 1], [g.nz - 1, 0]]
     ref = orc.beamform_pixels(w.rf, g, 3, pix)                      # [F][n_pix]
     got = gpu[:, pix[:, 0], pix[:, 1]]
-    # Full images of 8 of the 64 frames (one per octet the kernel carries in registers): relative L2 <= 1e-4 and
-    # the per-pixel bound.  Sampled pixels of all 64 frames: the per-pixel bound against the image peak.  (No L2
-    # on the sample: the error is heavy-tailed, largest on the few bright absorber pixels, so the rms of a
-    # 1500-pixel sample is not an estimate of the image's; measured full-image relative L2 is 1e-5 .. 7e-5.)
-    full_peak = 0.0
-    for f in (0, 9, 18, 27, 36, 45, 54, 63):
+    # Full images of ALL 64 frames: relative L2 <= 1e-4 and the per-pixel bound on every one (the oracle does a C2b
+    # frame in ~0.1 s on the GPU box's cores).  Sampled pixels of all 64 frames through the oracle's per-pixel entry
+    # point as well: the per-pixel bound against the image peak.  (No L2 on the sample: the error is heavy-tailed,
+    # largest on the few bright absorber pixels, so the rms of a 1500-pixel sample is not an estimate of the image's.)
+    full_peak, worst = 0.0, 0.0
+    for f in range(64):
         full = orc.beamform(w.rf[f:f + 1], g, 3)[0]
-        check_raw(gpu[f], full, 3)
+        worst = max(worst, check_raw(gpu[f], full, 3))
         full_peak = max(full_peak, float(np.max(np.abs(full))))
+    assert worst <= 2.5e-5, worst                         # the margin test_margin_on_fresh_seeds asks of other seeds
     assert np.max(np.abs(got - ref)) <= 1e-3 * full_peak
 
 
@@ -193,6 +194,73 @@ def test_post_chain_streaming_configs(pab, orc, cfg, frames):
         else:
             rel = np.sqrt(np.sum((gpu - ref) ** 2) / np.sum(ref ** 2))
             assert rel <= 2e-4, f"{cfg} {mode}: relative L2 {rel:.3e}"
+
+
+def _check_log(gpu, ref, dr):
+    sel = ref > -40.0
+    assert np.max(np.abs(gpu - ref)[sel]) <= 0.05
+    assert np.all(gpu <= 1e-4) and np.all(gpu >= -dr - 1e-4)
+    assert np.max(gpu) > -1e-3                                            # 0 dB at the frame max
+
+
+@pytest.mark.parametrize("delay_cache", ["all", "off"])
+def test_c5_defining_shape_64_frame_int16_batch(pab, orc, delay_cache):
+    """Config C5 as BASELINE.json states it: ONE 64-frame int16 batch at 768 x 192 pixels x 192 elements, order 3 with
+    band-pass + envelope + log (16-frame groups on the int16 ingest path: the launch configuration bench.py --sweep
+    times).  Frames 0 and 63 (first and last of the batch) in full against the oracle, before
+    the band-pass (north_star's bound) and after the whole post chain; cached taps and in-kernel delays."""
+    w = synth.make_config("C5", n_frames=64)
+    g = w.geom
+    assert w.rf.dtype == np.int16 and w.rf.shape == (64, 192, 3072)
+    post = dict(w.post)
+    raw, launches = run_gpu(pab, g, w.rf, 3, dtype="int16", delay_cache=delay_cache)
+    assert launches >= 2
+    out, _ = run_gpu(pab, g, w.rf, 3, dtype="int16", post=post, delay_cache=delay_cache)
+    for f in (0, 63):
+        ref = orc.beamform(w.rf[f:f + 1], g, 3)
+        check_raw(raw[f], ref[0], 3)
+        ref_log = orc.post(ref, g, post["f_center"], post["f_halfwidth"], post["n_taps_bp"], post["n_taps_hilbert"],
+                           post["dyn_range_db"], mode="log")[0]
+        _check_log(out[f], ref_log, post["dyn_range_db"])
+
+
+def test_c3_defining_shape_256_frame_call(pab, orc):
+    """Config C3 as stated: ONE call of 256 frames (512 x 128 pixels, order 3, post = log); frames 0, 63, 64, 255
+    (first / last of the 64-frame batches) in full, raw and after the post chain."""
+    w = synth.make_config("C3", n_frames=256)
+    g = w.geom
+    post = dict(w.post)
+    raw, _ = run_gpu(pab, g, w.rf, 3, delay_cache="all")
+    out, _ = run_gpu(pab, g, w.rf, 3, post=post, delay_cache="all")
+    for f in (0, 63, 64, 255):
+        ref = orc.beamform(w.rf[f:f + 1], g, 3)
+        check_raw(raw[f], ref[0], 3)
+        ref_log = orc.post(ref, g, post["f_center"], post["f_halfwidth"], post["n_taps_bp"], post["n_taps_hilbert"],
+                           post["dyn_range_db"], mode="log")[0]
+        _check_log(out[f], ref_log, post["dyn_range_db"])
+
+
+@pytest.mark.parametrize("delay_cache", ["all", "off"])
+@pytest.mark.parametrize("order", [4, 5])
+def test_c4_16_frame_batch(pab, orc, order, delay_cache):
+    """Config C4 in one 16-frame call (8 frames per thread at orders 4, 5: the sweep's batched rows): sampled whole
+    rows of frames 0, 7, 8 and 15 of the full-size image."""
+    w = synth.make_config("C4", n_frames=16)
+    g = w.geom
+    gpu, _ = run_gpu(pab, g, w.rf, order, delay_cache=delay_cache)
+    rng = np.random.default_rng(13)
+    rows = np.unique(np.concatenate([[0, g.nz - 1], rng.integers(0, g.nz, 22)]))
+    sub = synth.Geometry(g.n_elem, g.n_samp, g.fs, g.c, g.pitch, g.nx, 1, g.x0, g.dx, g.z0, g.dz)
+    frames = (0, 7, 8, 15)
+    ref = np.empty((len(frames), len(rows), g.nx))
+    for r, m in enumerate(rows):
+        sub.z0 = float(np.float64(g.z0) + m * np.float64(g.dz))
+        ref[:, r] = orc.beamform(w.rf[list(frames)], sub, order)[:, 0]
+    for k, f in enumerate(frames):
+        got = gpu[f][rows]
+        err = np.abs(got - ref[k])
+        assert np.sqrt(np.sum(err ** 2) / np.sum(ref[k] ** 2)) <= 1e-4, (order, f)
+        assert np.max(err) <= 5e-3 * np.max(np.abs(ref[k])), (order, f)
 
 
 @pytest.mark.parametrize("n_bp,n_h", [(31, 21), (64, 63), (50, 41), (96, 95)])
