@@ -13,6 +13,8 @@
 // that the table and the staged window agree exactly.
 #pragma once
 #include <cstdint>
+#include <cstdlib>
+#include <type_traits>
 #include <cuda_runtime.h>
 #include "pab_math.cuh"
 #include "pab_pipe.cuh"
@@ -67,7 +69,9 @@ __device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
 // per thread.  In-range geometries.
 // COMPACT: taps come from the (d, row) table through L1/L2 (q = pitch / dx), only the window starts are staged.
 // W = 1: coherence-factor weighting (row f1), frame groups with the tile-major table only (NQ = 1, 2; orders 4, 5: NQ = 1).
-template <int K, int NQ, bool COMPACT, int W = 0>
+// RM (root mix, order 3, 16 frames per thread): how many of a thread's 8 frame pairs take their cube root on the FMA
+// pipe (cbrt_fma2) instead of the XU pipe: 0, 1 (pair 7) or 2 (pairs 3 and 7).
+template <int K, int NQ, bool COMPACT, int W = 0, int RM = 0>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParams P, const StagedCfg C,
                                                                     const uint32_t* __restrict__ taps,
                                                                     const int* __restrict__ w0s,
@@ -85,6 +89,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
     const int quad_bytes = C.window * BPS;
     const int slot_bytes = quad_bytes * NCOPY;
     const int stage_bytes = C.chunk * slot_bytes;
+    const uint32_t ebuf = data0 + C.stages * stage_bytes;          // epilogue transpose buffer (C.epi)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_chunks = (P.N + C.chunk - 1) / C.chunk;
     const int n_tiles = C.tiles_x * C.tiles_z * C.groups;
@@ -111,7 +116,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
             const size_t blk0 = (size_t)txy * P.N;
             for (int ck = 0; ck < n_chunks; ++ck) {
                 const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
-                mbar_wait(empty, ph);
+                mbar_wait_relaxed(empty, ph);
                 const int ch = ck * C.chunk + lane;
                 if (ch < P.N) {
                     const int w0 = __ldg(w0s + blk0 + ch);
@@ -129,8 +134,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                     }
                     const char* src = grp + (size_t)ch * chan_stride + (size_t)w0 * BPS;
 #pragma unroll
-                    for (int q = 0; q < NCOPY; ++q)
-                        bulk_g2s(data0 + slot + q * quad_bytes, src + q * grp_stride, bytes, full);
+                    for (int c = 0; c < NCOPY; ++c)
+                        bulk_g2s(data0 + slot + c * quad_bytes, src + c * grp_stride, bytes, full);
                 } else {
                     mbar_arrive(full);
                 }
@@ -141,14 +146,15 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
     }
 
     const int col = warp & 7;
-    const uint32_t my = (uint32_t)((col * kStgRows + (warp >> 3) * 32 + lane) * 4);
+    const int trow = (warp >> 3) * 32 + lane;                        // this thread's row inside the tile
+    const uint32_t my = (uint32_t)((col * kStgRows + trow) * 4);
     int s = 0;
     uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int bz = tile % C.groups, txy = tile / C.groups;
         const int bx = txy % C.tiles_x, by = txy / C.tiles_x;
         const int j = bx * kStgCols + col;
-        const int m = by * kStgRows + (warp >> 3) * 32 + lane;
+        const int m = by * kStgRows + trow;
         // one frame per thread: scalar accumulators; frame groups: the frames in pairs, packed f32x2 arithmetic
         float p[1][kAcc<K, W>];
         float2 pp[NQ == 0 ? 1 : NF / 2][kAcc<K, W>];
@@ -187,13 +193,18 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                     const float s0 = lds32(addr), s1 = lds32(addr + 4);
                     accumulate_w<K, W>(fmaf(a, s1 - s0, s0), p[0]);
                 } else {
-#pragma unroll
-                    for (int q = 0; q < NQ; ++q) {
-                        const float4 s0 = lds128(addr + q * quad_bytes);
-                        const float4 s1 = lds128(addr + q * quad_bytes + 16);
-                        accumulate2_w<K, W>(interp2(a, make_float2(s0.x, s0.y), make_float2(s1.x, s1.y)), pp[2 * q + 0]);
-                        accumulate2_w<K, W>(interp2(a, make_float2(s0.z, s0.w), make_float2(s1.z, s1.w)), pp[2 * q + 1]);
-                    }
+                    // quad c of the group (compile-time c: which of its two frame pairs takes the FMA-pipe root)
+                    auto quad = [&](auto qc) {
+                        constexpr int c = decltype(qc)::value;
+                        const float4 s0 = lds128(addr + c * quad_bytes);
+                        const float4 s1 = lds128(addr + c * quad_bytes + 16);
+                        constexpr bool fma_root = K == 3 && NQ == 4 && W == 0 && ((RM == 2 && (c & 1)) || (RM == 1 && c == 3));
+                        accumulate2_w<K, W>(interp2(a, make_float2(s0.x, s0.y), make_float2(s1.x, s1.y)), pp[2 * c + 0]);
+                        accumulate2_w<K, W, fma_root>(interp2(a, make_float2(s0.z, s0.w), make_float2(s1.z, s1.w)), pp[2 * c + 1]);
+                    };
+                    quad(std::integral_constant<int, 0>{});
+                    if constexpr (NQ >= 2) quad(std::integral_constant<int, 1>{});
+                    if constexpr (NQ >= 4) { quad(std::integral_constant<int, 2>{}); quad(std::integral_constant<int, 3>{}); }
                 }
             }
             __syncwarp();
@@ -201,17 +212,23 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
             if (++s == C.stages) { s = 0; ph ^= 1; }
         }
 
-        if (j < P.nx && m < P.nz) {
-            const size_t img = (size_t)P.nz * P.nx;
+        const size_t img = (size_t)P.nz * P.nx;
+        if constexpr (NQ == 0) {
+            if (j < P.nx && m < P.nz && bz < P.n_frames) P.out[(size_t)bz * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[0], P.inv_n);
+        } else if (C.epi) {
+#pragma unroll
+            for (int c = 0; c < NQ; ++c) {
+                const float v[4] = {combine2_w<K, W>(pp[2 * c], 0, P.inv_n), combine2_w<K, W>(pp[2 * c], 1, P.inv_n),
+                                    combine2_w<K, W>(pp[2 * c + 1], 0, P.inv_n), combine2_w<K, W>(pp[2 * c + 1], 1, P.inv_n)};
+                const int frame0 = bz * NF + 4 * c;
+                store_quad_transposed(ebuf, v, warp, lane, trow, col, P.out + (size_t)frame0 * img, img,
+                                      min(4, P.n_frames - frame0), by * kStgRows, bx * kStgCols, P.nz, P.nx);
+            }
+        } else if (j < P.nx && m < P.nz) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
-                if (frame < P.n_frames) {
-                    float v;
-                    if constexpr (NQ == 0) v = combine_w<K, W>(p[0], P.inv_n);
-                    else v = combine2_w<K, W>(pp[f / 2], f & 1, P.inv_n);
-                    P.out[(size_t)frame * img + (size_t)m * P.nx + j] = v;
-                }
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine2_w<K, W>(pp[f / 2], f & 1, P.inv_n);
             }
         }
     }
@@ -221,7 +238,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 inline size_t cached_smem_bytes(const StagedCfg& c, int nq, bool compact) {
     const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
     const size_t blk = compact ? 4 : kCacheBlockBytes;
-    return 64 + (((size_t)c.stages * c.chunk * blk + 127) & ~(size_t)127) + (size_t)c.stages * c.chunk * (size_t)c.window * bps * ncopy;
+    return 64 + (((size_t)c.stages * c.chunk * blk + 127) & ~(size_t)127) + (size_t)c.stages * c.chunk * (size_t)c.window * bps * ncopy +
+           (c.epi ? kEpiBytes : 0);
 }
 template <int K, int NQ>
 inline cudaError_t cached_set_attr(int smem_optin) {
@@ -242,6 +260,7 @@ inline cudaError_t cached_set_attr_k(int smem_optin) {
         return cached_set_attr<K, 4>(smem_optin);
     } else return cudaSuccess;
 }
+constexpr int kRootMix = 1;          // order 3, 16 frames per thread: frame pairs rooted on the FMA pipe (measured best)
 inline cudaError_t cached_configure(int smem_optin) {
     cudaError_t e;
     if ((e = cached_set_attr_k<1>(smem_optin)) != cudaSuccess) return e;
@@ -249,18 +268,29 @@ inline cudaError_t cached_configure(int smem_optin) {
     if ((e = cached_set_attr_k<3>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr_k<4>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr_k<5>(smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<3, 4, false, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<3, 4, false, 0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
     // orders 6..8 (row f2): 4-frame groups with the tile-major table only
     if ((e = cudaFuncSetAttribute(bf_cached_kernel<6, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(bf_cached_kernel<7, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(bf_cached_kernel<8, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
+template <int K, int NQ, bool COMPACT, int W = 0, int RM = 0>
+inline void launch_cached_rm(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    const size_t smem = cached_smem_bytes(c, NQ, COMPACT);
+    const int per_sm = resident_per_sm(bf_cached_kernel<K, NQ, COMPACT, W, RM>, kStgThreads, smem);
+    const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
+    bf_cached_kernel<K, NQ, COMPACT, W, RM><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
+        P, c, T.taps, T.w0s, T.compact, T.q);
+}
 template <int K, int NQ, bool COMPACT, int W = 0>
 inline void launch_cached_kc(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
-    const size_t smem = cached_smem_bytes(c, NQ, COMPACT);
-    const int per_sm = resident_per_sm(bf_cached_kernel<K, NQ, COMPACT, W>, kStgThreads, smem);
-    const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
-    bf_cached_kernel<K, NQ, COMPACT, W><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
-        P, c, T.taps, T.w0s, T.compact, T.q);
+    if constexpr (K == 3 && NQ == 4 && !COMPACT && W == 0) {
+        static const int rm = [] { const char* e = getenv("PAB_ROOT_MIX"); return e ? atoi(e) : kRootMix; }();   // tuning knob
+        if (rm == 1) { launch_cached_rm<K, NQ, COMPACT, W, 1>(P, c, T, sm_count, st); return; }
+        if (rm == 2) { launch_cached_rm<K, NQ, COMPACT, W, 2>(P, c, T, sm_count, st); return; }
+    }
+    launch_cached_rm<K, NQ, COMPACT, W, 0>(P, c, T, sm_count, st);
 }
 template <int K, int NQ>
 inline void launch_cached_k(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
@@ -294,13 +324,7 @@ inline bool cached_weight_ok(int order, int nq, bool compact) {
 inline void launch_cached(int order, int nq, int weight, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
                           int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (T.compact ? 4 : kCacheBlockBytes);
-    long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
-    if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
-    if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
-    if (chunk > P.N) chunk = P.N;
-    if (chunk < 1) chunk = 1;
-    StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
-                (P.nz + kStgRows - 1) / kStgRows, groups};
+    const StagedCfg c = make_cfg(slot, plan.stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups);
     switch (order) {
     case 1: launch_cached_nq<1>(nq, weight, P, c, T, sm_count, st); break;
     case 2: launch_cached_nq<2>(nq, weight, P, c, T, sm_count, st); break;

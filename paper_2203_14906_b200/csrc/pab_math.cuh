@@ -18,6 +18,13 @@ __device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.appro
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+// The same MUFU operations as volatile statements: ptxas keeps volatile asm statements in program order, which is how
+// accumulate_batch pins its stage structure (otherwise the scheduler pulls every consumer up behind its MUFU).
+__device__ __forceinline__ float lg2_pinned(float x) { float y; asm volatile("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float ex2_pinned(float x) { float y; asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sqrt_pinned(float x) { float y; asm volatile("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_pinned(float x) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 // copysign(|r|, s) as one LOP3: (r & 0x7fffffff) | (s & 0x80000000)
 __device__ __forceinline__ float copy_sign(float r, float s) {
     return __uint_as_float((__float_as_uint(r) & 0x7fffffffu) | (__float_as_uint(s) & 0x80000000u));
@@ -153,11 +160,34 @@ __device__ __forceinline__ float2 bcast2(float a) { return make_float2(a, a); }
 // a3 for an in-range tap: s = s0 + a (s1 - s0) on two frames
 __device__ __forceinline__ float2 interp2(float a, float2 s0, float2 s1) { return fma2(bcast2(a), sub2(s1, s0), s0); }
 
+// Signed cube root of two samples on the FMA and ALU pipes only (no MUFU), so that a fraction of a thread's frames can
+// take their root beside the XU pipe instead of queueing for it ("move a fraction of cube roots to a
+// division-free Newton iteration for x^(-1/k) on the FMA pipe to balance the two pipes").  y ~ |s|^(-1/3): integer seed
+// (magic - bits / 3, residual 1 - |s| y^3 within 0.103), one third-order step y (1 + e/3 + 2 e^2/9), one Newton step
+// y (1 + e/3); u = (s y) y carries the sign of s.  Relative error <= 3.8e-7 over 1e-30 .. 1e30 (the lg2/ex2 pair:
+// 5e-7 .. 2.7e-6); s = 0 gives 0 (y stays finite).
+__device__ __forceinline__ float2 cbrt_fma2(float2 s) {
+    const float2 x = make_float2(fabsf(s.x), fabsf(s.y));
+    float2 y = make_float2(__uint_as_float(0x54a20000u - __umulhi(__float_as_uint(x.x), 0x55555556u)),
+                           __uint_as_float(0x54a20000u - __umulhi(__float_as_uint(x.y), 0x55555556u)));
+    float2 e = fma2(mul2(x, y), mul2(y, y), bcast2(-1.0f));                  // -(residual) = |s| y^3 - 1
+    y = mul2(y, fma2(fma2(e, bcast2(2.0f / 9.0f), bcast2(-1.0f / 3.0f)), e, bcast2(1.0f)));
+    e = fma2(mul2(x, y), mul2(y, y), bcast2(-1.0f));
+    y = fma2(mul2(y, e), bcast2(-1.0f / 3.0f), y);
+    return mul2(mul2(s, y), y);
+}
+
 // a4 + a5 on two frames: p[m] holds the pair's p_(m+1).  The even powers need no sign, so they are formed from the
 // unsigned root r; p_K = sum s (odd K) is accumulated from s itself; for even K, |s| = r^K to 2^-22 relative.
-template <int K>
+// FMA_ROOT (order 3 only): the root of this pair is taken on the FMA pipe (cbrt_fma2) instead of MUFU lg2 + ex2.
+template <int K, bool FMA_ROOT = false>
 __device__ __forceinline__ void accumulate2(float2 s, float2 (&p)[K]) {
-    if constexpr (K == 1) {
+    if constexpr (K == 3 && FMA_ROOT) {
+        const float2 u = cbrt_fma2(s);
+        p[0] = add2(p[0], u);
+        p[1] = fma2(u, u, p[1]);
+        p[2] = add2(p[2], s);
+    } else if constexpr (K == 1) {
         p[0] = add2(p[0], s);
     } else if constexpr (K == 2) {
         const float2 r = make_float2(sqrt_approx(fabsf(s.x)), sqrt_approx(fabsf(s.y)));
@@ -198,12 +228,80 @@ __device__ __forceinline__ void accumulate2(float2 s, float2 (&p)[K]) {
     }
 }
 
-template <int K, int W>
+template <int K, int W, bool FMA_ROOT = false>
 __device__ __forceinline__ void accumulate2_w(float2 s, float2 (&p)[kAcc<K, W>]) {
-    accumulate2<K>(s, reinterpret_cast<float2 (&)[K]>(p));
+    accumulate2<K, FMA_ROOT>(s, reinterpret_cast<float2 (&)[K]>(p));
     if constexpr (W == 1) {
         p[K] = fma2(s, s, p[K]);
         if constexpr ((K & 1) == 0) p[K + 1] = add2(p[K + 1], s);
+    }
+}
+
+// a4 + a5 for the NP frame pairs a thread carries, stage by stage over all pairs: every first-stage MUFU of the tap,
+// then the scalings, then every second-stage MUFU, then the sign copies and the power-sum updates.  A warp issues in
+// order and stalls at the first instruction whose operand is not back yet; the XU pipe serves a warp's MUFU in 8 clocks
+// and is shared by the scheduler's warps, so a result returns tens to hundreds of clocks after issue.  Pair by pair
+// (accumulate2) the consumer sits a few instructions behind its MUFU and every warp keeps draining the XU queue and
+// waiting for it; stage by stage the consumer of MUFU j sits NP - 1 MUFU pairs behind it and the queue stays fed.
+// FM: bit j set = pair j takes its root on the FMA pipe (order 3 only, cbrt_fma2).
+template <int K, int W, int NP, unsigned FM = 0u>
+__device__ __forceinline__ void accumulate_batch(const float2 (&s)[NP], float2 (&p)[NP][kAcc<K, W>]) {
+    if constexpr (K == 1) {
+#pragma unroll
+        for (int j = 0; j < NP; ++j) accumulate2_w<K, W>(s[j], p[j]);
+    } else {
+        float2 r[NP];
+        constexpr bool kLog = K == 3 || K >= 5;             // lg2 -> x 1/K -> ex2; else sqrt (K = 2) or rsqrt twice (K = 4)
+#pragma unroll
+        for (int j = 0; j < NP; ++j) {
+            if ((FM >> j) & 1u) continue;
+            if constexpr (kLog) r[j] = make_float2(lg2_pinned(fabsf(s[j].x)), lg2_pinned(fabsf(s[j].y)));
+            else if constexpr (K == 2) r[j] = make_float2(sqrt_pinned(fabsf(s[j].x)), sqrt_pinned(fabsf(s[j].y)));
+            else r[j] = make_float2(rsqrt_pinned(fabsf(s[j].x)), rsqrt_pinned(fabsf(s[j].y)));
+        }
+        if constexpr (kLog) {
+#pragma unroll
+            for (int j = 0; j < NP; ++j)
+                if (!((FM >> j) & 1u)) r[j] = mul2(r[j], bcast2(1.0f / (float)K));
+        }
+        if constexpr (K != 2) {
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+                if ((FM >> j) & 1u) continue;
+                if constexpr (kLog) r[j] = make_float2(ex2_pinned(r[j].x), ex2_pinned(r[j].y));
+                else r[j] = make_float2(rsqrt_pinned(r[j].x), rsqrt_pinned(r[j].y));
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NP; ++j) {
+            float2 u;
+            if ((FM >> j) & 1u) { u = cbrt_fma2(s[j]); r[j] = u; }           // r only enters through r^2 below
+            else u = make_float2(copy_sign(r[j].x, s[j].x), copy_sign(r[j].y, s[j].y));
+            float2 (&q)[kAcc<K, W>] = p[j];
+            if constexpr (K == 2) {
+                q[0] = add2(q[0], u);
+                q[1] = fma2(r[j], r[j], q[1]);
+            } else if constexpr (K == 3) {
+                q[0] = add2(q[0], u);
+                q[1] = fma2(r[j], r[j], q[1]);
+                q[2] = add2(q[2], s[j]);
+            } else if constexpr (K == 4 || K == 5) {
+                const float2 u2 = mul2(r[j], r[j]);
+                q[0] = add2(q[0], u);
+                q[1] = add2(q[1], u2);
+                q[2] = fma2(u2, u, q[2]);
+                q[3] = fma2(u2, u2, q[3]);
+                if constexpr (K == 5) q[4] = add2(q[4], s[j]);
+            } else {
+#pragma unroll
+                for (int m = K - 1; m >= 1; --m) q[m] = fma2(u, q[m - 1], q[m]);
+                q[0] = add2(q[0], u);
+            }
+            if constexpr (W == 1) {
+                q[K] = fma2(s[j], s[j], q[K]);
+                if constexpr ((K & 1) == 0) q[K + 1] = add2(q[K + 1], s[j]);
+            }
+        }
     }
 }
 

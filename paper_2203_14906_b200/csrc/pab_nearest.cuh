@@ -131,6 +131,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
     const int slot_bytes = quad_bytes * NQ;
     const int stage_bytes = C.chunk * slot_bytes;
     const uint32_t bar0 = smem_u32(bars);
+    const uint32_t ebuf = data0 + C.stages * stage_bytes;          // epilogue transpose buffer (C.epi)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_chunks = (P.N + C.chunk - 1) / C.chunk;
     const int n_tiles = C.tiles_x * C.tiles_z * C.groups;
@@ -160,7 +161,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
             const char* tblk = reinterpret_cast<const char*>(table) + ((size_t)by * C.tiles_x + bx) * (size_t)P.N * kNearBlockBytes;
             for (int ck = 0; ck < n_chunks; ++ck) {
                 const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
-                mbar_wait(empty, ph);
+                mbar_wait_relaxed(empty, ph);
                 const int ch = ck * C.chunk + lane;
                 if (ch < P.N) {
                     const float2 xe = __ldg(P.xe + ch);
@@ -241,8 +242,17 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_nearest_staged_kernel(const
             if (++s == C.stages) { s = 0; ph ^= 1; }
         }
 
-        if (j < P.nx && m < P.nz) {
-            const size_t img = (size_t)P.nz * P.nx;
+        const size_t img = (size_t)P.nz * P.nx;
+        if (C.epi) {
+#pragma unroll
+            for (int c = 0; c < NQ; ++c) {
+                const float v[4] = {combine_half<K>(p[2 * c], 0), combine_half<K>(p[2 * c], 1), combine_half<K>(p[2 * c + 1], 0),
+                                    combine_half<K>(p[2 * c + 1], 1)};
+                const int frame0 = bz * NF + 4 * c;
+                store_quad_transposed(ebuf, v, warp, lane, (warp >> 3) * 32 + lane, col, P.out + (size_t)frame0 * img, img,
+                                      min(4, P.n_frames - frame0), by * kStgRows, bx * kStgCols, P.nz, P.nx);
+            }
+        } else if (j < P.nx && m < P.nz) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
@@ -301,7 +311,7 @@ __global__ void __launch_bounds__(256) bf_nearest_direct_kernel(const BfParams P
 template <int K, int NQ, bool INR>
 inline void launch_nearest_staged_k(const BfParams& P, const StagedCfg& c, const unsigned short* table, int sm_count,
                                     int smem_optin, cudaStream_t st) {
-    const size_t smem = staged_smem_bytes(c, NQ) + (size_t)c.stages * c.chunk * kNearBlockBytes;
+    const size_t smem = staged_smem_bytes(c, NQ) + (size_t)c.stages * c.chunk * kNearBlockBytes;      // includes the epilogue buffer
     (void)smem_optin;
     const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups;
     bf_nearest_staged_kernel<K, NQ, INR><<<(unsigned)(tiles < sm_count ? tiles : sm_count), kStgThreads, smem, st>>>(P, c, table);
@@ -362,13 +372,7 @@ inline void launch_nearest_staged(int order, int nq, bool in_range, const BfPara
     // channels measured 4 % faster than three shallower ones (stages = 0: that default)
     if (stages <= 0) stages = 2;
     const long long slot = (long long)plan.window_samples * 16 * nq + (long long)sizeof(ChanEntry) + kNearBlockBytes;
-    long long chunk = (smem_limit - 64 - 128) / (stages * slot);
-    if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
-    if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
-    if (chunk > P.N) chunk = P.N;
-    if (chunk < 1) chunk = 1;
-    StagedCfg c{(int)chunk, stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
-                (P.nz + kStgRows - 1) / kStgRows, groups};
+    const StagedCfg c = make_cfg(slot, stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups);
     if (in_range) launch_nearest_staged_inr<true>(order, nq, P, c, table, sm_count, smem_limit, st);
     else launch_nearest_staged_inr<false>(order, nq, P, c, table, sm_count, smem_limit, st);
 }

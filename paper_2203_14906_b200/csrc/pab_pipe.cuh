@@ -45,6 +45,22 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// The producer's wait on an empty slot: it runs stages ahead of the consumers, so it can afford to sleep between
+// polls instead of spinning on try_wait (a spinning producer warp takes issue and MIO slots from the four consumer
+// warps of its scheduler, and every consumer warp of the CTA is coupled to the slowest one through the ring).
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "WAIT_%=:\n"
+        "nanosleep.u32 256;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
@@ -60,12 +76,44 @@ __device__ __forceinline__ float lds32(uint32_t addr) {
     return v;
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Tile epilogue of the frame-group kernels.  A consumer warp holds one column and 32 rows of the tile (lanes along
+// depth), so a direct store puts every lane in a different 32-byte sector of the image: 32 sectors per warp store,
+// 8192 partial-sector writes per tile and frame group of 16, which the SM's store path takes one per clock (5 % of
+// the kernel at C2b, all of it with the XU pipe idle because every warp of the CTA is there together).  Instead the
+// 4 frames of a quad go through a 64 x 8 x 4 transpose buffer in shared memory and leave as whole 32-byte row
+// segments: 4 sectors per warp store.
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void consumer_barrier() {
+    asm volatile("bar.sync 1, %0;" ::"n"(kStgConsumerWarps * 32) : "memory");
+}
+// v[f]: this thread's pixel (tile row `row`, tile column `col`) of the quad's 4 frames.  out0 = image of the quad's
+// first frame; n_valid = how many of the 4 frames exist.  Every consumer thread of the CTA must call it.
+__device__ __forceinline__ void store_quad_transposed(uint32_t ebuf, const float (&v)[4], int warp, int lane, int row, int col,
+                                                      float* out0, size_t img, int n_valid, int m0, int j0, int nz, int nx) {
+#pragma unroll
+    for (int f = 0; f < 4; ++f)
+        asm volatile("st.shared.f32 [%0], %1;" ::"r"(ebuf + (uint32_t)(((f * kStgRows + row) * kEpiRowFloats + col) * 4)), "f"(v[f]) : "memory");
+    consumer_barrier();
+    const int f = warp >> 2, c = lane & 7;
+    if (f < n_valid && j0 + c < nx) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int r = (warp & 3) * 16 + i * 4 + (lane >> 3);
+            float x;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(ebuf + (uint32_t)(((f * kStgRows + r) * kEpiRowFloats + c) * 4)));
+            if (m0 + r < nz) out0[(size_t)f * img + (size_t)(m0 + r) * nx + (j0 + c)] = x;
+        }
+    }
+    consumer_barrier();                 // the buffer is free for the next quad
+}
+
 // Shared-memory bytes of one launch: the plan's chunk is sized for `frames_per_thread / 4` quads per channel;
 // with fewer bytes per sample the same chunk fits with room to spare.
 inline size_t staged_smem_bytes(const StagedCfg& c, int nq) {
     const int bps = nq == 0 ? 4 : 16, ncopy = nq == 0 ? 1 : nq;
     const size_t tab = ((size_t)c.stages * c.chunk * sizeof(ChanEntry) + 127) & ~(size_t)127;
-    return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy;
+    return 64 + tab + (size_t)c.stages * c.chunk * c.window * bps * ncopy + (c.epi ? kEpiBytes : 0);
 }
 
 // Resident CTAs per SM of a kernel instantiation at a given dynamic shared-memory size, asked of the runtime once per
@@ -87,6 +135,28 @@ inline int resident_per_sm(Kernel kernel, int threads, size_t smem) {
     }
     memo.fn = fn; memo.dev = dev; memo.smem = smem; memo.per_sm = per_sm;
     return per_sm;
+}
+
+// Channels per stage for a launch whose channel slot is `slot` bytes, and whether the epilogue buffer fits beside the
+// ring: the buffer is taken when at least two channels per stage still fit with it (frame groups only).
+inline StagedCfg make_cfg(long long slot, int stages, int window, int nq, int chunk_cap, int smem_limit, const BfParams& P, int groups) {
+    auto fit = [&](long long avail) {
+        long long ch = avail / (stages * slot);
+        if (ch > kStagedMaxChunk) ch = kStagedMaxChunk;
+        if (chunk_cap > 0 && ch > chunk_cap) ch = chunk_cap;
+        if (ch > P.N) ch = P.N;
+        return ch;
+    };
+    const long long avail = smem_limit - 64 - 128;
+    long long chunk = fit(avail);
+    int epi = 0;
+    if (nq > 0) {
+        const long long ce = fit(avail - kEpiBytes);
+        if (ce >= 2 || ce == chunk) { chunk = ce; epi = 1; }
+    }
+    if (chunk > 2 && (chunk & 1) && chunk < P.N) --chunk;      // even: the element loop is unrolled by two
+    if (chunk < 1) chunk = 1;
+    return StagedCfg{(int)chunk, stages, window, (P.nx + kStgCols - 1) / kStgCols, (P.nz + kStgRows - 1) / kStgRows, groups, epi};
 }
 
 }  // namespace pab

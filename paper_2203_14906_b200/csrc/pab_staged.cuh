@@ -34,6 +34,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
     const int slot_bytes = quad_bytes * NCOPY;
     const int stage_bytes = C.chunk * slot_bytes;
     const uint32_t bar0 = smem_u32(bars);
+    const uint32_t ebuf = data0 + C.stages * stage_bytes;          // epilogue transpose buffer (C.epi)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_chunks = (P.N + C.chunk - 1) / C.chunk;
@@ -67,7 +68,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
             const char* grp = reinterpret_cast<const char*>(P.rf) + (size_t)bz * (NQ == 0 ? 1 : NQ) * grp_stride;
             for (int ck = 0; ck < n_chunks; ++ck) {
                 const uint32_t full = bar0 + 8 * s, empty = bar0 + 8 * (C.stages + s);
-                mbar_wait(empty, ph);
+                mbar_wait_relaxed(empty, ph);
                 const int ch = ck * C.chunk + lane;
                 if (ch < P.N) {
                     const float2 xe = __ldg(P.xe + ch);
@@ -171,17 +172,23 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
             if (++s == C.stages) { s = 0; ph ^= 1; }
         }
 
-        if (j < P.nx && m < P.nz) {
-            const size_t img = (size_t)P.nz * P.nx;
+        const size_t img = (size_t)P.nz * P.nx;
+        if constexpr (NQ == 0) {
+            if (j < P.nx && m < P.nz && bz < P.n_frames) P.out[(size_t)bz * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[0], P.inv_n);
+        } else if (C.epi) {
+#pragma unroll
+            for (int c = 0; c < NQ; ++c) {
+                const float v[4] = {combine2_w<K, W>(pp[2 * c], 0, P.inv_n), combine2_w<K, W>(pp[2 * c], 1, P.inv_n),
+                                    combine2_w<K, W>(pp[2 * c + 1], 0, P.inv_n), combine2_w<K, W>(pp[2 * c + 1], 1, P.inv_n)};
+                const int frame0 = bz * NF + 4 * c;
+                store_quad_transposed(ebuf, v, warp, lane, (warp >> 3) * 32 + lane, col, P.out + (size_t)frame0 * img, img,
+                                      min(4, P.n_frames - frame0), by * kStgRows, bx * kStgCols, P.nz, P.nx);
+            }
+        } else if (j < P.nx && m < P.nz) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
-                if (frame < P.n_frames) {
-                    float v;
-                    if constexpr (NQ == 0) v = combine_w<K, W>(p[0], P.inv_n);
-                    else v = combine2_w<K, W>(pp[f / 2], f & 1, P.inv_n);
-                    P.out[(size_t)frame * img + (size_t)m * P.nx + j] = v;
-                }
+                if (frame < P.n_frames) P.out[(size_t)frame * img + (size_t)m * P.nx + j] = combine2_w<K, W>(pp[f / 2], f & 1, P.inv_n);
             }
         }
     }
@@ -259,13 +266,7 @@ inline void launch_staged_t(int order, int nq, int weight, const BfParams& P, in
                             int chunk_cap, int smem_limit, int sm_count, cudaStream_t st) {
     // the plan's chunk is sized for frames_per_thread / 4 quads per channel; fewer quads -> more channels per stage
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (long long)sizeof(ChanEntry);
-    long long chunk = (smem_limit - 64 - 128) / (plan.stages * slot);
-    if (chunk > kStagedMaxChunk) chunk = kStagedMaxChunk;
-    if (chunk_cap > 0 && chunk > chunk_cap) chunk = chunk_cap;
-    if (chunk > P.N) chunk = P.N;
-    if (chunk < 1) chunk = 1;       // cannot happen: the plan fitted >= 1 channel at the largest nq
-    StagedCfg c{(int)chunk, plan.stages, plan.window_samples, (P.nx + kStgCols - 1) / kStgCols,
-                (P.nz + kStgRows - 1) / kStgRows, groups};
+    const StagedCfg c = make_cfg(slot, plan.stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups);
     launch_staged_inr<INR>(order, nq, weight, P, c, sm_count, st);
 }
 

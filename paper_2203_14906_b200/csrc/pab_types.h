@@ -38,12 +38,16 @@ constexpr int kDirectRows = 32;
 constexpr int kStgRows = 64, kStgCols = 8, kStgConsumerWarps = 16;
 constexpr int kStgThreads = (kStgConsumerWarps + 1) * 32;
 constexpr int kStgMaxStages = 4;
+// epilogue buffer of the frame-group kernels: one quad of frames of a tile, rows padded to 9 floats (conflict-free)
+constexpr int kEpiRowFloats = kStgCols + 1;
+constexpr int kEpiBytes = 4 * kStgRows * kEpiRowFloats * 4;
 
 struct StagedCfg {
     int chunk;          // channels per stage (<= 32)
     int stages;         // ring depth
     int window;         // samples per channel slot per quad (multiple of 4)
     int tiles_x, tiles_z, groups;   // tile grid: columns / 8, rows / 64, frame groups; tile t = (t % tiles_x, ...)
+    int epi;            // 1: the tile's images leave through the shared-memory transpose buffer (coalesced stores)
 };
 
 // cached interpolation taps (pab_cache.cuh)
