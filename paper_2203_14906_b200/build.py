@@ -26,6 +26,7 @@ UNITS = {
     "pab_tu_staged.cu": _KERNEL + ["pab_staged.cuh"],
     "pab_tu_staged_gen.cu": _KERNEL + ["pab_staged.cuh"],
     "pab_tu_cached.cu": _KERNEL + ["pab_cache.cuh"],
+    "pab_tu_diag.cu": _KERNEL + ["pab_diag.cuh"],
     "pab_tu_nearest.cu": _KERNEL + ["pab_nearest.cuh"],
     "pab_tu_post.cu": _KERNEL + ["pab_post.cuh", "pab_metrics.cuh"],
     "pab_tu_peaks.cu": [os.path.join("..", "..", "include", "pab.h")],

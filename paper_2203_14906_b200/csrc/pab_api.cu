@@ -34,6 +34,7 @@ struct pab_ctx {
     int* d_w0s = nullptr;                // window start of every (tile, element)
     uint2* d_compact = nullptr;          // (d, row) tap table when pitch = q dx exactly (translation invariance)
     int cache_q = 0;
+    DiagSet diag[2];                     // single-frame diagonal kernel: [0] orders 1..3 (16 pixels per thread), [1] orders 4, 5 (8)
     void* d_metric = nullptr;            // MetricAcc + double[1] + 2 x 4096 histogram bins (row f3), lazy
     unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
@@ -81,6 +82,7 @@ size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
 void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
     cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact);
+    xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]);
     for (int b = 0; b < 2; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -283,6 +285,16 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
                 return cuda_fail(ctx, e, "delay cache");
             }
         }
+    }
+    // translation-invariant geometries: calls of 1..3 frames take the diagonal kernel (pab_diag.cuh), which shares one
+    // tap among the 16 (8 for orders 4, 5) pairs of a diagonal and reads the caller's frame in place
+    if (mode != PAB_CACHE_OFF && ctx->d_compact && ctx->diag[0].smem_bytes == 0 && ctx->diag[1].smem_bytes == 0) {
+        PAB_CUDA(ctx, xl_diag_configure(ctx->smem_optin));
+        cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q,
+                                      (getenv("PAB_DIAG_NPG") && atoi(getenv("PAB_DIAG_NPG")) == 2) ? 2 : 4, 3, ctx->smem_optin, &ctx->diag[0]);
+        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, &ctx->diag[1]);
+        if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
+        ctx->launches += 4;
     }
     ctx->cache_mode = mode;
     return PAB_OK;

@@ -25,6 +25,13 @@ void xl_cached(int order, int nq, int weight, const BfParams& P, int groups, con
 void xl_build_delay_cache(const CacheGeom& G, int tiles_z, uint32_t* taps, int* w0s);
 void xl_build_delay_compact(const CacheGeom& G, int q, int nd, uint2* compact);
 
+// ---- pab_tu_diag.cu: single frames on translation-invariant geometries ----
+cudaError_t xl_diag_configure(int smem_optin);
+cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, int q, int npg, int max_order, int smem_limit, DiagSet* D);
+void xl_diag_free(DiagSet* D);
+void xl_diag(int order, int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
+             cudaStream_t st);
+
 // ---- pab_tu_nearest.cu: row f4 ----
 cudaError_t xl_nearest_configure(int smem_optin);
 bool xl_nearest_table(const NearestGeom& G, unsigned short* table);      // false: grid too large

@@ -138,7 +138,7 @@ inline int resident_per_sm(Kernel kernel, int threads, size_t smem) {
 }
 
 // Channels per stage for a launch whose channel slot is `slot` bytes, and whether the epilogue buffer fits beside the
-// ring: the buffer is taken when at least two channels per stage still fit with it (frame groups only).
+// ring: the buffer is taken when at least two channels per stage still fit with it (groups of 8 and 16 frames only).
 inline StagedCfg make_cfg(long long slot, int stages, int window, int nq, int chunk_cap, int smem_limit, const BfParams& P, int groups) {
     auto fit = [&](long long avail) {
         long long ch = avail / (stages * slot);
@@ -150,7 +150,7 @@ inline StagedCfg make_cfg(long long slot, int stages, int window, int nq, int ch
     const long long avail = smem_limit - 64 - 128;
     long long chunk = fit(avail);
     int epi = 0;
-    if (nq > 0) {
+    if (nq > 1) {            // 4-frame groups keep the direct stores: two block barriers per quad cost them more
         const long long ce = fit(avail - kEpiBytes);
         if (ce >= 2 || ce == chunk) { chunk = ce; epi = 1; }
     }

@@ -57,6 +57,11 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             q0 += groups * g;
             nq -= groups * g;
         }
+    } else if (F < 4 && ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
+               ctx->diag[order <= 3 ? 0 : 1].smem_bytes > 0) {
+        // translation-invariant geometry: the diagonal kernel, straight from the caller's frames (no ingest pass)
+        Span sp(ctx, PAB_STAGE_BEAMFORM, st);
+        xl_diag(order, ctx->dtype, ctx->diag[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
     } else if (F < 4) {
         const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
                             xl_cached_fits(ctx->plan, 0, ctx->d_compact != nullptr, ctx->smem_optin);

@@ -163,7 +163,12 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
                         const float4 s0 = lds128(a + q * quad_bytes);
                         const float4 s1 = lds128(a + q * quad_bytes + 16);
                         accumulate2_w<K, W>(interp2<INR>(t, make_float2(s0.x, s0.y), make_float2(s1.x, s1.y)), pp[2 * q + 0]);
-                        accumulate2_w<K, W>(interp2<INR>(t, make_float2(s0.z, s0.w), make_float2(s1.z, s1.w)), pp[2 * q + 1]);
+                        // order 3, 16 frames per thread: the last frame pair takes its cube root on the FMA pipe (cbrt_fma2),
+                        // which relieves the XU pipe (measured: pab_cache.cuh, kRootMix)
+                        if (K == 3 && NQ == 4 && W == 0 && q == 3)
+                            accumulate2_w<K, W, K == 3 && NQ == 4 && W == 0>(interp2<INR>(t, make_float2(s0.z, s0.w), make_float2(s1.z, s1.w)), pp[2 * q + 1]);
+                        else
+                            accumulate2_w<K, W>(interp2<INR>(t, make_float2(s0.z, s0.w), make_float2(s1.z, s1.w)), pp[2 * q + 1]);
                     }
                 }
             }

@@ -1,0 +1,163 @@
+// pab_tu_diag.cu -- translation unit: the single-frame "diagonal" beamforming kernel (pab_diag.cuh) and its tables.
+#include <algorithm>
+#include <cstdlib>
+#include <vector>
+#include "pab_diag.cuh"
+#include "pab_launch.h"
+
+namespace pab {
+
+namespace {
+
+// Split the G diagonal groups into `parts` consecutive ranges of nearly equal work.  The work of group g (eg = g - NPG)
+// is its number of live pixel groups (blocks with at least one pair on the array).  Returns the largest part's work.
+int split_parts(int G, int npg, int nq_real, int parts, int* lo) {
+    std::vector<int> w(G);
+    int total = 0;
+    for (int g = 0; g < G; ++g) {
+        const int eg = g - npg;
+        int n = 0;
+        for (int cg = 0; cg < npg; ++cg) n += (eg + cg + 1 >= 0 && eg + cg < nq_real) ? 1 : 0;
+        w[g] = n; total += n;
+    }
+    int best_cap = total;              // smallest cap such that a greedy left-to-right packing needs <= parts ranges
+    for (int cap = (total + parts - 1) / parts; cap <= total; ++cap) {
+        int used = 1, acc = 0;
+        bool ok = true;
+        for (int g = 0; g < G; ++g) {
+            if (w[g] > cap) { ok = false; break; }
+            if (acc + w[g] > cap) { ++used; acc = 0; }
+            acc += w[g];
+        }
+        if (ok && used <= parts) { best_cap = cap; break; }
+    }
+    int p = 0, acc = 0;
+    lo[0] = 0;
+    for (int g = 0; g < G; ++g) {
+        if (acc + w[g] > best_cap) { lo[++p] = g; acc = 0; }
+        acc += w[g];
+    }
+    while (p < parts) lo[++p] = G;
+    return best_cap;
+}
+
+template <int K, int NPG, typename T>
+void launch_diag_t(const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale, cudaStream_t st) {
+    dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, F);
+    const DiagTables tabs{D.taps, D.qw0, D.qoff};
+    bf_diag_kernel<K, NPG, T><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
+}
+template <int K, int NPG>
+void launch_diag_k(int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
+                   cudaStream_t st) {
+    if (dtype == PAB_I16) launch_diag_t<K, NPG, int16_t>(D, rf, out, F, N, S, nx, nz, scale, st);
+    else launch_diag_t<K, NPG, float>(D, rf, out, F, N, S, nx, nz, scale, st);
+}
+template <int K, int NPG>
+cudaError_t diag_attr(int smem_optin) {
+    cudaError_t e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+}
+
+}  // namespace
+
+cudaError_t xl_diag_configure(int smem_optin) {
+    cudaError_t e;
+    if ((e = diag_attr<1, 4>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<2, 4>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<3, 4>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<1, 2>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<2, 2>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<3, 2>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<4, 2>(smem_optin)) != cudaSuccess) return e;
+    return diag_attr<5, 2>(smem_optin);
+}
+
+void xl_diag_free(DiagSet* D) {
+    cudaFree(D->taps); cudaFree(D->qw0); cudaFree(D->qoff);
+    *D = DiagSet();
+}
+
+// Build the tables of one set (npg = 4: orders 1..3, npg = 2: orders 4, 5).  Leaves D->smem_bytes = 0 when the geometry
+// does not qualify (N not a multiple of 4, too many warps, a tile that does not fit in shared memory); returns a CUDA
+// error only for failed calls.  Synchronises the device.
+cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, int q, int npg, int max_order, int smem_limit,
+                          DiagSet* D) {
+    *D = DiagSet();
+    const int P = 4 * npg;
+    if (N % 4 != 0 || N < 4 || q < 1 || q > 8) return cudaSuccess;
+    // tuning knobs (environment, read when the tables are built): rows per tile and warps per CTA
+    auto knob = [](const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; };
+    DiagCfg cfg{};
+    cfg.q = q;
+    cfg.rows = knob("PAB_DIAG_ROWS", 32) == 16 ? 16 : 32;
+    const int lj = 32 / cfg.rows;
+    cfg.cp = (q % lj == 0 ? q : q * lj) * std::max(1, std::min(4, knob("PAB_DIAG_BLOCKS", 1)));      // lcm(q, lj) x column blocks per tile
+    cfg.wpp = cfg.cp / lj;
+    cfg.cols = P * cfg.cp;
+    cfg.tiles_x = (g.nx + cfg.cols - 1) / cfg.cols;
+    cfg.tiles_z = (g.nz + cfg.rows - 1) / cfg.rows;
+    cfg.quads = N / 4 + 2;
+    cfg.nd = cfg.tiles_x * cfg.cols + q * (N + P + 4);
+    if ((long long)cfg.nd * g.nz >= (1LL << 27) || cfg.wpp > kDiagMaxWarps) return cudaSuccess;
+    // warps per CTA = wpp * parts: near the target, the split of the diagonal groups with the least idle warp time
+    const int G = N / 4 + npg;
+    int best_parts = 0;
+    double best_cost = 1e30;
+    const int target = knob("PAB_DIAG_WARPS", 8);          // measured best at C2 and C4: 8 warps, two CTAs per SM
+    const int max_warps = kDiagMaxWarps;
+    const int max_parts = std::max(1, std::min(std::min(kDiagMaxParts, max_warps / cfg.wpp), target / cfg.wpp));
+    for (int parts = std::max(1, max_parts - 1); parts <= max_parts; ++parts) {
+        int lo[kDiagMaxParts + 1];
+        const double cost = (double)split_parts(G, npg, N / 4, parts, lo) * parts;        // warp slots of the CTA, idle ones included
+        if (cost <= best_cost) { best_cost = cost; best_parts = parts; }
+    }
+    if (best_parts == 0) return cudaSuccess;
+    cfg.parts = best_parts;
+    split_parts(G, npg, N / 4, cfg.parts, cfg.part_lo);
+
+    const DiagGeom geo{fs, c, (double)g.x0, (double)g.dx, (double)g.z0, (double)g.dz, N, S, g.nx, g.nz, q, P};
+    const size_t tiles = (size_t)cfg.tiles_x * cfg.tiles_z, nq = tiles * cfg.quads;
+    int* d_len = nullptr;
+    cudaError_t e;
+    if ((e = cudaMalloc(&D->taps, (size_t)cfg.nd * g.nz * sizeof(uint2))) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&D->qw0, nq * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
+    if ((e = cudaMalloc(&D->qoff, (nq + tiles) * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
+    if ((e = cudaMalloc(&d_len, nq * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
+    diag_taps_kernel<<<dim3((g.nz + 255) / 256, cfg.nd), 256>>>(geo, D->taps);
+    diag_window_kernel<<<dim3((unsigned)tiles, cfg.quads), 256>>>(geo, cfg.rows, cfg.cols, cfg.tiles_x, cfg.quads, D->qw0, d_len);
+    std::vector<int> len(nq), off(nq + tiles);
+    e = cudaMemcpy(len.data(), d_len, nq * sizeof(int), cudaMemcpyDeviceToHost);
+    cudaFree(d_len);
+    if (e != cudaSuccess) { xl_diag_free(D); return e; }
+    long long worst = 0;
+    for (size_t t = 0; t < tiles; ++t) {
+        long long o = 0;
+        for (int sq = 0; sq < cfg.quads; ++sq) { off[t * (cfg.quads + 1) + sq] = (int)o; o += (long long)len[t * cfg.quads + sq] * 16; }
+        off[t * (cfg.quads + 1) + cfg.quads] = (int)o;
+        worst = std::max(worst, o);
+    }
+    if ((e = cudaMemcpy(D->qoff, off.data(), off.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) { xl_diag_free(D); return e; }
+    const long long head = ((cfg.quads + 2 * (npg + 1)) * 4 + 127) & ~127;
+    const long long red = (long long)cfg.parts * cfg.wpp * P * max_order * 32 * 4;
+    const long long smem = head + std::max(worst, red);
+    if (smem > smem_limit) { xl_diag_free(D); return cudaSuccess; }          // a tile does not fit: the caller keeps its other kernels
+    D->cfg = cfg;
+    D->npg = npg;
+    D->smem_bytes = (int)smem;
+    return cudaDeviceSynchronize();
+}
+
+void xl_diag(int order, int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
+             cudaStream_t st) {
+    switch (order) {
+    case 1: D.npg == 4 ? launch_diag_k<1, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st) : launch_diag_k<1, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    case 2: D.npg == 4 ? launch_diag_k<2, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st) : launch_diag_k<2, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    case 3: D.npg == 4 ? launch_diag_k<3, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st) : launch_diag_k<3, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    case 4: launch_diag_k<4, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    default: launch_diag_k<5, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    }
+}
+
+}  // namespace pab

@@ -66,6 +66,39 @@ struct CacheTables {
     int q;                     // pitch / dx
 };
 
+// single-frame diagonal kernel (pab_diag.cuh)
+constexpr int kDiagMaxWarps = 16;
+constexpr int kDiagMaxParts = 16;
+
+struct DiagCfg {
+    int q;                  // pitch / dx
+    int rows;               // rows per tile = rows along a warp's lanes: 16 or 32; a warp holds 32 / rows column phases
+    int cp;                 // column phases per tile: lcm(q, 32 / rows); phase ph = residue ph % q of column block ph / q
+    int wpp;                // warps per diagonal part: cp / (32 / rows)
+    int parts;              // EP: diagonal parts; warps per CTA = wpp * parts
+    int cols;               // P cp: columns per tile
+    int tiles_x, tiles_z;
+    int quads;              // staged quads per tile: N / 4 + 2 (one zero quad on either side)
+    int nd;                 // columns of the tap table
+    int part_lo[kDiagMaxParts + 1];     // diagonal groups [part_lo[p], part_lo[p + 1]) of part p, as eg + P / 4 >= 0
+};
+
+struct DiagTables {
+    const uint2* taps;      // [nd][nz]: (floor(idx), fraction bits) of d = j - q i + q (N - 1 + P)
+    const int* qw0;         // [tiles][quads]     first staged sample of the quad's window
+    const int* qoff;        // [tiles][quads + 1] byte offset of the quad's window in the staging area (16-byte units x 16)
+};
+
+// one set of device tables of the diagonal kernel (P = 16 pixels per thread for orders 1..3, P = 8 for orders 4, 5)
+struct DiagSet {
+    DiagCfg cfg;
+    uint2* taps = nullptr;
+    int* qw0 = nullptr;
+    int* qoff = nullptr;
+    int npg = 0;            // pixel groups of 4 per thread
+    int smem_bytes = 0;     // dynamic shared memory per CTA; 0: not built / does not fit
+};
+
 // nearest-sample delays (pab_nearest.cuh)
 constexpr unsigned short kNearestInvalid = 0xFFFFu;
 constexpr int kNearBlockBytes = kStgRows * kStgCols * 2;      // one element's delay-table block for one tile

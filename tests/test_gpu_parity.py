@@ -286,9 +286,13 @@ def test_host_entry_point_matches_device_entry_point(pab):
         dev = bf.beamform(torch.from_numpy(w.rf).cuda(), 3)
         torch.cuda.synchronize()
         host = bf.beamform_host(w.rf, 3)
-        assert np.array_equal(dev.cpu().numpy(), host)
+        # the two entry points group the 21 frames differently (16 + 4 + 1 against 8 + 8 + 4 + 1), and in a 16-frame
+        # group one frame pair takes its cube root on the FMA pipe instead of the XU pipe: the
+        # same images to rounding, not to the bit
+        peak = float(np.max(np.abs(host)))
+        assert np.max(np.abs(dev.cpu().numpy() - host)) <= 2e-6 * peak
         pinned = torch.from_numpy(w.rf).pin_memory()
-        assert np.array_equal(bf.beamform_host(pinned, 3).numpy(), host)
+        assert np.array_equal(bf.beamform_host(pinned, 3).numpy(), host)          # same grouping: same bits
     finally:
         bf.close()
 
@@ -636,7 +640,7 @@ def test_more_frames_than_one_internal_batch(pab, orc):
         dev = bf.beamform(torch.from_numpy(w.rf).cuda(), 3)
         torch.cuda.synchronize()
         host = bf.beamform_host(w.rf, 3)
-        assert np.array_equal(dev.cpu().numpy(), host)
+        assert np.max(np.abs(dev.cpu().numpy() - host)) <= 2e-6 * float(np.max(np.abs(host)))     # 16- against 64-frame pieces
         for f in (0, 255, 256, 299):
             check_raw(host[f].astype(np.float64), orc.beamform(w.rf[f:f + 1], w.geom, 3)[0], 3)
     finally:
