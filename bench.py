@@ -48,6 +48,10 @@ METRIC = "beamformed frames/s, order-3 DMAS, 128ch (C2b: 128 el x 2048 samp x 10
 # 2 + 1/64 and 6 + 3/64: one square root and three FP32 slots per (pixel, element), shared by the 64 frames.)
 XU_PER_ITEM = 2.0
 FP32_PER_ITEM = 6.0
+# What the build issues per item (its SASS mix, profiles/r2_headline_sass.txt): two of a thread's 16 frames take their cube
+# root on the FMA pipe (pab_math.cuh cbrt_fma2), so 14/16 x 2 = 1.75 MUFU per item; the interpolation and the power sums
+# are packed f32x2 (one slot per two frames).  The roofline fraction keeps the algorithmic 2.0 in its numerator.
+XU_PER_ITEM_ISSUED = 1.75
 DELAY_CACHE = "all"
 SM_COUNT = 148
 NCU_TRAFFIC_BYTES = 185_511_680 + 51_419_136   # per 64-frame launch; profiles/r1_step_ncu_f.md
@@ -300,8 +304,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         t_fp32 = items_per_launch * FP32_PER_ITEM / fp32_peak
         t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
         achieved = items_per_launch * XU_PER_ITEM / (bf_launch_ms * 1e-3)
-        roofline = {"bound": "alu", "kernel": "bf_cached_kernel<3,4,false> (fused tap fetch + interpolation + root + power sums + Newton, 16 frames "
-                              "per thread, cached interpolation taps)",
+        roofline = {"bound": "alu", "kernel": "bf_cached_kernel<3,4,false,0,1> (fused tap fetch + interpolation + root + power sums + Newton, 16 "
+                              "frames per thread, cached interpolation taps, packed f32x2 arithmetic, 2 of 16 roots on the FMA pipe)",
                     "achieved": achieved / 1e9, "peak": xu_peak / 1e9, "unit": "Gop/s (XU/MUFU lane-ops)",
                     "frac": achieved / xu_peak, "frac_definition": "XU (MUFU) pipe term of T_roof (DESIGN.md reading B3)",
                     "frac_xu": t_xu / (bf_launch_ms * 1e-3),
@@ -317,6 +321,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                     "t_roof_ms": {"xu": t_xu * 1e3, "fp32": t_fp32 * 1e3, "hbm": t_hbm * 1e3},
                     "algorithmic_per_item": {"xu_ops": XU_PER_ITEM, "fp32_slots": FP32_PER_ITEM,
                                              "hbm_bytes": hbm_bytes / items_per_launch},
+                    "issued_per_item": {"xu_ops": XU_PER_ITEM_ISSUED,
+                                        "xu_pipe_busy": items_per_launch * XU_PER_ITEM_ISSUED / xu_peak / (bf_launch_ms * 1e-3),
+                                        "note": "2 of 16 cube roots per thread run on the FMA pipe; frac keeps the algorithmic 2.0"},
                     "items_per_s": items_per_launch / (bf_launch_ms * 1e-3),
                     "hbm_achieved_gbs": hbm_bytes / (bf_launch_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]}
         stages = {k: {"ms_per_step": v[0] / K, "launches_per_step": v[1] / K} for k, v in prof.items()}
@@ -386,6 +393,11 @@ def run_sweep(args):
               ("C2b", 64, (1, 2, 3), False, "cache-all"), ("C4", 16, (4, 5), False, "cache-all"),
               ("C2b", 64, (3,), False, "cf-cache-all"), ("C4", 16, (5,), False, "cf-cache-all"),
               ("C2b", 64, (6, 8), False, "cache-all")]
+    if args.case:                         # --case C2:1:cache-single[:3]  ->  one config / frame count / mode [/ order]
+        want = args.case.split(":")
+        cases = [c for c in cases if c[0] == want[0] and str(c[1]) == want[1] and c[4] == want[2]]
+        if len(want) > 3:
+            cases = [(c[0], c[1], (int(want[3]),), c[3], c[4]) for c in cases]
     for cfg, F, orders, post, weight in cases:
         interp = "nearest" if weight == "nearest" else "linear"
         cache = weight.split("cache-")[1] if "cache-" in weight else "off"
@@ -511,6 +523,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--table2", action="store_true", help="square grids shaped like the paper's Table II; 1 GPU")
     ap.add_argument("--sweep", action="store_true", help="per-config table (C1..C5), one JSON line each; 1 GPU")
+    ap.add_argument("--case", default="", help="with --sweep: only config:frames:mode[:order], e.g. C2:1:cache-single:3")
     ap.add_argument("--peaks", action="store_true", help="pab_measure_peaks: MUFU / FFMA / LDS.128 unit rates and pinned "
                                                          "copy rates of this box, one JSON line; 1 GPU")
     args = ap.parse_args()
