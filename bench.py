@@ -54,8 +54,8 @@ FP32_PER_ITEM = 6.0
 XU_PER_ITEM_ISSUED = 1.75
 DELAY_CACHE = "all"
 SM_COUNT = 148
-NCU_TRAFFIC_BYTES = 185_511_680 + 51_419_136   # per 64-frame launch; profiles/r1_step_ncu_f.md
-NCU_TRAFFIC_COMMIT = "17be8fa (round 1)"       # the build that capture was taken on: the constant goes stale silently otherwise
+NCU_TRAFFIC_BYTES = 181_811_968 + 49_764_864   # per 64-frame launch; profiles/r2_headline_ncu.md
+NCU_TRAFFIC_COMMIT = "1a0c0c6+ (round 2, diagonal-kernel build)"   # the build that capture was taken on: the constant goes stale silently otherwise
 XU_LANES_PER_CLK_SM = 16
 FP32_LANES_PER_CLK_SM = 128
 
@@ -314,7 +314,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                                          "frac_xu": items_per_launch * (XU_PER_ITEM + 1.0 / FRAMES) / xu_peak / (nc_launch_ms * 1e-3)},
                     "traffic": NCU_TRAFFIC_BYTES, "traffic_commit": NCU_TRAFFIC_COMMIT,
                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
-                                      "kernel at this workload: profiles/r1_step_ncu_f.md",
+                                      "kernel at this workload: profiles/r2_headline_ncu.md",
                     "peak_source": f"148 SM x 16 XU lanes/clk x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, "
                                    f"{peaks['source']}); DESIGN.md Roofline",
                     "launch_ms": bf_launch_ms, "launches_timed": bf_n,
