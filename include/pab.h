@@ -82,7 +82,8 @@ typedef struct {
     int   batch_frames;          /* internal frame batch per pass (ingest -> beamform -> post)                     */
     int   in_range;              /* 1 when every (pixel, element) delay index lies inside the record and z0 is at
                                     least one sample deep: the kernels then skip the out-of-record masks (A6)     */
-    int   reserved;
+    int   diagonal;              /* 1 once pab_set_delay_cache has built the tables of the single-frame diagonal kernel
+                                    (translation-invariant geometry: pitch an exact integer multiple of dx), else 0   */
     double zs_per_row;           /* dz * fs / c : delay samples per pixel row                                      */
     double xs_per_col;           /* dx * fs / c : delay samples per pixel column at grazing incidence              */
 } pab_plan_info;

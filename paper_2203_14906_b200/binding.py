@@ -36,7 +36,7 @@ class Grid(C.Structure):
 class PlanInfo(C.Structure):
     _fields_ = [("tile_z", C.c_int), ("tile_x", C.c_int), ("window_samples", C.c_int), ("chunk_channels", C.c_int),
                 ("stages", C.c_int), ("smem_bytes", C.c_int), ("frames_per_thread", C.c_int),
-                ("batch_frames", C.c_int), ("in_range", C.c_int), ("reserved", C.c_int), ("zs_per_row", C.c_double), ("xs_per_col", C.c_double)]
+                ("batch_frames", C.c_int), ("in_range", C.c_int), ("diagonal", C.c_int), ("zs_per_row", C.c_double), ("xs_per_col", C.c_double)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -230,6 +230,7 @@ int pab_set_tuning(pab_ctx* ctx, int frames_per_thread, int stages, int chunk_ch
     if (!plan_geometry(ctx->N, ctx->S, ctx->fs, ctx->c, ctx->pitch, ctx->grid, ctx->smem_optin, &plan, t)) return PAB_ERR_INVALID;
     PAB_CUDA(ctx, cudaDeviceSynchronize());
     ctx->tuning = t;
+    plan.diagonal = ctx->plan.diagonal;
     ctx->plan = plan;
     if (ctx->variant == PAB_VARIANT_STAGED && plan.smem_bytes == 0) ctx->variant = PAB_VARIANT_AUTO;
     return PAB_OK;
@@ -296,6 +297,7 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
         if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
         ctx->launches += 4;
     }
+    ctx->plan.diagonal = (mode != PAB_CACHE_OFF && (ctx->diag[0].smem_bytes > 0 || ctx->diag[1].smem_bytes > 0)) ? 1 : 0;
     ctx->cache_mode = mode;
     return PAB_OK;
 }

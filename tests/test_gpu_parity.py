@@ -609,6 +609,42 @@ def test_delay_cache_ragged_int16_and_batches(pab, orc):
                 check_raw(gpu[f], ref[f], order)
 
 
+@pytest.mark.parametrize("q,n_elem,nx,nz,frames,dtype", [(1, 16, 37, 70, 1, "float32"), (2, 24, 45, 33, 3, "float32"),
+                                                         (3, 8, 50, 129, 2, "int16"), (2, 4, 7, 5, 1, "float32"),
+                                                         (1, 64, 130, 95, 2, "int16"), (4, 12, 64, 64, 1, "float32")])
+def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, nz, frames, dtype):
+    """The single-frame diagonal kernel (pitch = q dx exactly: one tap per diagonal, channel-quad staging from the caller's
+    frame) on ragged grids: nx, nz off the tile sizes, arrays of 1..16 channel quads, q = 1..4, 1..3 frames, int16 input
+    with a scale, every order 1..5 (16 pixels per thread for orders 1..3, 8 for orders 4, 5)."""
+    rng = np.random.default_rng(100 + 7 * q + n_elem)
+    fs, c, S = 40e6, 1540.0, 900
+    dx = 2.0 ** -13                                              # 0.122 mm: q dx is a float32 for every small q
+    pitch = float(np.float32(q * np.float64(dx)))
+    assert pitch == q * dx                                       # exactly representable: the library's own test
+    x0 = -(nx - 1) / 2 * dx + 0.3 * dx
+    g = synth.Geometry(n_elem, S, fs, c, pitch, nx, nz, x0, dx, 2.1e-3, 0.09e-3).f32()
+    assert float(g.pitch) == q * float(g.dx)
+    base = [(rng.uniform(-1e-3, 1e-3), rng.uniform(3e-3, 9e-3), 1.0, 0.0) for _ in range(3)]
+    rf, _ = synth._frames(rng, g, base, 5e6, frames, 20.0, True)
+    scale = 1.0
+    if dtype == "int16":
+        rf, scale = np.rint(rf * 4000.0).astype(np.int16), 0.25
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, delay_cache="single")
+    try:
+        assert bf.plan()["in_range"] == 1 and bf.plan()["diagonal"] == 1          # the diagonal kernel is what runs
+        for order in (1, 2, 3, 4, 5):
+            if order > n_elem:
+                continue
+            out = bf.beamform(torch.from_numpy(rf).cuda(), order)
+            torch.cuda.synchronize()
+            gpu = out.cpu().numpy().astype(np.float64)
+            ref = orc.beamform(rf, g, order, scale=scale)
+            for f in range(frames):
+                assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
+    finally:
+        bf.close()
+
+
 def test_delay_cache_c2b_groups_and_fallbacks(pab, orc):
     w = synth.make_config("C2b", n_frames=20)
     gpu, _ = run_gpu(pab, w.geom, w.rf, 3, delay_cache="all")                 # one 16-frame group cached + 4 frames not
