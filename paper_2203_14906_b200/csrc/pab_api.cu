@@ -32,6 +32,8 @@ struct pab_ctx {
     int cache_mode = PAB_CACHE_OFF;
     uint32_t* d_taps = nullptr;          // cached interpolation taps, tile-major (pab_set_delay_cache)
     int* d_w0s = nullptr;                // window start of every (tile, element)
+    uint32_t* d_taps7 = nullptr;         // the same tables for 56-row tiles (order 1 at row pitches in (1, 8/7] samples)
+    int* d_w0s7 = nullptr;
     uint2* d_compact = nullptr;          // (d, row) tap table when pitch = q dx exactly (translation invariance)
     int cache_q = 0;
     DiagSet diag[2];                     // single-frame diagonal kernel: [0] orders 1..3 (16 pixels per thread), [1] orders 4, 5 (8)
@@ -81,7 +83,7 @@ size_t elem_size(int dtype) { return dtype == PAB_I16 ? 2 : 4; }
 
 void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
-    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact);
+    cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact); cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
     xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]);
     for (int b = 0; b < 2; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
@@ -268,7 +270,7 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
             if (e == cudaSuccess && need_compact) e = cudaMalloc(&ctx->d_compact, (size_t)nd * ctx->grid.nz * sizeof(uint2));
             if (e == cudaSuccess) {
                 CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
-                            (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x};
+                            (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x, kStgRows};
                 if (need_taps || need_w0s) {
                     xl_build_delay_cache(G, tiles_z, ctx->d_taps, ctx->d_w0s);
                     ctx->launches++;
@@ -284,6 +286,29 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
                 cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact);
                 ctx->d_taps = nullptr; ctx->d_w0s = nullptr; ctx->d_compact = nullptr;
                 return cuda_fail(ctx, e, "delay cache");
+            }
+        }
+    }
+    // Order 1 in frame groups is bound by the shared-memory data pipe, and at row pitches in (1, 8/7] samples 64-row
+    // tiles pay a bank conflict in every quarter-warp (tile_row, pab_pipe.cuh): a second table set for 56-row tiles,
+    // when it stays below 512 MB.
+    if (mode == PAB_CACHE_ALL && !ctx->d_taps7 && ctx->plan.zs_per_row > 1.0 && ctx->plan.zs_per_row <= 8.0 / 7.0 + 1e-9) {
+        const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z7 = (ctx->grid.nz + 55) / 56;
+        const size_t blocks7 = (size_t)tiles_x * tiles_z7 * ctx->N;
+        if (tiles_z7 <= 65535 && blocks7 * kCacheBlockBytes <= (512u << 20)) {
+            cudaError_t e = cudaMalloc(&ctx->d_w0s7, blocks7 * sizeof(int));
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_taps7, blocks7 * kCacheBlockBytes);
+            if (e == cudaSuccess) {
+                CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
+                            (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x, 56};
+                xl_build_delay_cache(G, tiles_z7, ctx->d_taps7, ctx->d_w0s7);
+                ctx->launches++;
+                e = cudaDeviceSynchronize();
+            }
+            if (e != cudaSuccess) {          // not fatal: order 1 keeps the 64-row tables
+                cudaGetLastError();
+                cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
+                ctx->d_taps7 = nullptr; ctx->d_w0s7 = nullptr;
             }
         }
     }

@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(kStgRows * kStgCols) delay_cache_kernel(const 
                                                                            int* __restrict__ w0s) {
     __shared__ int s_min;
     const int col = threadIdx.x / kStgRows, row = threadIdx.x % kStgRows;
-    const int j = min((int)blockIdx.x * kStgCols + col, G.nx - 1), m = min((int)blockIdx.y * kStgRows + row, G.nz - 1);
+    const int j = min((int)blockIdx.x * kStgCols + col, G.nx - 1), m = min((int)blockIdx.y * G.tile_rows + min(row, G.tile_rows - 1), G.nz - 1);
     const int i = blockIdx.z;
     // the definition, every operation individually rounded in fp64 (readings A5)
     const double x = __dadd_rn(G.x0, __dmul_rn((double)j, G.dx));
@@ -146,7 +146,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
     }
 
     const int col = warp & 7;
-    const int trow = (warp >> 3) * 32 + lane;                        // this thread's row inside the tile
+    bool live;
+    const int trow = tile_row(C.tile_rows, warp, lane, &live);       // this thread's row inside the tile
     const uint32_t my = (uint32_t)((col * kStgRows + trow) * 4);
     int s = 0;
     uint32_t ph = 0;
@@ -154,7 +155,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
         const int bz = tile % C.groups, txy = tile / C.groups;
         const int bx = txy % C.tiles_x, by = txy / C.tiles_x;
         const int j = bx * kStgCols + col;
-        const int m = by * kStgRows + trow;
+        const int m = by * C.tile_rows + trow;
         // one frame per thread: scalar accumulators; frame groups: the frames in pairs, packed f32x2 arithmetic
         float p[1][kAcc<K, W>];
         float2 pp[NQ == 0 ? 1 : NF / 2][kAcc<K, W>];
@@ -214,7 +215,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 
         const size_t img = (size_t)P.nz * P.nx;
         if constexpr (NQ == 0) {
-            if (j < P.nx && m < P.nz && bz < P.n_frames) P.out[(size_t)bz * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[0], P.inv_n);
+            if (live && j < P.nx && m < P.nz && bz < P.n_frames) P.out[(size_t)bz * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[0], P.inv_n);
         } else if (C.epi) {
 #pragma unroll
             for (int c = 0; c < NQ; ++c) {
@@ -222,9 +223,9 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                                     combine2_w<K, W>(pp[2 * c + 1], 0, P.inv_n), combine2_w<K, W>(pp[2 * c + 1], 1, P.inv_n)};
                 const int frame0 = bz * NF + 4 * c;
                 store_quad_transposed(ebuf, v, warp, lane, trow, col, P.out + (size_t)frame0 * img, img,
-                                      min(4, P.n_frames - frame0), by * kStgRows, bx * kStgCols, P.nz, P.nx);
+                                      min(4, P.n_frames - frame0), by * C.tile_rows, bx * kStgCols, P.nz, P.nx, C.tile_rows);
             }
-        } else if (j < P.nx && m < P.nz) {
+        } else if (live && j < P.nx && m < P.nz) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
@@ -324,7 +325,7 @@ inline bool cached_weight_ok(int order, int nq, bool compact) {
 inline void launch_cached(int order, int nq, int weight, const BfParams& P, int groups, const pab_plan_info& plan, int chunk_cap,
                           int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (T.compact ? 4 : kCacheBlockBytes);
-    const StagedCfg c = make_cfg(slot, plan.stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups);
+    const StagedCfg c = make_cfg(slot, plan.stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups, T.tile_rows);
     switch (order) {
     case 1: launch_cached_nq<1>(nq, weight, P, c, T, sm_count, st); break;
     case 2: launch_cached_nq<2>(nq, weight, P, c, T, sm_count, st); break;

@@ -84,13 +84,26 @@ __device__ __forceinline__ float lds32(uint32_t addr) {
 // 4 frames of a quad go through a 64 x 8 x 4 transpose buffer in shared memory and leave as whole 32-byte row
 // segments: 4 sectors per warp store.
 // ------------------------------------------------------------------------------------------------------
+// Row of the tile a consumer thread owns.  64-row tiles: warp half h = warp >> 3 holds rows 32 h + lane.  56-row tiles
+// (orders 1, 2 at row pitches in (1, 8/7] samples): a 128-bit shared load is served a quarter-warp at a time, 8 lanes
+// on 8 bank groups of 16 bytes; 8 consecutive rows at such a pitch span 9 samples, so the first and the last lane of a
+// quarter meet in one bank group and every quarter costs a second wavefront (measured: 28.6 % of the wavefronts of an
+// order-1 launch at C2b, whose kernel runs at 94 % of the shared-memory data pipe).  Seven rows never do (span < 8): the
+// eighth lane of every quarter repeats its neighbour's row (same address: a broadcast, no wavefront) and stores nothing.
+__device__ __forceinline__ int tile_row(int tile_rows, int warp, int lane, bool* live) {
+    if (tile_rows == kStgRows) { *live = true; return (warp >> 3) * 32 + lane; }
+    *live = (lane & 7) != 7;
+    return (warp >> 3) * 28 + (lane >> 3) * 7 + min(lane & 7, 6);
+}
+
 __device__ __forceinline__ void consumer_barrier() {
     asm volatile("bar.sync 1, %0;" ::"n"(kStgConsumerWarps * 32) : "memory");
 }
 // v[f]: this thread's pixel (tile row `row`, tile column `col`) of the quad's 4 frames.  out0 = image of the quad's
 // first frame; n_valid = how many of the 4 frames exist.  Every consumer thread of the CTA must call it.
 __device__ __forceinline__ void store_quad_transposed(uint32_t ebuf, const float (&v)[4], int warp, int lane, int row, int col,
-                                                      float* out0, size_t img, int n_valid, int m0, int j0, int nz, int nx) {
+                                                      float* out0, size_t img, int n_valid, int m0, int j0, int nz, int nx,
+                                                      int tile_rows = kStgRows) {
 #pragma unroll
     for (int f = 0; f < 4; ++f)
         asm volatile("st.shared.f32 [%0], %1;" ::"r"(ebuf + (uint32_t)(((f * kStgRows + row) * kEpiRowFloats + col) * 4)), "f"(v[f]) : "memory");
@@ -102,7 +115,7 @@ __device__ __forceinline__ void store_quad_transposed(uint32_t ebuf, const float
             const int r = (warp & 3) * 16 + i * 4 + (lane >> 3);
             float x;
             asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(ebuf + (uint32_t)(((f * kStgRows + r) * kEpiRowFloats + c) * 4)));
-            if (m0 + r < nz) out0[(size_t)f * img + (size_t)(m0 + r) * nx + (j0 + c)] = x;
+            if (r < tile_rows && m0 + r < nz) out0[(size_t)f * img + (size_t)(m0 + r) * nx + (j0 + c)] = x;
         }
     }
     consumer_barrier();                 // the buffer is free for the next quad
@@ -139,7 +152,8 @@ inline int resident_per_sm(Kernel kernel, int threads, size_t smem) {
 
 // Channels per stage for a launch whose channel slot is `slot` bytes, and whether the epilogue buffer fits beside the
 // ring: the buffer is taken when at least two channels per stage still fit with it (groups of 8 and 16 frames only).
-inline StagedCfg make_cfg(long long slot, int stages, int window, int nq, int chunk_cap, int smem_limit, const BfParams& P, int groups) {
+inline StagedCfg make_cfg(long long slot, int stages, int window, int nq, int chunk_cap, int smem_limit, const BfParams& P, int groups,
+                          int tile_rows = kStgRows) {
     auto fit = [&](long long avail) {
         long long ch = avail / (stages * slot);
         if (ch > kStagedMaxChunk) ch = kStagedMaxChunk;
@@ -156,7 +170,7 @@ inline StagedCfg make_cfg(long long slot, int stages, int window, int nq, int ch
     }
     if (chunk > 2 && (chunk & 1) && chunk < P.N) --chunk;      // even: the element loop is unrolled by two
     if (chunk < 1) chunk = 1;
-    return StagedCfg{(int)chunk, stages, window, (P.nx + kStgCols - 1) / kStgCols, (P.nz + kStgRows - 1) / kStgRows, groups, epi};
+    return StagedCfg{(int)chunk, stages, window, (P.nx + kStgCols - 1) / kStgCols, (P.nz + tile_rows - 1) / tile_rows, groups, epi, tile_rows};
 }
 
 }  // namespace pab

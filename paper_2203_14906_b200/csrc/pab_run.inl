@@ -81,7 +81,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         {
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
             if (cached) xl_cached(order, 0, 0, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
-                                      CacheTables{ctx->d_taps, ctx->d_w0s, ctx->d_compact, ctx->cache_q}, st);
+                                      CacheTables{ctx->d_taps, ctx->d_w0s, ctx->d_compact, ctx->cache_q, kStgRows}, st);
             else if (use_staged) xl_staged(order, 0, in_range, weight, P, F, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else xl_direct(order, 0, weight, P, F, st);
         }
@@ -108,7 +108,9 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && (order <= 5 || g == 1) &&
                 (weight == 0 || xl_cached_weight_ok(order, g, false)) && xl_cached_fits(ctx->plan, g, false, ctx->smem_optin))
                 xl_cached(order, g, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
-                              CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0}, st);
+                              (order == 1 && weight == 0 && g >= 2 && ctx->d_taps7)
+                                  ? CacheTables{ctx->d_taps7, ctx->d_w0s7, nullptr, 0, 56}
+                                  : CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0, kStgRows}, st);
             else if (use_staged) xl_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);
             else xl_direct(order, g, weight, R, groups, st);
             q0 += groups * g;

@@ -59,8 +59,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
         uint32_t ph = 1;                                     // parity to wait for on empty[s]
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             const int bx = tile % C.tiles_x, by = (tile / C.tiles_x) % C.tiles_z, bz = tile / (C.tiles_x * C.tiles_z);
-            const int c0 = bx * kStgCols, r0 = by * kStgRows;
-            const int rl = min(r0 + kStgRows - 1, P.nz - 1);
+            const int c0 = bx * kStgCols, r0 = by * C.tile_rows;
+            const int rl = min(r0 + C.tile_rows - 1, P.nz - 1);
             const float4 zf = P.zrow[r0], zl = P.zrow[rl];
             float2 xj[kStgCols];
 #pragma unroll
@@ -124,7 +124,9 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int bx = tile % C.tiles_x, by = (tile / C.tiles_x) % C.tiles_z, bz = tile / (C.tiles_x * C.tiles_z);
         const int j = bx * kStgCols + col;
-        const int m = by * kStgRows + (warp >> 3) * 32 + lane;
+        bool live;
+        const int trow = tile_row(C.tile_rows, warp, lane, &live);
+        const int m = by * C.tile_rows + trow;
         const float4 row = P.zrow[min(m, P.nz - 1)];
         // one frame per thread: scalar accumulators; frame groups: the frames in pairs, packed f32x2 arithmetic
         float p[1][kAcc<K, W>];
@@ -179,17 +181,17 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
 
         const size_t img = (size_t)P.nz * P.nx;
         if constexpr (NQ == 0) {
-            if (j < P.nx && m < P.nz && bz < P.n_frames) P.out[(size_t)bz * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[0], P.inv_n);
+            if (live && j < P.nx && m < P.nz && bz < P.n_frames) P.out[(size_t)bz * img + (size_t)m * P.nx + j] = combine_w<K, W>(p[0], P.inv_n);
         } else if (C.epi) {
 #pragma unroll
             for (int c = 0; c < NQ; ++c) {
                 const float v[4] = {combine2_w<K, W>(pp[2 * c], 0, P.inv_n), combine2_w<K, W>(pp[2 * c], 1, P.inv_n),
                                     combine2_w<K, W>(pp[2 * c + 1], 0, P.inv_n), combine2_w<K, W>(pp[2 * c + 1], 1, P.inv_n)};
                 const int frame0 = bz * NF + 4 * c;
-                store_quad_transposed(ebuf, v, warp, lane, (warp >> 3) * 32 + lane, col, P.out + (size_t)frame0 * img, img,
-                                      min(4, P.n_frames - frame0), by * kStgRows, bx * kStgCols, P.nz, P.nx);
+                store_quad_transposed(ebuf, v, warp, lane, trow, col, P.out + (size_t)frame0 * img, img,
+                                      min(4, P.n_frames - frame0), by * C.tile_rows, bx * kStgCols, P.nz, P.nx, C.tile_rows);
             }
-        } else if (j < P.nx && m < P.nz) {
+        } else if (live && j < P.nx && m < P.nz) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const int frame = bz * NF + f;
@@ -271,7 +273,11 @@ inline void launch_staged_t(int order, int nq, int weight, const BfParams& P, in
                             int chunk_cap, int smem_limit, int sm_count, cudaStream_t st) {
     // the plan's chunk is sized for frames_per_thread / 4 quads per channel; fewer quads -> more channels per stage
     const long long slot = (long long)plan.window_samples * (nq == 0 ? 4 : 16 * nq) + (long long)sizeof(ChanEntry);
-    const StagedCfg c = make_cfg(slot, plan.stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups);
+    // order 1 in groups of 8 / 16 frames is bound by the shared-memory data pipe: 56-row tiles where the row pitch makes
+    // 64-row tiles conflict (tile_row, pab_pipe.cuh).  Order 2 (one MUFU per item) loses more to the idle lanes than it
+    // gains (measured 0.831 -> 0.859 ms at C2b), so it keeps 64 rows.
+    const bool r7 = order == 1 && weight == 0 && nq >= 2 && plan.zs_per_row > 1.0 && plan.zs_per_row <= 8.0 / 7.0 + 1e-9;
+    const StagedCfg c = make_cfg(slot, plan.stages, plan.window_samples, nq, chunk_cap, smem_limit, P, groups, r7 ? 56 : kStgRows);
     launch_staged_inr<INR>(order, nq, weight, P, c, sm_count, st);
 }
 

@@ -11,7 +11,7 @@ void xl_cached(int order, int nq, int weight, const BfParams& P, int groups, con
                int smem_limit, int sm_count, const CacheTables& T, cudaStream_t st) {
     launch_cached(order, nq, weight, P, groups, plan, chunk_cap, smem_limit, sm_count, T, st);
 }
-void xl_build_delay_cache(const CacheGeom& G, int tiles_z, uint32_t* taps, int* w0s) {
+void xl_build_delay_cache(const CacheGeom& G, int tiles_z, uint32_t* taps, int* w0s) {          // tiles_z = ceil(nz / G.tile_rows)
     delay_cache_kernel<<<dim3(G.tiles_x, tiles_z, G.N), kStgRows * kStgCols>>>(G, taps, w0s);
 }
 void xl_build_delay_compact(const CacheGeom& G, int q, int nd, uint2* compact) {

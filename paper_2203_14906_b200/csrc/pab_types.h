@@ -48,6 +48,7 @@ struct StagedCfg {
     int window;         // samples per channel slot per quad (multiple of 4)
     int tiles_x, tiles_z, groups;   // tile grid: columns / 8, rows / 64, frame groups; tile t = (t % tiles_x, ...)
     int epi;            // 1: the tile's images leave through the shared-memory transpose buffer (coalesced stores)
+    int tile_rows;      // 64, or 56: seven rows per quarter-warp, the eighth lane idle (see tile_row in pab_pipe.cuh)
 };
 
 // cached interpolation taps (pab_cache.cuh)
@@ -58,12 +59,14 @@ constexpr int kCacheMaxWindow = 4000;        // the integer part must fit 12 bit
 struct CacheGeom {
     double fs, c, pitch, x0, dx, z0, dz;
     int N, S, nx, nz, tiles_x;
+    int tile_rows;             // rows of a tile that are in use: 64, or 56 (the block keeps 64 row slots either way)
 };
 struct CacheTables {
     const uint32_t* taps;      // tile-major 12+20-bit taps, or nullptr when the compact table is in use
     const int* w0s;            // window start of every (tile, element)
     const uint2* compact;      // (d, row) table of translation-invariant geometries, or nullptr
     int q;                     // pitch / dx
+    int tile_rows;             // 64, or 56 for the table set of order 1 (seven rows per quarter-warp)
 };
 
 // single-frame diagonal kernel (pab_diag.cuh)

@@ -645,6 +645,26 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
         bf.close()
 
 
+@pytest.mark.parametrize("delay_cache", ["all", "off"])
+def test_order1_56_row_tiles(pab, orc, delay_cache):
+    """Order 1 in groups of 8 / 16 frames at a row pitch in (1, 8/7] samples takes 56-row tiles (seven rows per
+    quarter-warp, the eighth lane idle: pab_pipe.cuh tile_row), with their own tap tables under PAB_CACHE_ALL: the C2b
+    geometry (nz = 1024 = 18 x 56 + 16: a ragged last tile) and a small ragged grid, 20 frames = 16 + 4."""
+    w = synth.make_config("C2b", n_frames=20)
+    assert 1.0 < pab.plan(w.geom)["zs_per_row"] <= 8.0 / 7.0
+    gpu, _ = run_gpu(pab, w.geom, w.rf, 1, delay_cache=delay_cache)
+    for f in (0, 15, 16, 19):
+        assert check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, 1)[0], 1) <= 2.5e-5
+    g = w.geom
+    small = synth.Geometry(24, 700, g.fs, g.c, g.pitch, 37, 131, -18 * g.dx, g.dx, 4e-3, g.dz).f32()
+    rng = np.random.default_rng(56)
+    rf = rng.standard_normal((24, 24, 700)).astype(np.float32)
+    gpu, _ = run_gpu(pab, small, rf, 1, delay_cache=delay_cache)
+    ref = orc.beamform(rf, small, 1)
+    for f in range(24):
+        check_raw(gpu[f], ref[f], 1)
+
+
 def test_delay_cache_c2b_groups_and_fallbacks(pab, orc):
     w = synth.make_config("C2b", n_frames=20)
     gpu, _ = run_gpu(pab, w.geom, w.rf, 3, delay_cache="all")                 # one 16-frame group cached + 4 frames not
