@@ -108,7 +108,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             if (ctx->cache_mode == PAB_CACHE_ALL && use_staged && (order <= 5 || g == 1) &&
                 (weight == 0 || xl_cached_weight_ok(order, g, false)) && xl_cached_fits(ctx->plan, g, false, ctx->smem_optin))
                 xl_cached(order, g, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count,
-                              (order == 1 && weight == 0 && g >= 2 && ctx->d_taps7)
+                              (order <= 2 && weight == 0 && g >= 2 && ctx->d_taps7)
                                   ? CacheTables{ctx->d_taps7, ctx->d_w0s7, nullptr, 0, 56}
                                   : CacheTables{ctx->d_taps, ctx->d_w0s, nullptr, 0, kStgRows}, st);
             else if (use_staged) xl_staged(order, g, in_range, weight, R, groups, ctx->plan, ctx->tuning.chunk_channels, ctx->smem_optin, ctx->sm_count, st);

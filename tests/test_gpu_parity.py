@@ -646,23 +646,26 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
 
 
 @pytest.mark.parametrize("delay_cache", ["all", "off"])
-def test_order1_56_row_tiles(pab, orc, delay_cache):
-    """Order 1 in groups of 8 / 16 frames at a row pitch in (1, 8/7] samples takes 56-row tiles (seven rows per
-    quarter-warp, the eighth lane idle: pab_pipe.cuh tile_row), with their own tap tables under PAB_CACHE_ALL: the C2b
-    geometry (nz = 1024 = 18 x 56 + 16: a ragged last tile) and a small ragged grid, 20 frames = 16 + 4."""
+@pytest.mark.parametrize("order", [1, 2])
+def test_56_row_tiles(pab, orc, order, delay_cache):
+    """Orders 1 and 2 (cached taps; order 1 also with in-kernel delays) in groups of 8 / 16 frames at a row pitch in
+    (1, 8/7] samples take 56-row tiles (seven rows per quarter-warp, the eighth lane idle: pab_pipe.cuh tile_row), with
+    their own tap tables under PAB_CACHE_ALL: the C2b geometry (nz = 1024 = 18 x 56 + 16: a ragged last tile) and a small
+    ragged grid, 20 and 24 frames (16 + 4, 16 + 8)."""
     w = synth.make_config("C2b", n_frames=20)
     assert 1.0 < pab.plan(w.geom)["zs_per_row"] <= 8.0 / 7.0
-    gpu, _ = run_gpu(pab, w.geom, w.rf, 1, delay_cache=delay_cache)
+    gpu, _ = run_gpu(pab, w.geom, w.rf, order, delay_cache=delay_cache)
     for f in (0, 15, 16, 19):
-        assert check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, 1)[0], 1) <= 2.5e-5
+        assert check_raw(gpu[f], orc.beamform(w.rf[f:f + 1], w.geom, order)[0], order) <= 2.5e-5
     g = w.geom
     small = synth.Geometry(24, 700, g.fs, g.c, g.pitch, 37, 131, -18 * g.dx, g.dx, 4e-3, g.dz).f32()
     rng = np.random.default_rng(56)
-    rf = rng.standard_normal((24, 24, 700)).astype(np.float32)
-    gpu, _ = run_gpu(pab, small, rf, 1, delay_cache=delay_cache)
-    ref = orc.beamform(rf, small, 1)
+    base = [(rng.uniform(-2e-3, 2e-3), rng.uniform(5e-3, 9e-3), 1.0, 0.0) for _ in range(3)]
+    rf, _ = synth._frames(rng, small, base, 5e6, 24, 20.0, True)
+    gpu, _ = run_gpu(pab, small, rf, order, delay_cache=delay_cache)
+    ref = orc.beamform(rf, small, order)
     for f in range(24):
-        check_raw(gpu[f], ref[f], 1)
+        check_raw(gpu[f], ref[f], order)
 
 
 def test_delay_cache_c2b_groups_and_fallbacks(pab, orc):
