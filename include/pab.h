@@ -168,6 +168,8 @@ int pab_set_variant(pab_ctx* ctx, int variant);
  *              O(N) evaluation of e_k, by its recurrence) with linear interpolation and no weighting only
  *   out_dev    device pointer, [n_frames][nz][nx], x fastest, fp32, 4-byte aligned; fully overwritten
  *   cuda_stream a cudaStream_t passed as void*; NULL = the legacy default stream
+ * Exception: under PAB_CACHE_ALL the first call of order 1 or 2 with >= 8 frames, at a row pitch in (1, 8/7] samples,
+ * builds a second tap table once (one device synchronisation; skipped while the stream is being captured).
  * One context must not be used from two streams at once (shared scratch).  The CUDA device that was current at
  * pab_create must be current at the call (PAB_ERR_INVALID otherwise).
  * Errors: PAB_ERR_INVALID (nothing launched), PAB_ERR_CUDA.

@@ -62,10 +62,11 @@ def load(build_if_missing: bool = False):
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_missing:
+    if build_if_missing and not os.path.exists(LIB_PATH):
+        # absent only: a copied tree (gpurun, a checkout) does not keep modification times, so "older than a source
+        # file" cannot be told from them; `python -m paper_2203_14906_b200.build` rebuilds a stale library
         from . import build as _b
-        if _b.is_stale():                       # absent, or older than a source file
-            _b.build_lib()
+        _b.build_lib()
     if not os.path.exists(LIB_PATH):
         raise PabError(f"{LIB_PATH} is missing: build it with `python -m paper_2203_14906_b200.build` "
                        "(there is no CPU fallback)")

@@ -34,6 +34,7 @@ struct pab_ctx {
     int* d_w0s = nullptr;                // window start of every (tile, element)
     uint32_t* d_taps7 = nullptr;         // the same tables for 56-row tiles (order 1 at row pitches in (1, 8/7] samples)
     int* d_w0s7 = nullptr;
+    bool taps7_tried = false;
     uint2* d_compact = nullptr;          // (d, row) tap table when pitch = q dx exactly (translation invariance)
     int cache_q = 0;
     DiagSet diag[2];                     // single-frame diagonal kernel: [0] orders 1..3 (16 pixels per thread), [1] orders 4, 5 (8)
@@ -96,6 +97,36 @@ void free_all(pab_ctx* ctx) {
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_run) cudaStreamDestroy(ctx->s_run);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+}
+
+// Orders 1 and 2 in frame groups are bound by the shared-memory data pipe, and at row pitches in (1, 8/7] samples 64-row
+// tiles pay a bank conflict in every quarter-warp (tile_row, pab_pipe.cuh): a second tap-table set for 56-row tiles, when
+// it stays below 512 MB.  Built on the first frame-group call of order 1 or 2 under PAB_CACHE_ALL (one device
+// synchronisation, skipped while the stream is being captured), so that contexts that never run those orders do not
+// carry the second table.
+void ensure_taps7(pab_ctx* ctx, cudaStream_t st) {
+    if (ctx->taps7_tried) return;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) { cudaGetLastError(); return; }
+    ctx->taps7_tried = true;
+    if (!(ctx->plan.zs_per_row > 1.0 && ctx->plan.zs_per_row <= 8.0 / 7.0 + 1e-9)) return;
+    const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z7 = (ctx->grid.nz + 55) / 56;
+    const size_t blocks7 = (size_t)tiles_x * tiles_z7 * ctx->N;
+    if (tiles_z7 > 65535 || blocks7 * kCacheBlockBytes > (512u << 20)) return;
+    cudaError_t e = cudaMalloc(&ctx->d_w0s7, blocks7 * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_taps7, blocks7 * kCacheBlockBytes);
+    if (e == cudaSuccess) {
+        CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
+                    (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x, 56};
+        xl_build_delay_cache(G, tiles_z7, ctx->d_taps7, ctx->d_w0s7);
+        ctx->launches++;
+        e = cudaDeviceSynchronize();
+    }
+    if (e != cudaSuccess) {          // not fatal: the orders keep the 64-row tables
+        cudaGetLastError();
+        cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
+        ctx->d_taps7 = nullptr; ctx->d_w0s7 = nullptr;
+    }
 }
 
 }  // namespace
@@ -289,35 +320,12 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
             }
         }
     }
-    // Order 1 in frame groups is bound by the shared-memory data pipe, and at row pitches in (1, 8/7] samples 64-row
-    // tiles pay a bank conflict in every quarter-warp (tile_row, pab_pipe.cuh): a second table set for 56-row tiles,
-    // when it stays below 512 MB.
-    if (mode == PAB_CACHE_ALL && !ctx->d_taps7 && ctx->plan.zs_per_row > 1.0 && ctx->plan.zs_per_row <= 8.0 / 7.0 + 1e-9) {
-        const int tiles_x = (ctx->grid.nx + kStgCols - 1) / kStgCols, tiles_z7 = (ctx->grid.nz + 55) / 56;
-        const size_t blocks7 = (size_t)tiles_x * tiles_z7 * ctx->N;
-        if (tiles_z7 <= 65535 && blocks7 * kCacheBlockBytes <= (512u << 20)) {
-            cudaError_t e = cudaMalloc(&ctx->d_w0s7, blocks7 * sizeof(int));
-            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_taps7, blocks7 * kCacheBlockBytes);
-            if (e == cudaSuccess) {
-                CacheGeom G{(double)ctx->fs, (double)ctx->c, (double)ctx->pitch, (double)ctx->grid.x0, (double)ctx->grid.dx,
-                            (double)ctx->grid.z0, (double)ctx->grid.dz, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, tiles_x, 56};
-                xl_build_delay_cache(G, tiles_z7, ctx->d_taps7, ctx->d_w0s7);
-                ctx->launches++;
-                e = cudaDeviceSynchronize();
-            }
-            if (e != cudaSuccess) {          // not fatal: order 1 keeps the 64-row tables
-                cudaGetLastError();
-                cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
-                ctx->d_taps7 = nullptr; ctx->d_w0s7 = nullptr;
-            }
-        }
-    }
     // translation-invariant geometries: calls of 1..3 frames take the diagonal kernel (pab_diag.cuh), which shares one
     // tap among the 16 (8 for orders 4, 5) pairs of a diagonal and reads the caller's frame in place
     if (mode != PAB_CACHE_OFF && ctx->d_compact && ctx->diag[0].smem_bytes == 0 && ctx->diag[1].smem_bytes == 0) {
         PAB_CUDA(ctx, xl_diag_configure(ctx->smem_optin));
         cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q,
-                                      (getenv("PAB_DIAG_NPG") && atoi(getenv("PAB_DIAG_NPG")) == 2) ? 2 : 4, 3, ctx->smem_optin, &ctx->diag[0]);
+                                      4, 3, ctx->smem_optin, &ctx->diag[0]);
         if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, &ctx->diag[1]);
         if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
         ctx->launches += 4;

@@ -13,7 +13,6 @@
 // that the table and the staged window agree exactly.
 #pragma once
 #include <cstdint>
-#include <cstdlib>
 #include <type_traits>
 #include <cuda_runtime.h>
 #include "pab_math.cuh"
@@ -71,7 +70,8 @@ __device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
 // W = 1: coherence-factor weighting (row f1), frame groups with the tile-major table only (NQ = 1, 2; orders 4, 5: NQ = 1).
 // RM (root mix, order 3, 16 frames per thread): how many of a thread's 8 frame pairs take their cube root on the FMA
 // pipe (cbrt_fma2) instead of the XU pipe: 0, 1 (pair 7) or 2 (pairs 3 and 7).
-template <int K, int NQ, bool COMPACT, int W = 0, int RM = 0>
+// R7: 56-row tiles (pab_pipe.cuh tile_row; orders 1, 2 with their own table set).
+template <int K, int NQ, bool COMPACT, int W = 0, int RM = 0, bool R7 = false>
 __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParams P, const StagedCfg C,
                                                                     const uint32_t* __restrict__ taps,
                                                                     const int* __restrict__ w0s,
@@ -147,7 +147,8 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
 
     const int col = warp & 7;
     bool live;
-    const int trow = tile_row(C.tile_rows, warp, lane, &live);       // this thread's row inside the tile
+    constexpr int TR = R7 ? 56 : kStgRows;
+    const int trow = tile_row(TR, warp, lane, &live);                // this thread's row inside the tile
     const uint32_t my = (uint32_t)((col * kStgRows + trow) * 4);
     int s = 0;
     uint32_t ph = 0;
@@ -155,7 +156,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
         const int bz = tile % C.groups, txy = tile / C.groups;
         const int bx = txy % C.tiles_x, by = txy / C.tiles_x;
         const int j = bx * kStgCols + col;
-        const int m = by * C.tile_rows + trow;
+        const int m = by * TR + trow;
         // one frame per thread: scalar accumulators; frame groups: the frames in pairs, packed f32x2 arithmetic
         float p[1][kAcc<K, W>];
         float2 pp[NQ == 0 ? 1 : NF / 2][kAcc<K, W>];
@@ -223,7 +224,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_cached_kernel(const BfParam
                                     combine2_w<K, W>(pp[2 * c + 1], 0, P.inv_n), combine2_w<K, W>(pp[2 * c + 1], 1, P.inv_n)};
                 const int frame0 = bz * NF + 4 * c;
                 store_quad_transposed(ebuf, v, warp, lane, trow, col, P.out + (size_t)frame0 * img, img,
-                                      min(4, P.n_frames - frame0), by * C.tile_rows, bx * kStgCols, P.nz, P.nx, C.tile_rows);
+                                      min(4, P.n_frames - frame0), by * TR, bx * kStgCols, P.nz, P.nx, TR);
             }
         } else if (live && j < P.nx && m < P.nz) {
 #pragma unroll
@@ -261,7 +262,8 @@ inline cudaError_t cached_set_attr_k(int smem_optin) {
         return cached_set_attr<K, 4>(smem_optin);
     } else return cudaSuccess;
 }
-constexpr int kRootMix = 1;          // order 3, 16 frames per thread: frame pairs rooted on the FMA pipe (measured best)
+constexpr int kRootMix = 1;          // order 3, 16 frames per thread: frame pairs rooted on the FMA pipe (0 / 1 / 2 pairs measured
+                                     // 1.037 / 0.981 / 1.006 ms at C2b: DESIGN.md section 6.1)
 inline cudaError_t cached_configure(int smem_optin) {
     cudaError_t e;
     if ((e = cached_set_attr_k<1>(smem_optin)) != cudaSuccess) return e;
@@ -269,8 +271,11 @@ inline cudaError_t cached_configure(int smem_optin) {
     if ((e = cached_set_attr_k<3>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr_k<4>(smem_optin)) != cudaSuccess) return e;
     if ((e = cached_set_attr_k<5>(smem_optin)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(bf_cached_kernel<3, 4, false, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(bf_cached_kernel<3, 4, false, 0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<3, 4, false, 0, kRootMix>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<1, 2, false, 0, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<1, 4, false, 0, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<2, 2, false, 0, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_cached_kernel<2, 4, false, 0, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
     // orders 6..8 (row f2): 4-frame groups with the tile-major table only
     if ((e = cudaFuncSetAttribute(bf_cached_kernel<6, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(bf_cached_kernel<7, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
@@ -284,12 +289,22 @@ inline void launch_cached_rm(const BfParams& P, const StagedCfg& c, const CacheT
     bf_cached_kernel<K, NQ, COMPACT, W, RM><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
         P, c, T.taps, T.w0s, T.compact, T.q);
 }
+template <int K, int NQ>
+inline void launch_cached_r7(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    const size_t smem = cached_smem_bytes(c, NQ, false);
+    const int per_sm = resident_per_sm(bf_cached_kernel<K, NQ, false, 0, 0, true>, kStgThreads, smem);
+    const long long tiles = (long long)c.tiles_x * c.tiles_z * c.groups, resident = (long long)sm_count * per_sm;
+    bf_cached_kernel<K, NQ, false, 0, 0, true><<<(unsigned)(tiles < resident ? tiles : resident), kStgThreads, smem, st>>>(
+        P, c, T.taps, T.w0s, T.compact, T.q);
+}
 template <int K, int NQ, bool COMPACT, int W = 0>
 inline void launch_cached_kc(const BfParams& P, const StagedCfg& c, const CacheTables& T, int sm_count, cudaStream_t st) {
+    if constexpr (K <= 2 && (NQ == 2 || NQ == 4) && !COMPACT && W == 0) {
+        if (c.tile_rows == 56) { launch_cached_r7<K, NQ>(P, c, T, sm_count, st); return; }
+    }
     if constexpr (K == 3 && NQ == 4 && !COMPACT && W == 0) {
-        static const int rm = [] { const char* e = getenv("PAB_ROOT_MIX"); return e ? atoi(e) : kRootMix; }();   // tuning knob
-        if (rm == 1) { launch_cached_rm<K, NQ, COMPACT, W, 1>(P, c, T, sm_count, st); return; }
-        if (rm == 2) { launch_cached_rm<K, NQ, COMPACT, W, 2>(P, c, T, sm_count, st); return; }
+        launch_cached_rm<K, NQ, COMPACT, W, kRootMix>(P, c, T, sm_count, st);
+        return;
     }
     launch_cached_rm<K, NQ, COMPACT, W, 0>(P, c, T, sm_count, st);
 }

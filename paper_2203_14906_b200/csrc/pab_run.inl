@@ -90,6 +90,7 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             Span sp(ctx, PAB_STAGE_INGEST, st);
             xl_ingest_quad(ctx->dtype, rf, ctx->d_stage, F, N, S, ctx->scale, st);
         }
+        if (ctx->cache_mode == PAB_CACHE_ALL && order <= 2 && weight == 0 && F >= 8) ensure_taps7(ctx, st);
         // quads are consumed in groups of frames_per_thread / 4, then the remainder in halves (4 -> 2 -> 1)
         int nq = (F + 3) / 4, q0 = 0;
         // orders 4 and 5 carry at most 8 frames per thread (16 x 5 accumulators would spill)

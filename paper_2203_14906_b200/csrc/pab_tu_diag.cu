@@ -1,6 +1,5 @@
 // pab_tu_diag.cu -- translation unit: the single-frame "diagonal" beamforming kernel (pab_diag.cuh) and its tables.
 #include <algorithm>
-#include <cstdlib>
 #include <vector>
 #include "pab_diag.cuh"
 #include "pab_launch.h"
@@ -67,9 +66,6 @@ cudaError_t xl_diag_configure(int smem_optin) {
     if ((e = diag_attr<1, 4>(smem_optin)) != cudaSuccess) return e;
     if ((e = diag_attr<2, 4>(smem_optin)) != cudaSuccess) return e;
     if ((e = diag_attr<3, 4>(smem_optin)) != cudaSuccess) return e;
-    if ((e = diag_attr<1, 2>(smem_optin)) != cudaSuccess) return e;
-    if ((e = diag_attr<2, 2>(smem_optin)) != cudaSuccess) return e;
-    if ((e = diag_attr<3, 2>(smem_optin)) != cudaSuccess) return e;
     if ((e = diag_attr<4, 2>(smem_optin)) != cudaSuccess) return e;
     return diag_attr<5, 2>(smem_optin);
 }
@@ -87,13 +83,14 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     *D = DiagSet();
     const int P = 4 * npg;
     if (N % 4 != 0 || N < 4 || q < 1 || q > 8) return cudaSuccess;
-    // tuning knobs (environment, read when the tables are built): rows per tile and warps per CTA
-    auto knob = [](const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; };
+    // Blocking, measured at C2 and C4: 32-row tiles of one column block, 8 warps per CTA (two CTAs
+    // per SM at 128 registers); 16-row tiles, 2..16 warps and 2..4 column blocks per tile were all slower.
+    constexpr int kRows = 32, kBlocks = 1, kWarps = 8;
     DiagCfg cfg{};
     cfg.q = q;
-    cfg.rows = knob("PAB_DIAG_ROWS", 32) == 16 ? 16 : 32;
+    cfg.rows = kRows;
     const int lj = 32 / cfg.rows;
-    cfg.cp = (q % lj == 0 ? q : q * lj) * std::max(1, std::min(4, knob("PAB_DIAG_BLOCKS", 1)));      // lcm(q, lj) x column blocks per tile
+    cfg.cp = (q % lj == 0 ? q : q * lj) * kBlocks;      // lcm(q, lj) x column blocks per tile
     cfg.wpp = cfg.cp / lj;
     cfg.cols = P * cfg.cp;
     cfg.tiles_x = (g.nx + cfg.cols - 1) / cfg.cols;
@@ -105,7 +102,7 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     const int G = N / 4 + npg;
     int best_parts = 0;
     double best_cost = 1e30;
-    const int target = knob("PAB_DIAG_WARPS", 8);          // measured best at C2 and C4: 8 warps, two CTAs per SM
+    const int target = kWarps;
     const int max_warps = kDiagMaxWarps;
     const int max_parts = std::max(1, std::min(std::min(kDiagMaxParts, max_warps / cfg.wpp), target / cfg.wpp));
     for (int parts = std::max(1, max_parts - 1); parts <= max_parts; ++parts) {
@@ -152,9 +149,9 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
 void xl_diag(int order, int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
              cudaStream_t st) {
     switch (order) {
-    case 1: D.npg == 4 ? launch_diag_k<1, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st) : launch_diag_k<1, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
-    case 2: D.npg == 4 ? launch_diag_k<2, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st) : launch_diag_k<2, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
-    case 3: D.npg == 4 ? launch_diag_k<3, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st) : launch_diag_k<3, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    case 1: launch_diag_k<1, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    case 2: launch_diag_k<2, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+    case 3: launch_diag_k<3, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
     case 4: launch_diag_k<4, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
     default: launch_diag_k<5, 2>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
     }
