@@ -224,6 +224,14 @@ long long pab_launch_count(const pab_ctx* ctx);
 int pab_set_profile(pab_ctx* ctx, int max_launches);
 int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset);
 
+/* pab_self_check -- diagnostic for the single-frame diagonal kernel (pab_plan_info.diagonal == 1; fp32 input): runs one
+ * frame through an instantiation that compares every shared-memory gather of its element loop with the staged window of
+ * the channel quad it reads from, and returns the number of out-of-window accesses (0 for a correct build).  Stands in
+ * for compute-sanitizer's memcheck, which is closed on the GPU pool this library was developed on.  order 1..5 selects
+ * the table set (orders 1..3 / 4, 5).  Synchronises the device.  Errors: PAB_ERR_INVALID (no diagonal tables, int16
+ * input), PAB_ERR_ALLOC, PAB_ERR_CUDA. */
+int pab_self_check(pab_ctx* ctx, const float* rf_dev, int order, long long* violations);
+
 /* pab_measure_peaks -- the microbenchmarks behind the roofline denominators, run on the
  * current device: out_host[0] MUFU (lg2/ex2) lanes per clock per SM, [1] FFMA lanes/clk/SM, [2] packed FFMA2 fp32
  * results/clk/SM, [3] conflict-free LDS.128 bytes/clk/SM (each timed with clock64 inside one 1024-thread CTA per

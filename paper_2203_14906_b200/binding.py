@@ -25,7 +25,7 @@ _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_S
 # every symbol include/pab.h declares
 SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_delay_cache", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
-           "pab_launch_count", "pab_measure_peaks", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
+           "pab_launch_count", "pab_measure_peaks", "pab_self_check", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
 
 class Grid(C.Structure):
@@ -92,6 +92,7 @@ def load(build_if_missing: bool = False):
     L.pab_launch_count.restype = C.c_longlong
     L.pab_image_metrics.argtypes = [vp, vp, C.POINTER(Roi), C.POINTER(Roi), ip, ip, C.POINTER(Metrics), vp]
     L.pab_measure_peaks.argtypes = [C.POINTER(C.c_double), ip]
+    L.pab_self_check.argtypes = [vp, vp, ip, C.POINTER(C.c_longlong)]
     L.pab_set_profile.argtypes = [vp, ip]
     L.pab_get_profile.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong), ip]
     L.pab_strerror.argtypes = [ip]
@@ -242,6 +243,12 @@ class Beamformer:
         st = torch.cuda.current_stream(rf.device) if stream is None else stream
         self._check(self._L.pab_beamform(self._h, rf.data_ptr(), F, order, out.data_ptr(), st.cuda_stream), "pab_beamform")
         return out
+
+    def self_check(self, rf, order: int) -> int:
+        """pab_self_check: out-of-window shared-memory gathers of the diagonal kernel on one fp32 CUDA frame [1][N][S]."""
+        n = C.c_longlong(-1)
+        self._check(self._L.pab_self_check(self._h, rf.data_ptr(), order, C.byref(n)), "pab_self_check")
+        return int(n.value)
 
     def image_metrics(self, img, target, background, n_bins: int = 256, fwhm_row: int = -1, stream=None) -> dict:
         """pab_image_metrics on one CUDA image [nz][nx] float32; target / background = (r0, r1, c0, c1)."""

@@ -335,6 +335,24 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
     return PAB_OK;
 }
 
+int pab_self_check(pab_ctx* ctx, const float* rf_dev, int order, long long* violations) {
+    if (!ctx || !rf_dev || !violations || order < 1 || order > 5) return PAB_ERR_INVALID;
+    const DiagSet& D = ctx->diag[order <= 3 ? 0 : 1];
+    if (ctx->cache_mode == PAB_CACHE_OFF || D.smem_bytes == 0 || ctx->dtype != PAB_F32) return PAB_ERR_INVALID;
+    float* out = nullptr;
+    int* d_viol = nullptr;
+    int h = 0;
+    cudaError_t e = cudaMalloc(&out, (size_t)ctx->grid.nz * ctx->grid.nx * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&d_viol, 4);
+    if (e == cudaSuccess) e = cudaMemset(d_viol, 0, 4);
+    if (e == cudaSuccess) e = xl_diag_check(order, D, rf_dev, out, ctx->N, ctx->S, ctx->grid.nx, ctx->grid.nz, d_viol, 0);
+    if (e == cudaSuccess) { ctx->launches++; e = cudaMemcpy(&h, d_viol, 4, cudaMemcpyDeviceToHost); }
+    cudaFree(out); cudaFree(d_viol);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "self check");
+    *violations = h;
+    return PAB_OK;
+}
+
 int pab_set_interp(pab_ctx* ctx, int interp) {
     if (!ctx || (interp != PAB_INTERP_LINEAR && interp != PAB_INTERP_NEAREST)) return PAB_ERR_INVALID;
     if (interp == PAB_INTERP_NEAREST) {

@@ -91,10 +91,13 @@ template <typename T> __device__ __forceinline__ float diag_ld(const T* p) { ret
 // K: order 1..5.  NPG: pixel groups of 4 per thread (P = 4 NPG pixels: 4 for orders 1..3, 2 for orders 4, 5).
 // T: float or int16_t (the caller's frame, read in place).  CTAs of up to 16 warps at 128 registers (NPG = 4) or up to 8
 // warps at 80 registers, three CTAs per SM (NPG = 2).
-template <int K, int NPG, typename T>
+// CHK (pab_self_check): every shared-memory gather of the element loop is compared with the staged window of its quad and
+// out-of-window accesses are counted in *viol (compute-sanitizer is closed on this GPU pool; this kernel's addressing is
+// the most intricate of the library).
+template <int K, int NPG, typename T, bool CHK = false>
 __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T* __restrict__ rf, float* __restrict__ out,
                                                                           const DiagCfg C, const DiagTables D, int N, int S,
-                                                                          int nx, int nz, float scale) {
+                                                                          int nx, int nz, float scale, int* __restrict__ viol = nullptr) {
     constexpr int P = 4 * NPG;
     extern __shared__ __align__(128) unsigned char dg_smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -104,7 +107,9 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
     // [NPG + 1 spare][quads][NPG + 1 spare] shared address of sample 0 of each staged quad (the spares are never used
     // for loads: the blocks that would are skipped; they keep the index arithmetic free of clamps)
     int* s_base = reinterpret_cast<int*>(dg_smem) + (NPG + 1);
-    const uint32_t stage0 = smem_u32(dg_smem) + (((C.quads + 2 * (NPG + 1)) * 4 + 127) & ~127);
+    const int head_bytes = ((C.quads + 2 * (NPG + 1) + (CHK ? 2 * C.quads : 0)) * 4 + 127) & ~127;
+    int* s_lim = s_base + C.quads + (NPG + 1);                               // CHK: [quads][2] window limits
+    const uint32_t stage0 = smem_u32(dg_smem) + head_bytes;
     const int* qw0 = D.qw0 + (size_t)tile * C.quads;
     const int* qoff = D.qoff + (size_t)tile * (C.quads + 1);
 
@@ -113,6 +118,7 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
     for (int sq = warp; sq < C.quads; sq += n_warps) {
         const int w0 = __ldg(qw0 + sq), o0 = __ldg(qoff + sq), len = (__ldg(qoff + sq + 1) - o0) >> 4;
         if (lane == 0) s_base[sq] = (int)(stage0 + o0) - w0 * 16;
+        if (CHK && lane == 0) { s_lim[2 * sq] = (int)(stage0 + o0); s_lim[2 * sq + 1] = (int)(stage0 + o0) + len * 16 - 32; }
         const bool real = sq >= 1 && sq <= C.quads - 2;
         const T* ch0 = fr + (size_t)((sq - 1) * 4) * S + w0;
         for (int s0 = 0; s0 < len; s0 += 64) {                               // two samples per lane in flight
@@ -177,6 +183,14 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
                 if constexpr (GUARD) {
                     if (!(eg + cg + 1 >= 0 && eg + cg < n_quads_real)) { have = false; continue; }      // no channel of the block is real
                 }
+                if constexpr (CHK) {          // both quads of the block: [first byte, last 32-byte pair] of their staged windows
+#pragma unroll
+                    for (int k = 0; k < (r != 0 ? 2 : 1); ++k) {
+                        const int sq = eg + cg + k + 1, a = qb[cg + k] + (int)off;
+                        const int* lim = s_lim + 2 * sq;
+                        if (a < lim[0] || a > lim[1]) atomicAdd(viol, 1);
+                    }
+                }
                 if (GUARD ? !have : (cg == 0 || r == 0)) { lo0 = lds128((uint32_t)qb[cg] + off); lo1 = lds128((uint32_t)qb[cg] + off + 16); }
                 float4 hi0 = lo0, hi1 = lo1;
                 if constexpr (r != 0) { hi0 = lds128((uint32_t)qb[cg + 1] + off); hi1 = lds128((uint32_t)qb[cg + 1] + off + 16); }
@@ -210,7 +224,7 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
 
     // ---- partial power sums of the parts meet in shared memory (the staging area is dead now) ----
     __syncthreads();
-    float* red = reinterpret_cast<float*>(dg_smem + (((C.quads + 2 * (NPG + 1)) * 4 + 127) & ~127));       // [part][warp of the part][P][K][32]
+    float* red = reinterpret_cast<float*>(dg_smem + head_bytes);       // [part][warp of the part][P][K][32]
     {
         float* mine = red + (size_t)((part * C.wpp + wph) * P * K) * 32 + lane;
 #pragma unroll

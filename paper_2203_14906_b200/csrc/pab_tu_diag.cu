@@ -61,6 +61,23 @@ cudaError_t diag_attr(int smem_optin) {
 
 }  // namespace
 
+// pab_self_check: one frame through the checking instantiation (orders <= 3: K = 3; orders 4, 5: K = 5), float input
+cudaError_t xl_diag_check(int order, const DiagSet& D, const float* rf, float* out, int N, int S, int nx, int nz, int* d_viol,
+                          cudaStream_t st) {
+    dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, 1);
+    const DiagTables tabs{D.taps, D.qw0, D.qoff};
+    const size_t smem = (size_t)D.smem_bytes + 2 * D.cfg.quads * 4 + 128;
+    cudaError_t e;
+    if (order <= 3) {
+        if ((e = cudaFuncSetAttribute(bf_diag_kernel<3, 4, float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        bf_diag_kernel<3, 4, float, true><<<grid, D.cfg.wpp * D.cfg.parts * 32, smem, st>>>(rf, out, D.cfg, tabs, N, S, nx, nz, 1.0f, d_viol);
+    } else {
+        if ((e = cudaFuncSetAttribute(bf_diag_kernel<5, 2, float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        bf_diag_kernel<5, 2, float, true><<<grid, D.cfg.wpp * D.cfg.parts * 32, smem, st>>>(rf, out, D.cfg, tabs, N, S, nx, nz, 1.0f, d_viol);
+    }
+    return cudaGetLastError();
+}
+
 cudaError_t xl_diag_configure(int smem_optin) {
     cudaError_t e;
     if ((e = diag_attr<1, 4>(smem_optin)) != cudaSuccess) return e;

@@ -641,6 +641,25 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
             ref = orc.beamform(rf, g, order, scale=scale)
             for f in range(frames):
                 assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
+        if dtype == "float32":                 # every shared-memory gather inside the staged window of its quad
+            for order in (3, 5):
+                if order <= n_elem:
+                    assert bf.self_check(torch.from_numpy(rf[:1]).cuda(), order) == 0
+    finally:
+        bf.close()
+
+
+@pytest.mark.parametrize("cfg,order", [("C2", 3), ("C4", 5), ("C3", 1), ("C5", 4)])
+def test_diagonal_kernel_self_check_named_geometries(pab, cfg, order):
+    """pab_self_check on the geometries of the named configs (C5's with fp32 frames): no gather of the diagonal kernel
+    leaves the staged window of its channel quad (the check compute-sanitizer would make; it is closed on this pool)."""
+    g = synth.geometry(cfg)
+    rng = np.random.default_rng(3)
+    rf = rng.standard_normal((1, g.n_elem, g.n_samp)).astype(np.float32)
+    bf = pab.Beamformer(g, delay_cache="single")
+    try:
+        assert bf.plan()["diagonal"] == 1
+        assert bf.self_check(torch.from_numpy(rf).cuda(), order) == 0
     finally:
         bf.close()
 
