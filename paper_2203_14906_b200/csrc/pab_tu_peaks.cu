@@ -99,7 +99,11 @@ extern "C" int pab_measure_peaks(double* out, int n_out) {
     float* d_sink = nullptr;
     long long* h_cyc = new long long[sms];
     cudaEvent_t e0, e1;
-    if (cudaMalloc(&d_cyc, sms * sizeof(long long)) != cudaSuccess || cudaMalloc(&d_sink, 64) != cudaSuccess) return PAB_ERR_ALLOC;
+    if (cudaMalloc(&d_cyc, sms * sizeof(long long)) != cudaSuccess || cudaMalloc(&d_sink, 64) != cudaSuccess) {
+        cudaFree(d_cyc); cudaFree(d_sink); delete[] h_cyc;
+        cudaGetLastError();
+        return PAB_ERR_ALLOC;
+    }
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     auto cyc = [&]() { cudaMemcpy(h_cyc, d_cyc, sms * sizeof(long long), cudaMemcpyDeviceToHost); return slowest(h_cyc, sms); };
     for (int rep = 0; rep < 2; ++rep) {          // first pass warms clocks and caches
