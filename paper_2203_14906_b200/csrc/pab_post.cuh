@@ -5,6 +5,7 @@
 //   y[m] = sum_{t<T} h[t] x[m + T/2 - t]      (A11, A12)      q[m] = sum_{t'} g[t'] y[m + L - t']   (A9)
 //   env = sqrt(y^2 + q^2), per-frame max by atomicMax on the bit pattern.
 #pragma once
+#include <cuda.h>            // CUtensorMap (the encode function itself is fetched through the runtime, no libcuda link)
 #include <cuda_runtime.h>
 #include "pab_math.cuh"
 #include "pab_pipe.cuh"   // mbarrier / bulk-copy helpers
@@ -229,11 +230,21 @@ __device__ __forceinline__ void fir_hilbert64(const float* base, const PostTaps6
 
 constexpr int kPostFastTZ = 256;
 
+// 3-D tiled TMA load of a box of rows x 32 columns of frame f, first row r (may be negative), first column c; rows and
+// columns outside the image arrive as zeros.
+__device__ __forceinline__ void tma_box(uint32_t dst, const CUtensorMap* tm, int c, int r, int f, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(dst), "l"(tm), "r"(c), "r"(r), "r"(f), "r"(bar) : "memory");
+}
+
 // grid: (ceil(nx/32), ceil(nz/TZ), F), 256 threads; lanes own columns.
-// BULK (nx a multiple of 32): the tile rows (128 B each) come in as 1-D TMA bulk copies on one mbarrier, rows outside
-// the image are zero-filled by hand; otherwise plain predicated loads.
-template <int TZ, bool ENV, int HPAR, bool BULK>
-__global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, const __grid_constant__ PostTaps64 T) {
+// LD = 2 (rows of a multiple of 16 bytes at a 16-byte aligned address): the tile comes in as two boxes of a tiled TMA
+// tensor copy over the [F][nz][nx] image (one thread issues both; the halo outside the image is zero-filled by the copy
+// engine).  LD = 1 (nx a multiple of 32, no tensor map): one 1-D bulk copy per 128-byte tile row -- 350 copies issued lane
+// by lane, a fifth of the CTA's time.  LD = 0: plain predicated loads.
+template <int TZ, bool ENV, int HPAR, int LD>
+__global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, const __grid_constant__ PostTaps64 T,
+                                                          const __grid_constant__ CUtensorMap TM) {
     extern __shared__ __align__(128) float post64_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int col0 = blockIdx.x * 32, r0 = blockIdx.y * TZ, f = blockIdx.z;
@@ -242,10 +253,23 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
     constexpr int YR = ENV ? ((TZ + 63 + 7) & ~7) : TZ;
     const int xr0 = yr0 + P.shiftB - 63;                     // first x row those need
     constexpr int XR = YR + 63;
-    float* xs = post64_smem;            // [XR][32]
-    float* ys = xs + XR * 32;           // [YR][32]   (ENV only)
+    constexpr int XRA = XR + 1;         // two TMA boxes of XRA / 2 rows
+    float* xs = post64_smem;            // [XRA][32]
+    float* ys = xs + XRA * 32;          // [YR][32]   (ENV only)
     const float* img = P.x + (size_t)f * P.nz * P.nx;
-    if constexpr (BULK) {
+    if constexpr (LD == 2) {
+        __shared__ __align__(8) unsigned long long bar;
+        const uint32_t barA = smem_u32(&bar);
+        if (threadIdx.x == 0) {
+            mbar_init(barA, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            mbar_arrive_expect_tx(barA, (uint32_t)XRA * 128u);
+            tma_box(smem_u32(xs), &TM, col0, xr0, f, barA);
+            tma_box(smem_u32(xs) + (XRA / 2) * 128, &TM, col0, xr0 + XRA / 2, f, barA);
+        }
+        __syncthreads();
+        mbar_wait(barA, 0);
+    } else if constexpr (LD == 1) {
         __shared__ __align__(8) unsigned long long bar;
         const uint32_t barA = smem_u32(&bar);
         const int lo = max(0, -xr0), hi = min(XR, P.nz - xr0);           // tile rows [lo, hi) lie inside the image
@@ -334,12 +358,16 @@ __global__ void __launch_bounds__(256) post_fir64_kernel(const PostParams P, con
     }
 }
 
+inline int post64_box_rows(bool env) {
+    const int YR = env ? ((kPostFastTZ + 63 + 7) & ~7) : kPostFastTZ;
+    return (YR + 64) / 2;
+}
 inline size_t post64_smem_bytes(bool env) {
     const int YR = env ? ((kPostFastTZ + 63 + 7) & ~7) : kPostFastTZ;
-    return ((size_t)(YR + 63) * 32 + (env ? (size_t)YR * 32 : 0)) * 4;
+    return ((size_t)(YR + 64) * 32 + (env ? (size_t)YR * 32 : 0)) * 4;
 }
 
-template <bool BULK>
+template <int BULK>
 inline cudaError_t post64_configure_b(int smem_optin) {
     cudaError_t e;
     smem_optin = (int)post64_smem_bytes(true);   // what the kernels use (the bulk variant adds a static mbarrier)
@@ -350,25 +378,52 @@ inline cudaError_t post64_configure_b(int smem_optin) {
 }
 
 inline cudaError_t post64_configure(int smem_optin) {
-    cudaError_t e = post64_configure_b<false>(smem_optin);
-    return e != cudaSuccess ? e : post64_configure_b<true>(smem_optin);
+    cudaError_t e = post64_configure_b<0>(smem_optin);
+    if (e == cudaSuccess) e = post64_configure_b<1>(smem_optin);
+    return e != cudaSuccess ? e : post64_configure_b<2>(smem_optin);
 }
 
-template <bool BULK>
-inline void launch_post64_b(const PostParams& Q, const PostTaps64& T, bool env, int hpar, int F, cudaStream_t st) {
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libpab.so does not link libcuda); nullptr: unavailable
+using TensorMapEncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+inline TensorMapEncodeFn tensor_map_encode_fn() {
+    static const TensorMapEncodeFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return reinterpret_cast<TensorMapEncodeFn>(p);
+    }();
+    return fn;
+}
+// tensor map of the [F][nz][nx] fp32 image with boxes of box_rows x 32 columns; false: not expressible / no driver support
+inline bool post64_tensor_map(const float* x, int nx, int nz, int F, int box_rows, CUtensorMap* tm) {
+    const TensorMapEncodeFn enc = tensor_map_encode_fn();
+    if (!enc || nx % 4 != 0 || (reinterpret_cast<uintptr_t>(x) & 15) != 0) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)nz, (cuuint64_t)F};
+    const cuuint64_t strides[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * nz * 4};
+    const cuuint32_t box[3] = {32, (cuuint32_t)box_rows, 1}, estr[3] = {1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(x), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int LD>
+inline void launch_post64_b(const PostParams& Q, const PostTaps64& T, const CUtensorMap& tm, bool env, int hpar, int F, cudaStream_t st) {
     dim3 grid((Q.nx + 31) / 32, (Q.nz + kPostFastTZ - 1) / kPostFastTZ, F);
     const size_t sm = post64_smem_bytes(env);
-    if (!env) post_fir64_kernel<kPostFastTZ, false, 2, BULK><<<grid, 256, sm, st>>>(Q, T);
-    else if (hpar == 0) post_fir64_kernel<kPostFastTZ, true, 0, BULK><<<grid, 256, sm, st>>>(Q, T);
-    else if (hpar == 1) post_fir64_kernel<kPostFastTZ, true, 1, BULK><<<grid, 256, sm, st>>>(Q, T);
-    else post_fir64_kernel<kPostFastTZ, true, 2, BULK><<<grid, 256, sm, st>>>(Q, T);
+    if (!env) post_fir64_kernel<kPostFastTZ, false, 2, LD><<<grid, 256, sm, st>>>(Q, T, tm);
+    else if (hpar == 0) post_fir64_kernel<kPostFastTZ, true, 0, LD><<<grid, 256, sm, st>>>(Q, T, tm);
+    else if (hpar == 1) post_fir64_kernel<kPostFastTZ, true, 1, LD><<<grid, 256, sm, st>>>(Q, T, tm);
+    else post_fir64_kernel<kPostFastTZ, true, 2, LD><<<grid, 256, sm, st>>>(Q, T, tm);
 }
 
-// bulk row copies need 128-byte rows of whole tiles at 16-byte aligned addresses
 inline void launch_post64(const PostParams& Q, const PostTaps64& T, bool env, int hpar, int F, cudaStream_t st) {
-    const bool bulk = Q.nx % 32 == 0 && (reinterpret_cast<uintptr_t>(Q.x) & 15) == 0;
-    if (bulk) launch_post64_b<true>(Q, T, env, hpar, F, st);
-    else launch_post64_b<false>(Q, T, env, hpar, F, st);
+    alignas(64) CUtensorMap tm{};
+    if (post64_tensor_map(Q.x, Q.nx, Q.nz, F, post64_box_rows(env), &tm)) launch_post64_b<2>(Q, T, tm, env, hpar, F, st);
+    // bulk row copies need 128-byte rows of whole tiles at 16-byte aligned addresses
+    else if (Q.nx % 32 == 0 && (reinterpret_cast<uintptr_t>(Q.x) & 15) == 0) launch_post64_b<1>(Q, T, tm, env, hpar, F, st);
+    else launch_post64_b<0>(Q, T, tm, env, hpar, F, st);
 }
 
 }  // namespace pab
