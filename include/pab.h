@@ -33,6 +33,7 @@ extern "C" {
 #define PAB_ERR_DEVICE   (-2)   /* no CUDA device, or the current device is not compute capability 10.x           */
 #define PAB_ERR_ALLOC    (-3)   /* device or pinned-host allocation failed                                        */
 #define PAB_ERR_CUDA     (-4)   /* a CUDA call or kernel launch failed (see pab_last_cuda_error)                  */
+#define PAB_ERR_LIMIT    (-5)   /* a size beyond the fixed maximum of a no-allocation entry point (pab_post_no_alloc) */
 
 /* input sample type (pab_set_input) */
 #define PAB_F32 0
@@ -263,6 +264,27 @@ typedef struct {
  */
 int pab_image_metrics(pab_ctx* ctx, const float* img_dev, const pab_roi* target, const pab_roi* background, int n_bins,
                       int fwhm_row, pab_metrics* out_host, void* cuda_stream);
+
+/*
+ * pab_post_no_alloc -- the post chain of the context (a7..a9: band-pass, Hilbert envelope, and under PAB_LOG the log
+ * compression) on images the caller already holds, for callers that must not allocate (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Calls no cudaMalloc / cudaFree and no
+ * allocating library routine: the only scratch of the chain, the per-frame envelope maxima, lives in a fixed
+ * file-scope device array of PAB_NO_ALLOC_MAX_FRAMES entries (4 KiB, held by every GPU that loads the library until the
+ * process exits).  Enqueues one memset and the kernels on `cuda_stream`; never synchronises.
+ *   img_dev   device pointer, [n_frames][nz][nx] fp32 beamformed images (what pab_beamform writes under PAB_RAW); read only
+ *   n_frames  1..PAB_NO_ALLOC_MAX_FRAMES; more is rejected with PAB_ERR_LIMIT (nothing launched; the message of
+ *             pab_last_cuda_error names the limit)
+ *   out_dev   device pointer, [n_frames][nz][nx] fp32, caller-owned, must not overlap img_dev; holds what pab_beamform
+ *             would have written under the context's post mode
+ * The context must be in PAB_ENVELOPE or PAB_LOG mode with filters of 33..64 taps each (after padding to 8).
+ * All calls on one GPU share the array, which keeps the last call's values (the entry point clears what it uses on its
+ * stream first): calls that overlap on the GPU -- two streams, two contexts, two threads -- race on it.
+ * Errors: PAB_ERR_INVALID (null / misaligned / overlapping pointers, mode or filter length not covered, wrong current
+ * device), PAB_ERR_LIMIT, PAB_ERR_CUDA.
+ */
+#define PAB_NO_ALLOC_MAX_FRAMES 1024
+int pab_post_no_alloc(pab_ctx* ctx, const float* img_dev, int n_frames, float* out_dev, void* cuda_stream);
 
 /* pab_strerror -- static string for an error code.  pab_last_cuda_error -- the last cudaError_t string seen
  * by this context ("" if none). */

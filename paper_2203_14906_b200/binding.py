@@ -12,7 +12,8 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpab.so")
 
-OK, ERR_INVALID, ERR_DEVICE, ERR_ALLOC, ERR_CUDA = 0, -1, -2, -3, -4
+OK, ERR_INVALID, ERR_DEVICE, ERR_ALLOC, ERR_CUDA, ERR_LIMIT = 0, -1, -2, -3, -4, -5
+NO_ALLOC_MAX_FRAMES = 1024      # PAB_NO_ALLOC_MAX_FRAMES
 F32, I16 = 0, 1
 RAW, BANDPASS, ENVELOPE, LOG = 0, 1, 2, 3
 VARIANT_AUTO, VARIANT_DIRECT, VARIANT_STAGED = 0, 1, 2
@@ -25,7 +26,7 @@ _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_S
 # every symbol include/pab.h declares
 SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_delay_cache", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
-           "pab_launch_count", "pab_measure_peaks", "pab_self_check", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
+           "pab_launch_count", "pab_measure_peaks", "pab_self_check", "pab_post_no_alloc", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
 
 class Grid(C.Structure):
@@ -93,6 +94,7 @@ def load(build_if_missing: bool = False):
     L.pab_image_metrics.argtypes = [vp, vp, C.POINTER(Roi), C.POINTER(Roi), ip, ip, C.POINTER(Metrics), vp]
     L.pab_measure_peaks.argtypes = [C.POINTER(C.c_double), ip]
     L.pab_self_check.argtypes = [vp, vp, ip, C.POINTER(C.c_longlong)]
+    L.pab_post_no_alloc.argtypes = [vp, vp, ip, vp, vp]
     L.pab_set_profile.argtypes = [vp, ip]
     L.pab_get_profile.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_longlong), ip]
     L.pab_strerror.argtypes = [ip]
@@ -249,6 +251,18 @@ class Beamformer:
         n = C.c_longlong(-1)
         self._check(self._L.pab_self_check(self._h, rf.data_ptr(), order, C.byref(n)), "pab_self_check")
         return int(n.value)
+
+    def post_no_alloc(self, img, out, stream=None):
+        """pab_post_no_alloc: the context's post chain (ENVELOPE / LOG) on CUDA images [F][nz][nx] float32 -> out (same
+        shape, caller-allocated, not overlapping img); allocates nothing (fixed scratch array, F <= NO_ALLOC_MAX_FRAMES)."""
+        import torch
+        g = self.geom
+        F = img.shape[0]
+        for t in (img, out):
+            assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32 and tuple(t.shape) == (F, g.nz, g.nx)
+        st = torch.cuda.current_stream(img.device) if stream is None else stream
+        self._check(self._L.pab_post_no_alloc(self._h, img.data_ptr(), F, out.data_ptr(), st.cuda_stream), "pab_post_no_alloc")
+        return out
 
     def image_metrics(self, img, target, background, n_bins: int = 256, fwhm_row: int = -1, stream=None) -> dict:
         """pab_image_metrics on one CUDA image [nz][nx] float32; target / background = (r0, r1, c0, c1)."""

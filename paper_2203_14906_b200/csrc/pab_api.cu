@@ -142,6 +142,7 @@ const char* pab_strerror(int code) {
     case PAB_ERR_DEVICE: return "no usable sm_100 CUDA device";
     case PAB_ERR_ALLOC: return "allocation failed";
     case PAB_ERR_CUDA: return "CUDA call failed";
+    case PAB_ERR_LIMIT: return "size beyond the fixed maximum of a no-allocation entry point";
     default: return "unknown error code";
     }
 }
@@ -210,6 +211,9 @@ int pab_create(pab_ctx** out, int n_elem, int n_samp, float fs_hz, float c_m_s, 
     if (rc == PAB_OK) rc = xl_staged_configure(ctx->smem_optin);
     if (rc == PAB_OK && xl_post_configure(ctx->smem_optin) != cudaSuccess) rc = PAB_ERR_CUDA;
     if (rc != PAB_OK) { free_all(ctx); delete ctx; return rc; }
+    // set-up of pab_post_no_alloc: the address of its fixed scratch array on this device.  A failure here is reported by
+    // that entry point (which retries), not by pab_create.
+    if (xl_post_no_alloc_setup(nullptr) != cudaSuccess) cudaGetLastError();
     *out = ctx;
     return PAB_OK;
 }
@@ -432,6 +436,34 @@ int pab_set_post(pab_ctx* ctx, int mode, float f_center_hz, float f_halfwidth_hz
     }
     ctx->post_mode = mode; ctx->n_taps_bp = n_taps_bp; ctx->n_taps_h = n_taps_hilbert;
     ctx->TpB = TpB; ctx->TpH = TpH; ctx->dyn_range_db = dyn_range_db;
+    return PAB_OK;
+}
+
+int pab_post_no_alloc(pab_ctx* ctx, const float* img_dev, int n_frames, float* out_dev, void* cuda_stream) {
+    if (!ctx || !img_dev || !out_dev || n_frames < 1) return PAB_ERR_INVALID;
+    if (((uintptr_t)img_dev % 4) != 0 || ((uintptr_t)out_dev % 4) != 0) return PAB_ERR_INVALID;
+    if (n_frames > PAB_NO_ALLOC_MAX_FRAMES) {
+        snprintf(ctx->err, sizeof ctx->err, "pab_post_no_alloc: n_frames = %d exceeds PAB_NO_ALLOC_MAX_FRAMES = %d (fixed scratch array)",
+                 n_frames, PAB_NO_ALLOC_MAX_FRAMES);
+        return PAB_ERR_LIMIT;
+    }
+    if (ctx->post_mode < PAB_ENVELOPE || !ctx->post_fast) return PAB_ERR_INVALID;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device) return PAB_ERR_INVALID;
+    const int nx = ctx->grid.nx, nz = ctx->grid.nz;
+    const size_t bytes = (size_t)n_frames * nz * (size_t)nx * 4;
+    const uintptr_t a = (uintptr_t)img_dev, b = (uintptr_t)out_dev;
+    if (a < b + bytes && b < a + bytes) return PAB_ERR_INVALID;          // the FIR tiles read their neighbours' rows
+    PostParams Q{};
+    Q.x = img_dev; Q.out = out_dev;
+    Q.TpB = ctx->TpB; Q.shiftB = ctx->n_taps_bp / 2;
+    Q.TpH = ctx->TpH; Q.shiftH = (ctx->n_taps_h - 1) / 2;
+    Q.nx = nx; Q.nz = nz;
+    int launches = 0;
+    const cudaError_t e = xl_post_no_alloc(Q, ctx->taps64, ctx->hilbert_parity, n_frames, ctx->post_mode == PAB_LOG, ctx->dyn_range_db,
+                                           (cudaStream_t)cuda_stream, &launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "pab_post_no_alloc");
+    ctx->launches += launches;
     return PAB_OK;
 }
 

@@ -47,6 +47,9 @@ void xl_nearest_direct(int order, int nq, const BfParams& P, int groups, const u
 cudaError_t xl_post_configure(int smem_optin);
 void xl_post64(const PostParams& Q, const PostTaps64& T, bool env, int hpar, int F, cudaStream_t st);
 void xl_post_generic(const PostParams& Q, bool env, int F, cudaStream_t st);
+// no-allocation post chain (pab_post_no_alloc): frame maxima in a file-scope device array of pab_tu_post.cu
+cudaError_t xl_post_no_alloc_setup(unsigned int** ptr_out);
+cudaError_t xl_post_no_alloc(PostParams Q, const PostTaps64& T, int hpar, int F, bool log, float dr, cudaStream_t st, int* launches);
 void xl_post_log(float* out, const unsigned int* frame_max, int npix, int F, float dr, cudaStream_t st);
 int xl_metrics(const float* img, int nx, const RoiPair& R, MetricAcc* acc, unsigned int* hist, int n_bins, int fwhm_row,
                double* fw, cudaStream_t st);        // returns the number of kernels launched

@@ -1,9 +1,53 @@
 // pab_tu_post.cu -- translation unit: post chain (a7..a9) and image metrics (row f3).
+#include <mutex>
 #include "pab_post.cuh"
 #include "pab_metrics.cuh"
 #include "pab_launch.h"
 
+// Scratch of pab_post_no_alloc: the per-frame envelope maxima (a8 -> a9) live in this fixed array instead of a buffer
+// from cudaMalloc.  Every GPU that loads libpab.so holds its 4 KiB until the process exits.  Every call on a device shares
+// it (it keeps the last call's values: the entry point clears the frames it uses on its stream before the FIR kernel),
+// so two calls that overlap on one GPU race.  In host code the name is a stand-in, not a device address: the kernels get
+// the address cudaGetSymbolAddress returns for the current device (xl_post_no_alloc_setup).
+static __device__ __align__(256) unsigned int pab_no_alloc_frame_max[PAB_NO_ALLOC_MAX_FRAMES];
+
 namespace pab {
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_no_alloc_mutex;
+unsigned int* g_no_alloc_ptr[kNoAllocMaxDevices];     // device address of pab_no_alloc_frame_max on device [i], once resolved
+}  // namespace
+
+// Once per device, with that device current (pab_create calls it; idempotent): resolves the scratch array's address.
+cudaError_t xl_post_no_alloc_setup(unsigned int** ptr_out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_no_alloc_mutex);
+    if (!g_no_alloc_ptr[dev]) {
+        unsigned int* p = nullptr;
+        if ((e = cudaGetSymbolAddress((void**)&p, pab_no_alloc_frame_max)) != cudaSuccess) return e;
+        g_no_alloc_ptr[dev] = p;
+    }
+    if (ptr_out) *ptr_out = g_no_alloc_ptr[dev];
+    return cudaSuccess;
+}
+
+// Band-pass + envelope (+ log) of F <= PAB_NO_ALLOC_MAX_FRAMES frames with the frame maxima in the fixed array.  Q.frame_max
+// is ignored.  No allocation: a memset and two (one) launches on st.  Returns the number of kernels through *launches.
+cudaError_t xl_post_no_alloc(PostParams Q, const PostTaps64& T, int hpar, int F, bool log, float dr, cudaStream_t st, int* launches) {
+    unsigned int* fmax = nullptr;
+    cudaError_t e = xl_post_no_alloc_setup(&fmax);
+    if (e != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(fmax, 0, (size_t)F * sizeof(unsigned int), st)) != cudaSuccess) return e;
+    Q.frame_max = fmax;
+    launch_post64(Q, T, true, hpar, F, st);
+    if (log) launch_post_log(Q.out, fmax, Q.nx * Q.nz, F, dr, st);
+    *launches = log ? 2 : 1;
+    return cudaGetLastError();
+}
 
 cudaError_t xl_post_configure(int smem_optin) {
     cudaError_t e;
