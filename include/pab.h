@@ -187,6 +187,20 @@ int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int order, floa
  */
 int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host);
 
+/*
+ * pab_beamform_host_async / pab_host_sync -- the streaming form of pab_beamform_host: enqueues the copies and kernels of
+ * the call on the context's internal streams and returns; pab_host_sync waits for everything enqueued so far.
+ * Successive calls overlap one another (host-to-device copy of call i + 1, kernels of call i and device-to-host copy of
+ * call i - 1 run side by side on two device buffer sets), so a stream of 64-frame batches runs at the rate of its slowest
+ * leg -- at C2b the host-to-device copy -- where the blocking call pays its own ramp-up and drain every time.
+ *   rf_host, out_host   as for pab_beamform_host, but PINNED (cudaHostAlloc / cudaHostRegister) for the copies to be
+ *                       asynchronous, and kept alive and unmodified (rf) / unread (out) until pab_host_sync returns
+ * Between the first call and pab_host_sync the context's settings must not change and pab_beamform must not be called on
+ * it (shared scratch).  Errors: as pab_beamform_host; an error of the asynchronous work surfaces at pab_host_sync.
+ */
+int pab_beamform_host_async(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host);
+int pab_host_sync(pab_ctx* ctx);
+
 /* pab_destroy -- free the context and everything it owns.  NULL is a no-op.  Synchronises the device. */
 void pab_destroy(pab_ctx* ctx);
 

@@ -24,7 +24,7 @@ _MODES = {"raw": RAW, "bandpass": BANDPASS, "envelope": ENVELOPE, "log": LOG}
 _VARIANTS = {"auto": VARIANT_AUTO, "direct": VARIANT_DIRECT, "staged": VARIANT_STAGED}
 
 # every symbol include/pab.h declares
-SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_delay_cache", "pab_set_tuning", "pab_beamform", "pab_beamform_host",
+SYMBOLS = ["pab_create", "pab_set_input", "pab_set_post", "pab_set_variant", "pab_set_weight", "pab_set_interp", "pab_set_delay_cache", "pab_set_tuning", "pab_beamform", "pab_beamform_host", "pab_beamform_host_async", "pab_host_sync",
            "pab_destroy", "pab_plan", "pab_get_plan", "pab_design_bandpass", "pab_design_hilbert",
            "pab_launch_count", "pab_measure_peaks", "pab_self_check", "pab_post_no_alloc", "pab_image_metrics", "pab_set_profile", "pab_get_profile", "pab_strerror", "pab_last_cuda_error", "pab_version"]
 
@@ -83,6 +83,8 @@ def load(build_if_missing: bool = False):
     L.pab_set_tuning.argtypes = [vp, ip, ip, ip, ip]
     L.pab_beamform.argtypes = [vp, vp, ip, ip, vp, vp]
     L.pab_beamform_host.argtypes = [vp, vp, ip, ip, vp]
+    L.pab_beamform_host_async.argtypes = [vp, vp, ip, ip, vp]
+    L.pab_host_sync.argtypes = [vp]
     L.pab_destroy.argtypes = [vp]
     L.pab_destroy.restype = None
     L.pab_plan.argtypes = [ip, ip, fp, fp, fp, C.POINTER(Grid), ip, C.POINTER(PlanInfo)]
@@ -300,6 +302,23 @@ class Beamformer:
             src, dst = rf.ctypes.data, out.ctypes.data
         self._check(self._L.pab_beamform_host(self._h, src, F, order, dst), "pab_beamform_host")
         return out
+
+    def beamform_host_async(self, rf, order: int, out):
+        """pab_beamform_host_async: rf, out pinned CPU torch tensors ([F][N][S] -> [F][nz][nx]); enqueue only.  The caller
+        keeps both alive and untouched until host_sync() returns."""
+        import torch
+        g = self.geom
+        F = rf.shape[0]
+        assert isinstance(rf, torch.Tensor) and not rf.is_cuda and rf.is_contiguous() and rf.is_pinned()
+        assert tuple(rf.shape) == (F, g.n_elem, g.n_samp), rf.shape
+        assert rf.dtype == (torch.int16 if self.dtype == "int16" else torch.float32), rf.dtype
+        assert not out.is_cuda and out.is_contiguous() and out.is_pinned() and out.dtype == torch.float32
+        assert tuple(out.shape) == (F, g.nz, g.nx), out.shape
+        self._check(self._L.pab_beamform_host_async(self._h, rf.data_ptr(), F, order, out.data_ptr()), "pab_beamform_host_async")
+        return out
+
+    def host_sync(self):
+        self._check(self._L.pab_host_sync(self._h), "pab_host_sync")
 
     def close(self):
         if self._h:

@@ -14,6 +14,10 @@
 
 using namespace pab;
 
+// device buffer sets of the host path (pab_beamform_host*): with three, a whole-batch piece can be copied in, computed and
+// copied out at the same time without one leg waiting for the hand-over of the set two pieces back
+constexpr int kHostSets = 3;
+
 struct pab_ctx {
     int N = 0, S = 0, Sp = 0;
     float fs = 0, c = 0, pitch = 0;
@@ -54,11 +58,12 @@ struct pab_ctx {
     float* d_taps_h = nullptr;
     unsigned int* d_max = nullptr;   // [batch] per-frame max of the envelope
     // host-buffer path (lazy)
-    void* d_in[2] = {nullptr, nullptr};
-    float* d_out[2] = {nullptr, nullptr};
+    void* d_in[kHostSets] = {};
+    float* d_out[kHostSets] = {};
     cudaStream_t s_h2d = nullptr, s_run = nullptr, s_d2h = nullptr;
-    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_run[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    cudaEvent_t ev_in[kHostSets] = {}, ev_run[kHostSets] = {}, ev_out[kHostSets] = {};
     long long launches = 0;
+    long long host_it = 0;               // pieces the host path has enqueued so far (buffer set = host_it & 1)
     // per-launch device timing (pab_set_profile): events 2*slot, 2*slot+1 bracket launch `slot`
     bool profiling = false;
     std::vector<cudaEvent_t> prof_ev;
@@ -86,7 +91,7 @@ void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
     cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact); cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
     xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]);
-    for (int b = 0; b < 2; ++b) {
+    for (int b = 0; b < kHostSets; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
         if (ctx->ev_run[b]) cudaEventDestroy(ctx->ev_run[b]);

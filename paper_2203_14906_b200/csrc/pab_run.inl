@@ -167,22 +167,20 @@ extern "C" int pab_beamform(pab_ctx* ctx, const void* rf_dev, int n_frames, int 
     return PAB_OK;
 }
 
-extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host) {
-    int rc = check_args(ctx, rf_host, n_frames, order, out_host);
-    if (rc != PAB_OK) return rc;
-    // Host path batches: short calls are cut into 8-frame pieces so that H2D, kernels and D2H of successive pieces
-    // overlap inside one call (measured best at C2b, where the call is bound by the 35 GB/s host-to-device copy);
-    // long streams use 64-frame pieces (more tiles per launch, negligible ramp).
+namespace {
+
+// Enqueue the host path for one call on the context's three internal streams (H2D, kernels, D2H) with kHostSets device
+// buffer sets.  `ctx->host_it` counts pieces over the life of the context, so that the buffer hand-over events order successive
+// calls as well as successive pieces of one call.  B: frames per piece; ramp: half pieces at both ends of the call.
+int host_enqueue(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host, int B, bool ramp) {
     const int Bcap = ctx->plan.batch_frames < 64 ? ctx->plan.batch_frames : 64;
-    int B = (n_frames >= 256 || Bcap < 8) ? Bcap : 8;
-    if (ctx->tuning.host_batch_frames > 0) B = ctx->tuning.host_batch_frames < Bcap ? ctx->tuning.host_batch_frames : Bcap;
     const size_t frame_in = (size_t)ctx->N * ctx->S * elem_size(ctx->dtype);
     const size_t frame_out = (size_t)ctx->grid.nz * ctx->grid.nx * 4;
     if (!ctx->s_h2d) {
         PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
         PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_run, cudaStreamNonBlocking));
         PAB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < kHostSets; ++b) {
             PAB_CUDA(ctx, cudaMalloc(&ctx->d_in[b], (size_t)Bcap * ctx->N * ctx->S * 4));   // sized for fp32
             PAB_CUDA(ctx, cudaMalloc(&ctx->d_out[b], (size_t)Bcap * frame_out));
             PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_in[b], cudaEventDisableTiming));
@@ -190,22 +188,19 @@ extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames
             PAB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_out[b], cudaEventDisableTiming));
         }
     }
-    // Double-buffered: H2D of batch b+1 and D2H of batch b-1 overlap the kernels of batch b.
-    int it = 0;
-    // The first and the last piece are half pieces (when there are enough frames): the pipeline starts computing and
-    // starts its last device-to-host copy sooner.
-    const bool ramp = B >= 8 && n_frames >= 4 * B;
-    for (int f0 = 0, F = 0; f0 < n_frames; f0 += F, ++it) {
+    // H2D of piece b+1 and D2H of piece b-1 overlap the kernels of piece b.
+    for (int f0 = 0, F = 0; f0 < n_frames; f0 += F, ++ctx->host_it) {
         F = n_frames - f0 < B ? n_frames - f0 : B;
         if (ramp && (f0 == 0 || n_frames - f0 <= B)) F = (f0 == 0 || n_frames - f0 > B / 2) ? B / 2 : n_frames - f0;
-        const int b = it & 1;
-        if (it >= 2) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_run[b], 0));   // d_in[b] consumed
+        const long long it = ctx->host_it;
+        const int b = (int)(it % kHostSets);
+        if (it >= kHostSets) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_run[b], 0));   // d_in[b] consumed
         PAB_CUDA(ctx, cudaMemcpyAsync(ctx->d_in[b], (const char*)rf_host + (size_t)f0 * frame_in, (size_t)F * frame_in,
                                       cudaMemcpyHostToDevice, ctx->s_h2d));
         PAB_CUDA(ctx, cudaEventRecord(ctx->ev_in[b], ctx->s_h2d));
         PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_run, ctx->ev_in[b], 0));
-        if (it >= 2) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_run, ctx->ev_out[b], 0));   // d_out[b] drained
-        rc = run_batch(ctx, ctx->d_in[b], F, order, ctx->d_out[b], ctx->s_run);
+        if (it >= kHostSets) PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_run, ctx->ev_out[b], 0));   // d_out[b] drained
+        const int rc = run_batch(ctx, ctx->d_in[b], F, order, ctx->d_out[b], ctx->s_run);
         if (rc != PAB_OK) return rc;
         PAB_CUDA(ctx, cudaEventRecord(ctx->ev_run[b], ctx->s_run));
         PAB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_run[b], 0));
@@ -213,7 +208,42 @@ extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames
                                       cudaMemcpyDeviceToHost, ctx->s_d2h));
         PAB_CUDA(ctx, cudaEventRecord(ctx->ev_out[b], ctx->s_d2h));
     }
+    return PAB_OK;
+}
+
+}  // namespace
+
+extern "C" int pab_host_sync(pab_ctx* ctx) {
+    if (!ctx) return PAB_ERR_INVALID;
+    if (!ctx->s_h2d) return PAB_OK;
     PAB_CUDA(ctx, cudaStreamSynchronize(ctx->s_d2h));
     PAB_CUDA(ctx, cudaStreamSynchronize(ctx->s_run));
     return PAB_OK;
+}
+
+extern "C" int pab_beamform_host(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host) {
+    int rc = check_args(ctx, rf_host, n_frames, order, out_host);
+    if (rc != PAB_OK) return rc;
+    // Host path batches: short calls are cut into 8-frame pieces so that H2D, kernels and D2H of successive pieces
+    // overlap inside one call (the call ends with its last piece's kernels and copy, which nothing overlaps: small pieces
+    // keep that tail short); long streams use 64-frame pieces (more tiles per launch, negligible ramp).
+    const int Bcap = ctx->plan.batch_frames < 64 ? ctx->plan.batch_frames : 64;
+    int B = (n_frames >= 256 || Bcap < 8) ? Bcap : 8;
+    if (ctx->tuning.host_batch_frames > 0) B = ctx->tuning.host_batch_frames < Bcap ? ctx->tuning.host_batch_frames : Bcap;
+    // The first and the last piece are half pieces (when there are enough frames): the pipeline starts computing and
+    // starts its last device-to-host copy sooner.
+    rc = host_enqueue(ctx, rf_host, n_frames, order, out_host, B, B >= 8 && n_frames >= 4 * B);
+    const int rs = pab_host_sync(ctx);           // also after a failed enqueue: nothing of this call stays in flight
+    return rc != PAB_OK ? rc : rs;
+}
+
+// The streaming form: successive calls overlap each other (the copies of call i + 1 and of call i - 1 run beside the
+// kernels of call i), so a call needs no small pieces to hide its own ramp: whole 64-frame pieces, the most efficient launch.
+extern "C" int pab_beamform_host_async(pab_ctx* ctx, const void* rf_host, int n_frames, int order, float* out_host) {
+    int rc = check_args(ctx, rf_host, n_frames, order, out_host);
+    if (rc != PAB_OK) return rc;
+    const int Bcap = ctx->plan.batch_frames < 64 ? ctx->plan.batch_frames : 64;
+    int B = Bcap;
+    if (ctx->tuning.host_batch_frames > 0) B = ctx->tuning.host_batch_frames < Bcap ? ctx->tuning.host_batch_frames : Bcap;
+    return host_enqueue(ctx, rf_host, n_frames, order, out_host, B, false);
 }

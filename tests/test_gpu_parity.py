@@ -297,6 +297,35 @@ def test_host_entry_point_matches_device_entry_point(pab):
         bf.close()
 
 
+def test_host_async_stream_of_calls_matches_blocking_calls(pab):
+    """pab_beamform_host_async: five calls in flight over the three device buffer sets (different frames, different frame
+    counts, so a buffer handed over too early would show), one pab_host_sync; against the device entry point."""
+    sizes = (16, 5, 16, 1, 12)
+    w = synth.make_config("C1", n_frames=sum(sizes))
+    g = w.geom
+    bf = pab.Beamformer(g)
+    try:
+        ref = bf.beamform(torch.from_numpy(w.rf).cuda(), 3).cpu().numpy()
+        torch.cuda.synchronize()
+        ins, outs, f0 = [], [], 0
+        for n in sizes:
+            ins.append(torch.from_numpy(w.rf[f0:f0 + n].copy()).pin_memory())
+            outs.append(torch.full((n, g.nz, g.nx), float("nan")).pin_memory())
+            f0 += n
+        for a, b in zip(ins, outs):
+            bf.beamform_host_async(a, 3, b)
+        bf.host_sync()
+        got = np.concatenate([o.numpy() for o in outs])
+        assert np.all(np.isfinite(got))
+        # the calls group the frames differently (see test_host_entry_point_matches_device_entry_point): rounding only
+        assert np.max(np.abs(got - ref)) <= 2e-6 * float(np.max(np.abs(ref)))
+        bf.host_sync()                                      # nothing in flight: returns at once
+        again = bf.beamform_host(ins[0], 3).numpy()                                   # the blocking call still works after
+        assert np.max(np.abs(again - outs[0].numpy())) <= 2e-6 * float(np.max(np.abs(ref)))
+    finally:
+        bf.close()
+
+
 def test_argument_errors_launch_nothing(pab):
     w = synth.make_config("C1")
     bf = pab.Beamformer(w.geom)
