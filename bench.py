@@ -442,7 +442,8 @@ def run_sweep(args):
     cases += [("C2", 1, (1, 2, 3), False, "cache-single"), ("C4", 1, (4, 5), False, "cache-single"),
               ("C2b", 64, (1, 2, 3), False, "cache-all"), ("C4", 16, (4, 5), False, "cache-all"),
               ("C2b", 64, (3,), False, "cf-cache-all"), ("C4", 16, (5,), False, "cf-cache-all"),
-              ("C2b", 64, (6, 8), False, "cache-all")]
+              ("C2b", 64, (6, 8), False, "cache-all"),
+              ("C3", 256, (3,), True, "cache-all"), ("C5", 1024, (3,), True, "cache-all")]
     if args.case:                         # --case C2:1:cache-single[:3]  ->  one config / frame count / mode [/ order]
         want = args.case.split(":")
         cases = [c for c in cases if c[0] == want[0] and str(c[1]) == want[1] and c[4] == want[2]]
