@@ -371,6 +371,33 @@ __device__ __forceinline__ Tap delay_tap(float xs2, float c0, const float4 row, 
     return o;
 }
 
+// The same step for in-range geometries on the FP64 pipe (B200: 64 lanes/clk/SM beside the FP32 pipes, otherwise idle in
+// this library): idx = sqrt(xs^2 + zs^2) from one MUFU.RSQ64H seed and one Newton step in double (relative error ~1e-12),
+// floor and fraction by the 1.5 * 2^52 rounding constant (the integer is the low word of the sum: no conversion
+// instruction, which would queue on the XU pipe beside the roots), the fraction's 23 leading bits moved into a float in
+// [1, 2) by a funnel shift.  15 instructions of which 10 on the FP64 pipe, against 23 on the FP32 / ALU pipes above.
+//   xs2d  the lateral offset squared, in samples^2 (double; warp-uniform, from the producer)
+//   zs    z fs / c (double)
+// Returns floor(idx) and the fraction in [0, 1] (1 only when idx is an integer to the last bit and the tie rounded down).
+__device__ __forceinline__ Tap delay_tap_f64(double xs2d, double zs) {
+    const double q = fma(zs, zs, xs2d);
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(q));
+    double d = q * r;
+    const double e = fma(-d, d, q);
+    d = fma(e * r, 0.5, d);                                        // sqrt(q) to ~1e-12 relative
+    const double kM = 6755399441055744.0;                          // 1.5 * 2^52: adding it rounds to an integer
+    const double t = (d - 0.5) + kM;                               // low word = floor(d) (ties fall either way: the interpolant is continuous)
+    const double f1 = d - (t - (kM + 1.0));                        // fraction + 1, in [1, 2]
+    const int lo = __double2loint(f1), hi = __double2hiint(f1);
+    const float a1 = __int_as_float((__funnelshift_l(lo, hi, 3) & 0x007fffff) | 0x3f800000);
+    Tap o;
+    o.i0 = __double2loint(t);
+    o.wa = (hi >= 0x40000000) ? 1.0f : a1 - 1.0f;                  // f1 = 2 exactly (a tie rounded down): weight 1
+    o.wb = 0.0f;
+    return o;
+}
+
 // (xs2, c0) of delay_tap from the hi + lo table entries of a pixel column and an element, in fp32 with
 // error-free differences (the direct kernel; the staged kernel's producer does this in fp64)
 __device__ __forceinline__ float2 lateral_square(float2 xj, float2 xe) {

@@ -9,7 +9,8 @@ namespace pab {
 
 // per staged channel: what a consumer needs besides the samples (80 bytes; every read is a warp broadcast)
 struct __align__(16) ChanEntry {
-    float2 xs[8];           // per pixel column c of the tile: (xs2, c0) of delay_tap, xs = column - element in samples
+    float2 xs[8];           // per pixel column c of the tile: (xs2, c0) of delay_tap, xs = column - element in samples;
+                            // in-range launches: xs^2 as a double in the same 8 bytes (delay_tap_f64)
     int base;               // shared-space address such that sample i of the first quad lives at base + i * BPS
     int w0;                 // first staged sample
     int w1m2;               // last valid i0 (staged end - 2)

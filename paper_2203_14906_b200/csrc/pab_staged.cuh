@@ -79,7 +79,12 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
                         const double d = ((double)xj[c].x + (double)xj[c].y) - ((double)xe.x + (double)xe.y);
                         const float hi = (float)d;
                         const float xs2 = hi * hi;
-                        e.xs[c] = make_float2(xs2, (float)((double)xs2 - d * d));
+                        if constexpr (INR) {        // in-range: the square itself, as a double in the entry's 8 bytes (delay_tap_f64)
+                            const double dd = d * d;
+                            e.xs[c] = make_float2(__int_as_float(__double2loint(dd)), __int_as_float(__double2hiint(dd)));
+                        } else {
+                            e.xs[c] = make_float2(xs2, (float)((double)xs2 - d * d));
+                        }
                         if (c == 0) xlo = hi;
                         if (c == kStgCols - 1) xhi = hi;
                     }
@@ -128,6 +133,7 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
         const int trow = tile_row(C.tile_rows, warp, lane, &live);
         const int m = by * C.tile_rows + trow;
         const float4 row = P.zrow[min(m, P.nz - 1)];
+        const double zs64 = fma(0.5, (double)row.y, (double)row.x);          // zs = zs_hi + zs_lo (used by the in-range variant)
         // one frame per thread: scalar accumulators; frame groups: the frames in pairs, packed f32x2 arithmetic
         float p[1][kAcc<K, W>];
         float2 pp[NQ == 0 ? 1 : NF / 2][kAcc<K, W>];
@@ -148,7 +154,9 @@ __global__ void __launch_bounds__(kStgThreads, 1) bf_staged_kernel(const BfParam
             for (int l = 0; l < nch; ++l) {
                 const float2 xs = lds64(tab_s + l * kCE + col * 8);
                 const int base = __float_as_int(lds32(tab_s + l * kCE + 64));
-                const Tap t = delay_tap<INR>(xs.x, xs.y, row, P.S);
+                Tap t;
+                if constexpr (INR) t = delay_tap_f64(__hiloint2double(__float_as_int(xs.y), __float_as_int(xs.x)), zs64);
+                else t = delay_tap<INR>(xs.x, xs.y, row, P.S);
                 int i0 = t.i0;
                 if constexpr (!INR) {
                     const int w0 = __float_as_int(lds32(tab_s + l * kCE + 68));
