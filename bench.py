@@ -54,8 +54,8 @@ FP32_PER_ITEM = 6.0
 XU_PER_ITEM_ISSUED = 1.75
 DELAY_CACHE = "all"
 SM_COUNT = 148
-NCU_TRAFFIC_BYTES = 182_704_896 + 49_611_520   # per 64-frame launch; profiles/r2_headline_ncu.md
-NCU_TRAFFIC_COMMIT = "7de8b9a (round 2)"   # the build that capture was taken on: the constant goes stale silently otherwise
+NCU_TRAFFIC_BYTES = 181_827_584 + 49_893_376   # per 64-frame launch; profiles/r2_headline_ncu.md
+NCU_TRAFFIC_COMMIT = "666c3df (round 2)"   # the build that capture was taken on: the constant goes stale silently otherwise
 XU_LANES_PER_CLK_SM = 16
 FP32_LANES_PER_CLK_SM = 128
 
