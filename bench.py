@@ -493,9 +493,17 @@ def run_sweep(args):
                 xu = 0.0
             if cache != "off" and (F < 4 or cache == "all"):
                 xu = _XU[order][0]            # taps come from the table: no delay square root in the kernel
+            diag_share = 0
+            if cache == "off" and F < 4 and weight == "none" and interp == "linear" and bf.plan()["diagonal"] == 2:
+                # table-free diagonal kernel: one delay (one MUFU, 3 FP32-equivalent slots) per diagonal, shared by the
+                # 16 (orders 1..3) or 8 (orders 4, 5) pairs of the diagonal a thread owns
+                diag_share = 16 if order <= 3 else 8
+                xu = _XU[order][0] + _XU[order][1] / diag_share
             fp = _FP32[order][0] + _FP32[order][1] / batch + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
             if interp == "nearest":
                 fp = {1: 1.0, 2: 3.0, 3: 4.0, 4: 5.0, 5: 7.0}[order]
+            if diag_share:
+                fp = _FP32[order][0] + _FP32[order][1] / diag_share
             t_xu = items * F * xu / (SM_COUNT * XU_LANES_PER_CLK_SM * f_hz) * 1e3
             t_fp = items * F * fp / (SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz) * 1e3
             in_b = g.n_elem * g.n_samp * (2 if dtype == "int16" else 4)
@@ -510,6 +518,7 @@ def run_sweep(args):
                               "items_per_s": round(items * F / (ms * 1e-3), 0),
                               "stage_ms": {k: round(v[0] / reps, 5) for k, v in prof.items()},
                               "beamform_launches": prof["beamform"][1] / reps, "frames_per_thread": share,
+                              "pairs_per_delay": diag_share if diag_share else share,
                               "t_roof_ms": {"xu": round(t_xu, 5), "fp32": round(t_fp, 5), "hbm": round(t_hbm, 5)},
                               "t_smem_ceiling_ms": round(t_sm, 5),
                               "beamform_roofline_frac": round(max(t_xu, t_fp, t_hbm) / bf_ms, 4),

@@ -83,8 +83,10 @@ typedef struct {
     int   batch_frames;          /* internal frame batch per pass (ingest -> beamform -> post)                     */
     int   in_range;              /* 1 when every (pixel, element) delay index lies inside the record and z0 is at
                                     least one sample deep: the kernels then skip the out-of-record masks (A6)     */
-    int   diagonal;              /* 1 once pab_set_delay_cache has built the tables of the single-frame diagonal kernel
-                                    (translation-invariant geometry: pitch an exact integer multiple of dx), else 0   */
+    int   diagonal;              /* single-frame diagonal kernel (translation-invariant geometry: pitch an exact integer
+                                    multiple q <= 8 of dx, in range): 1 once pab_set_delay_cache has built its tap tables;
+                                    2 once a call of 1..3 frames with the delay cache off has built the windows of its
+                                    table-free form (taps computed in the kernel); else 0                             */
     double zs_per_row;           /* dz * fs / c : delay samples per pixel row                                      */
     double xs_per_col;           /* dx * fs / c : delay samples per pixel column at grazing incidence              */
 } pab_plan_info;
@@ -138,7 +140,8 @@ int pab_set_interp(pab_ctx* ctx, int interp);
 /* pab_set_delay_cache -- keep the interpolation tap (integer sample + fraction) of every (pixel, element) pair in
  * device memory, computed once in fp64, instead of recomputing the delay in every call (PAPER.md:190 keeps its
  * delays in GPU global memory; BASELINE.json north_star allows a cached table "where it wins").  It wins most for
- * calls of 1..3 frames, where the in-kernel delay cannot be shared between frames, and by ~7 % for 16-frame groups.
+ * calls of 1..3 frames on geometries that are not translation invariant, where the in-kernel delay cannot be shared
+ * between frames or pairs, and by ~7 % for 16-frame groups.
  * 4 bytes per (pixel, element): 134 MB at 128 elements x 1024 x 256 pixels; when pitch_m is an exact integer
  * multiple q of grid.dx the tap depends on (column - q * element, row) only, and calls of 1..3 frames use a compact
  * table of (nx + q (N-1)) * nz * 8 bytes (2 MB there) instead.  Linear interpolation; coherence-factor weighting
@@ -169,8 +172,12 @@ int pab_set_variant(pab_ctx* ctx, int variant);
  *              O(N) evaluation of e_k, by its recurrence) with linear interpolation and no weighting only
  *   out_dev    device pointer, [n_frames][nz][nx], x fastest, fp32, 4-byte aligned; fully overwritten
  *   cuda_stream a cudaStream_t passed as void*; NULL = the legacy default stream
- * Exception: under PAB_CACHE_ALL the first call of order 1 or 2 with >= 8 frames, at a row pitch in (1, 8/7] samples,
- * builds a second tap table once (one device synchronisation; skipped while the stream is being captured).
+ * Exceptions (one device synchronisation each, once per context; skipped while the stream is being captured): under
+ * PAB_CACHE_ALL the first call of order 1 or 2 with >= 8 frames, at a row pitch in (1, 8/7] samples, builds a second tap
+ * table; with the delay cache off and the automatic variant, the first call of 1..3 frames on a translation-invariant
+ * in-range geometry (pitch_m an exact integer multiple q <= 8 of grid.dx, n_elem a multiple of 4) builds the windows of
+ * the single-frame diagonal kernel (a few hundred KB; no delay table: that kernel computes one delay per diagonal of
+ * (column, element) pairs in the kernel, on the FP64 pipe, and is what such calls then run: pab_plan_info.diagonal = 2).
  * One context must not be used from two streams at once (shared scratch).  The CUDA device that was current at
  * pab_create must be current at the call (PAB_ERR_INVALID otherwise).
  * Errors: PAB_ERR_INVALID (nothing launched), PAB_ERR_CUDA.

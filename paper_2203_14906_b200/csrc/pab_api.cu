@@ -42,6 +42,8 @@ struct pab_ctx {
     uint2* d_compact = nullptr;          // (d, row) tap table when pitch = q dx exactly (translation invariance)
     int cache_q = 0;
     DiagSet diag[2];                     // single-frame diagonal kernel: [0] orders 1..3 (16 pixels per thread), [1] orders 4, 5 (8)
+    DiagSet diag_nt[2];                  // the same for the table-free variant (delay cache off): windows only, taps in-kernel
+    bool diag_nt_tried = false;
     void* d_metric = nullptr;            // MetricAcc + double[1] + 2 x 4096 histogram bins (row f3), lazy
     unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
@@ -91,6 +93,7 @@ void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_xj); cudaFree(ctx->d_xe); cudaFree(ctx->d_zrow); cudaFree(ctx->d_stage); cudaFree(ctx->d_img);
     cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact); cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
     xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]);
+    xl_diag_free(&ctx->diag_nt[0]); xl_diag_free(&ctx->diag_nt[1]);
     for (int b = 0; b < kHostSets; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -102,6 +105,37 @@ void free_all(pab_ctx* ctx) {
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_run) cudaStreamDestroy(ctx->s_run);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+}
+
+// Calls of 1..3 frames with the delay cache OFF on translation-invariant, in-range geometries (pitch = q dx exactly, q <= 8):
+// the diagonal kernel in its table-free form (pab_diag.cuh, TAB = false: one tap per diagonal from delay_tap_f64, shared by
+// the 16 or 8 pairs of the diagonal).  It needs no delay table, only the window of every (tile, channel quad), a few
+// hundred KB built on the first such call (one device synchronisation, skipped while the stream is being captured).
+// Returns whether the set of this order is there.
+bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
+    if (!ctx->diag_nt_tried) {
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
+        ctx->diag_nt_tried = true;
+        const long long q = llround((double)ctx->pitch / (double)ctx->grid.dx);
+        if (ctx->plan.in_range && ctx->plan.smem_bytes > 0 && q >= 1 && q <= 8 && (double)ctx->pitch == (double)q * (double)ctx->grid.dx &&
+            xl_diag_configure(ctx->smem_optin) == cudaSuccess) {
+            cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 4, 3, ctx->smem_optin, false,
+                                          &ctx->diag_nt[0]);
+            if (e == cudaSuccess)
+                e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 2, 5, ctx->smem_optin, false, &ctx->diag_nt[1]);
+            if (e != cudaSuccess) {          // not fatal: the call keeps the one-frame-per-thread kernels
+                cudaGetLastError();
+                xl_diag_free(&ctx->diag_nt[0]); xl_diag_free(&ctx->diag_nt[1]);
+            } else {
+                ctx->launches += 2;
+                if (ctx->plan.diagonal == 0 && (ctx->diag_nt[0].smem_bytes > 0 || ctx->diag_nt[1].smem_bytes > 0)) ctx->plan.diagonal = 2;
+            }
+        } else {
+            cudaGetLastError();
+        }
+    }
+    return ctx->diag_nt[order <= 3 ? 0 : 1].smem_bytes > 0;
 }
 
 // Orders 1 and 2 in frame groups are bound by the shared-memory data pipe, and at row pitches in (1, 8/7] samples 64-row
@@ -334,12 +368,13 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
     if (mode != PAB_CACHE_OFF && ctx->d_compact && ctx->diag[0].smem_bytes == 0 && ctx->diag[1].smem_bytes == 0) {
         PAB_CUDA(ctx, xl_diag_configure(ctx->smem_optin));
         cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q,
-                                      4, 3, ctx->smem_optin, &ctx->diag[0]);
-        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, &ctx->diag[1]);
+                                      4, 3, ctx->smem_optin, true, &ctx->diag[0]);
+        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, true, &ctx->diag[1]);
         if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
         ctx->launches += 4;
     }
-    ctx->plan.diagonal = (mode != PAB_CACHE_OFF && (ctx->diag[0].smem_bytes > 0 || ctx->diag[1].smem_bytes > 0)) ? 1 : 0;
+    ctx->plan.diagonal = (mode != PAB_CACHE_OFF && (ctx->diag[0].smem_bytes > 0 || ctx->diag[1].smem_bytes > 0)) ? 1
+                         : (ctx->diag_nt[0].smem_bytes > 0 || ctx->diag_nt[1].smem_bytes > 0) ? 2 : 0;
     ctx->cache_mode = mode;
     return PAB_OK;
 }

@@ -58,7 +58,9 @@ __global__ void __launch_bounds__(256) diag_taps_kernel(const DiagGeom G, uint2*
 // last row (idx grows with depth), at some column: all columns of both rows are evaluated for the quad's 4 channels.
 // grid: (tiles_x * tiles_z, quads); block: 256 threads >= cols * 2 ... (loops).  sq = 0 is the zero quad before the
 // array (channels -4..-1), sq = quads - 1 the one after it.
-__global__ void __launch_bounds__(256) diag_window_kernel(const DiagGeom G, int rows, int cols, int tiles_x, int quads,
+// margin: extra samples on either side (the table-free variant computes its taps in the kernel, to ~1e-9 samples of this
+// expression: a floor that falls the other way at a window's edge must still land inside it).
+__global__ void __launch_bounds__(256) diag_window_kernel(const DiagGeom G, int rows, int cols, int tiles_x, int quads, int margin,
                                                            int* __restrict__ qw0, int* __restrict__ qlen) {
     __shared__ int s_min, s_max;
     const int tile = blockIdx.x, sq = blockIdx.y;
@@ -79,7 +81,7 @@ __global__ void __launch_bounds__(256) diag_window_kernel(const DiagGeom G, int 
     __syncthreads();
     if (threadIdx.x == 0) {
         const bool real = sq >= 1 && sq <= quads - 2;
-        int w0 = s_min, w1 = s_max + 2;                    // samples [w0, w1): i0 and i0 + 1 of every pair
+        int w0 = s_min - margin, w1 = s_max + 2 + margin;    // samples [w0, w1): i0 and i0 + 1 of every pair
         if (real) { w0 = max(w0, 0); w1 = min(w1, G.S); }
         qw0[(size_t)tile * quads + sq] = w0;
         qlen[(size_t)tile * quads + sq] = max(w1 - w0, 0);
@@ -94,7 +96,9 @@ template <typename T> __device__ __forceinline__ float diag_ld(const T* p) { ret
 // CHK (pab_self_check): every shared-memory gather of the element loop is compared with the staged window of its quad and
 // out-of-window accesses are counted in *viol (compute-sanitizer is closed on this GPU pool; this kernel's addressing is
 // the most intricate of the library).
-template <int K, int NPG, typename T, bool CHK = false>
+// TAB = false: no tap table; the tap of a diagonal comes from delay_tap_f64 (FP64 pipe), computed one diagonal ahead the
+// way the table variant prefetches it: 13 instructions per (thread, diagonal), shared by the thread's P pairs.
+template <int K, int NPG, typename T, bool CHK = false, bool TAB = true>
 __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T* __restrict__ rf, float* __restrict__ out,
                                                                           const DiagCfg C, const DiagTables D, int N, int S,
                                                                           int nx, int nz, float scale, int* __restrict__ viol = nullptr) {
@@ -161,7 +165,19 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
     const uint32_t tstep = (uint32_t)C.q * (uint32_t)nz;
     const uint32_t t0 = (uint32_t)(j0 + C.q * (N - 1 + P + 4 * NPG)) * (uint32_t)nz + (uint32_t)mc;
     const int f_lo = 4 * C.part_lo[part];
-    uint2 tap_next = __ldg(D.taps + (t0 - (uint32_t)f_lo * tstep));
+    // table-free: lateral offset (samples) of the next diagonal, stepped by -q xs_b per diagonal; depth of this lane's row
+    double xs_next = 0.0, xs_step = 0.0, zs = 0.0;
+    uint2 tap_next;
+    if constexpr (TAB) {
+        tap_next = __ldg(D.taps + (t0 - (uint32_t)f_lo * tstep));
+    } else {
+        xs_step = -(double)C.q * D.xs_b;
+        xs_next = fma((double)(j0 + C.q * (N - 1 + P + 4 * NPG) - C.q * f_lo), D.xs_b, D.xs_a);
+        zs = fma((double)mc, D.zs_b, D.zs_a);
+        const Tap t = delay_tap_f64(xs_next * xs_next, zs);
+        tap_next = make_uint2((unsigned)t.i0, __float_as_uint(t.wa));
+        xs_next += xs_step;
+    }
     for (int egp = C.part_lo[part]; egp < C.part_lo[part + 1]; ++egp) {
         const int eg = egp - NPG;                                      // first quad (unpadded index) of the group
         const uint32_t tg = t0 - (uint32_t)(4 * egp + 1) * tstep;      // entry of the group's second diagonal
@@ -175,7 +191,13 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
             constexpr bool GUARD = decltype(gc)::value;
             const float a = __uint_as_float(tap_next.y);
             const uint32_t off = tap_next.x * 16u;
-            tap_next = __ldg(D.taps + (tg - (uint32_t)r * tstep));           // diagonal f + 1
+            if constexpr (TAB) {
+                tap_next = __ldg(D.taps + (tg - (uint32_t)r * tstep));       // diagonal f + 1
+            } else {
+                const Tap t = delay_tap_f64(xs_next * xs_next, zs);
+                tap_next = make_uint2((unsigned)t.i0, __float_as_uint(t.wa));
+                xs_next += xs_step;
+            }
             float4 lo0, lo1;                                                   // samples i0, i0 + 1 of quad eg + cg
             bool have = false;
 #pragma unroll

@@ -62,6 +62,11 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         // translation-invariant geometry: the diagonal kernel, straight from the caller's frames (no ingest pass)
         Span sp(ctx, PAB_STAGE_BEAMFORM, st);
         xl_diag(order, ctx->dtype, ctx->diag[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
+    } else if (F < 4 && ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && weight == 0 && order <= 5 &&
+               ensure_diag_nt(ctx, order, st)) {
+        // the same kernel without any delay table: the tap of a diagonal is computed in the kernel (FP64 pipe)
+        Span sp(ctx, PAB_STAGE_BEAMFORM, st);
+        xl_diag(order, ctx->dtype, ctx->diag_nt[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
     } else if (F < 4) {
         const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
                             xl_cached_fits(ctx->plan, 0, ctx->d_compact != nullptr, ctx->smem_optin);

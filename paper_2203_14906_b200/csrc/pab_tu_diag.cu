@@ -43,8 +43,11 @@ int split_parts(int G, int npg, int nq_real, int parts, int* lo) {
 template <int K, int NPG, typename T>
 void launch_diag_t(const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale, cudaStream_t st) {
     dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, F);
-    const DiagTables tabs{D.taps, D.qw0, D.qoff};
-    bf_diag_kernel<K, NPG, T><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
+    const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b};
+    if (D.taps)
+        bf_diag_kernel<K, NPG, T><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
+    else
+        bf_diag_kernel<K, NPG, T, false, false><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
 }
 template <int K, int NPG>
 void launch_diag_k(int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
@@ -56,7 +59,9 @@ template <int K, int NPG>
 cudaError_t diag_attr(int smem_optin) {
     cudaError_t e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if ((e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 
 }  // namespace
@@ -65,7 +70,7 @@ cudaError_t diag_attr(int smem_optin) {
 cudaError_t xl_diag_check(int order, const DiagSet& D, const float* rf, float* out, int N, int S, int nx, int nz, int* d_viol,
                           cudaStream_t st) {
     dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, 1);
-    const DiagTables tabs{D.taps, D.qw0, D.qoff};
+    const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b};
     const size_t smem = (size_t)D.smem_bytes + 2 * D.cfg.quads * 4 + 128;
     cudaError_t e;
     if (order <= 3) {
@@ -95,8 +100,9 @@ void xl_diag_free(DiagSet* D) {
 // Build the tables of one set (npg = 4: orders 1..3, npg = 2: orders 4, 5).  Leaves D->smem_bytes = 0 when the geometry
 // does not qualify (N not a multiple of 4, too many warps, a tile that does not fit in shared memory); returns a CUDA
 // error only for failed calls.  Synchronises the device.
+// with_taps = false: the set of the table-free variant: windows only, one sample of margin on either side.
 cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, int q, int npg, int max_order, int smem_limit,
-                          DiagSet* D) {
+                          bool with_taps, DiagSet* D) {
     *D = DiagSet();
     const int P = 4 * npg;
     if (N % 4 != 0 || N < 4 || q < 1 || q > 8) return cudaSuccess;
@@ -135,12 +141,12 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     const size_t tiles = (size_t)cfg.tiles_x * cfg.tiles_z, nq = tiles * cfg.quads;
     int* d_len = nullptr;
     cudaError_t e;
-    if ((e = cudaMalloc(&D->taps, (size_t)cfg.nd * g.nz * sizeof(uint2))) != cudaSuccess) return e;
+    if (with_taps && (e = cudaMalloc(&D->taps, (size_t)cfg.nd * g.nz * sizeof(uint2))) != cudaSuccess) return e;
     if ((e = cudaMalloc(&D->qw0, nq * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
     if ((e = cudaMalloc(&D->qoff, (nq + tiles) * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
     if ((e = cudaMalloc(&d_len, nq * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
-    diag_taps_kernel<<<dim3((g.nz + 255) / 256, cfg.nd), 256>>>(geo, D->taps);
-    diag_window_kernel<<<dim3((unsigned)tiles, cfg.quads), 256>>>(geo, cfg.rows, cfg.cols, cfg.tiles_x, cfg.quads, D->qw0, d_len);
+    if (with_taps) diag_taps_kernel<<<dim3((g.nz + 255) / 256, cfg.nd), 256>>>(geo, D->taps);
+    diag_window_kernel<<<dim3((unsigned)tiles, cfg.quads), 256>>>(geo, cfg.rows, cfg.cols, cfg.tiles_x, cfg.quads, with_taps ? 0 : 1, D->qw0, d_len);
     std::vector<int> len(nq), off(nq + tiles);
     e = cudaMemcpy(len.data(), d_len, nq * sizeof(int), cudaMemcpyDeviceToHost);
     cudaFree(d_len);
@@ -160,6 +166,11 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     D->cfg = cfg;
     D->npg = npg;
     D->smem_bytes = (int)smem;
+    // diag_ddx / diag_idx in samples: xs(d) = (x0 + (d - q ((N - 1) / 2 + P)) dx) fs / c, zs(m) = (z0 + m dz) fs / c
+    D->xs_b = (double)g.dx * fs / c;
+    D->xs_a = ((double)g.x0 - (double)q * ((N - 1) / 2.0 + P) * (double)g.dx) * fs / c;
+    D->zs_b = (double)g.dz * fs / c;
+    D->zs_a = (double)g.z0 * fs / c;
     return cudaDeviceSynchronize();
 }
 

@@ -87,9 +87,12 @@ struct DiagCfg {
 };
 
 struct DiagTables {
-    const uint2* taps;      // [nd][nz]: (floor(idx), fraction bits) of d = j - q i + q (N - 1 + P)
+    const uint2* taps;      // [nd][nz]: (floor(idx), fraction bits) of d = j - q i + q (N - 1 + P); unused by the table-free variant
     const int* qw0;         // [tiles][quads]     first staged sample of the quad's window
     const int* qoff;        // [tiles][quads + 1] byte offset of the quad's window in the staging area (16-byte units x 16)
+    // table-free variant (taps computed in the kernel, delay_tap_f64): lateral offset in samples of table column d is
+    // xs_a + d xs_b, depth in samples of row m is zs_a + m zs_b
+    double xs_a, xs_b, zs_a, zs_b;
 };
 
 // one set of device tables of the diagonal kernel (P = 16 pixels per thread for orders 1..3, P = 8 for orders 4, 5)
@@ -100,6 +103,7 @@ struct DiagSet {
     int* qoff = nullptr;
     int npg = 0;            // pixel groups of 4 per thread
     int smem_bytes = 0;     // dynamic shared memory per CTA; 0: not built / does not fit
+    double xs_a = 0.0, xs_b = 0.0, zs_a = 0.0, zs_b = 0.0;       // see DiagTables (set for both variants)
 };
 
 // nearest-sample delays (pab_nearest.cuh)

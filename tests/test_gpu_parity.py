@@ -129,6 +129,25 @@ def test_c2_full_size_single_frame(pab, orc, variant, order):
     check_raw(gpu[0], orc.beamform(w.rf, w.geom, order)[0], order)
 
 
+@pytest.mark.parametrize("order", [1, 2, 3])
+def test_c2_full_size_single_frame_default_path(pab, orc, order):
+    """Config C2 through the default settings (automatic variant, no delay table): the table-free diagonal kernel
+    (taps computed in the kernel on the FP64 pipe, one per diagonal), fp32 and int16 input."""
+    w = synth.make_config("C2")
+    bf = pab.Beamformer(w.geom)
+    try:
+        out = bf.beamform(torch.from_numpy(w.rf).cuda(), order)
+        torch.cuda.synchronize()
+        assert bf.plan()["diagonal"] == 2                      # the table-free diagonal kernel is what ran
+        ref = orc.beamform(w.rf, w.geom, order)[0]
+        assert check_raw(out.cpu().numpy().astype(np.float64)[0], ref, order) <= 2.5e-5
+    finally:
+        bf.close()
+    rf16 = np.rint(w.rf * (8000.0 / np.max(np.abs(w.rf)))).astype(np.int16)
+    gpu, _ = run_gpu(pab, w.geom, rf16, order, dtype="int16", scale=0.5)
+    check_raw(gpu[0], orc.beamform(rf16, w.geom, order, scale=0.5)[0], order)
+
+
 @pytest.mark.parametrize("delay_cache", ["all", "off"])
 def test_c2b_headline_batch_sampled_pixels(pab, orc, delay_cache):
     """The launch configuration bench.py times (64 frames, order 3, auto variant, cached taps) on sampled pixels,
@@ -155,9 +174,11 @@ def test_c2b_headline_batch_sampled_pixels(pab, orc, delay_cache):
     assert np.max(np.abs(got - ref)) <= 1e-3 * full_peak
 
 
-@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("variant", VARIANTS + ["auto"])
 @pytest.mark.parametrize("order", [4, 5])
 def test_c4_large_aperture(pab, orc, variant, order):
+    """staged: the diagonal kernel with its tap table; direct: the direct kernel; auto (the default settings): the
+    table-free diagonal kernel."""
     w = synth.make_config("C4")
     g = w.geom
     gpu, _ = run_gpu(pab, g, w.rf, order, variant, delay_cache="single" if variant == "staged" else "off")
@@ -638,10 +659,11 @@ def test_delay_cache_ragged_int16_and_batches(pab, orc):
                 check_raw(gpu[f], ref[f], order)
 
 
+@pytest.mark.parametrize("tables", ["single", "off"])
 @pytest.mark.parametrize("q,n_elem,nx,nz,frames,dtype", [(1, 16, 37, 70, 1, "float32"), (2, 24, 45, 33, 3, "float32"),
                                                          (3, 8, 50, 129, 2, "int16"), (2, 4, 7, 5, 1, "float32"),
                                                          (1, 64, 130, 95, 2, "int16"), (4, 12, 64, 64, 1, "float32")])
-def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, nz, frames, dtype):
+def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, nz, frames, dtype, tables):
     """The single-frame diagonal kernel (pitch = q dx exactly: one tap per diagonal, channel-quad staging from the caller's
     frame) on ragged grids: nx, nz off the tile sizes, arrays of 1..16 channel quads, q = 1..4, 1..3 frames, int16 input
     with a scale, every order 1..5 (16 pixels per thread for orders 1..3, 8 for orders 4, 5)."""
@@ -658,9 +680,11 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
     scale = 1.0
     if dtype == "int16":
         rf, scale = np.rint(rf * 4000.0).astype(np.int16), 0.25
-    bf = pab.Beamformer(g, dtype=dtype, scale=scale, delay_cache="single")
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, delay_cache=tables)
     try:
-        assert bf.plan()["in_range"] == 1 and bf.plan()["diagonal"] == 1          # the diagonal kernel is what runs
+        assert bf.plan()["in_range"] == 1
+        if tables == "single":
+            assert bf.plan()["diagonal"] == 1                                     # the diagonal kernel is what runs
         for order in (1, 2, 3, 4, 5):
             if order > n_elem:
                 continue
@@ -670,7 +694,9 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
             ref = orc.beamform(rf, g, order, scale=scale)
             for f in range(frames):
                 assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
-        if dtype == "float32":                 # every shared-memory gather inside the staged window of its quad
+            if tables == "off":                # delay cache off: the table-free form of the kernel (taps on the FP64 pipe)
+                assert bf.plan()["diagonal"] == 2
+        if dtype == "float32" and tables == "single":      # every shared-memory gather inside the staged window of its quad
             for order in (3, 5):
                 if order <= n_elem:
                     assert bf.self_check(torch.from_numpy(rf[:1]).cuda(), order) == 0
