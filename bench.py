@@ -499,7 +499,8 @@ def run_sweep(args):
                 # 16 (orders 1..3) or 8 (orders 4, 5) pairs of the diagonal a thread owns
                 diag_share = 16 if order <= 3 else 8
                 xu = _XU[order][0] + _XU[order][1] / diag_share
-            fp = _FP32[order][0] + _FP32[order][1] / batch + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
+            taps_from_table = cache != "off" and (F < 4 or cache == "all")       # no delay arithmetic in the kernel at all
+            fp = _FP32[order][0] + (0.0 if taps_from_table else _FP32[order][1] / batch) + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
             if interp == "nearest":
                 fp = {1: 1.0, 2: 3.0, 3: 4.0, 4: 5.0, 5: 7.0}[order]
             if diag_share:
