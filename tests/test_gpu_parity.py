@@ -704,6 +704,45 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
         bf.close()
 
 
+@pytest.mark.parametrize("tables", ["off", "all"])
+@pytest.mark.parametrize("dtype", ["float32", "int16"])
+def test_remainder_frames_take_the_diagonal_kernel(pab, orc, dtype, tables):
+    """Frame counts that are not a multiple of 4 on a translation-invariant in-range geometry: the whole quads go through
+    the frame-group kernels, the 1..3 frames left over through the single-frame diagonal kernel (straight from the caller's
+    buffer), and the post chain sees all of them.  5, 7, 9 and 22 frames, orders 1..5, raw and log output."""
+    rng = np.random.default_rng(77)
+    q, n_elem, nx, nz, S = 2, 32, 45, 150, 900
+    dx = 2.0 ** -13
+    g = synth.Geometry(n_elem, S, 40e6, 1540.0, float(np.float32(q * np.float64(dx))), nx, nz, -(nx - 1) / 2 * dx, dx, 2.1e-3,
+                       0.06e-3).f32()
+    base = [(rng.uniform(-1e-3, 1e-3), rng.uniform(3e-3, 10e-3), 1.0, 0.0) for _ in range(4)]
+    rf, _ = synth._frames(rng, g, base, 5e6, 22, 20.0, True)
+    scale = 1.0
+    if dtype == "int16":
+        rf, scale = np.rint(rf * 4000.0).astype(np.int16), 0.25
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, delay_cache=tables)
+    try:
+        assert bf.plan()["in_range"] == 1
+        for frames in (5, 7, 9, 22):
+            x = torch.from_numpy(rf[:frames]).cuda()
+            for order in (1, 2, 3, 4, 5):
+                out = bf.beamform(x, order)
+                torch.cuda.synchronize()
+                assert bf.plan()["diagonal"] in (1, 2)
+                gpu = out.cpu().numpy().astype(np.float64)
+                ref = orc.beamform(rf[:frames], g, order, scale=scale)
+                for f in range(frames):
+                    check_raw(gpu[f], ref[f], order)
+    finally:
+        bf.close()
+    post = dict(mode="log", f_center=10e6, f_halfwidth=2.5e6, n_taps_bp=64, n_taps_hilbert=63, dyn_range_db=60.0)
+    gpu, _ = run_gpu(pab, g, rf[:7], 3, dtype=dtype, scale=scale, post=post, delay_cache=tables)
+    ref = orc.post(orc.beamform(rf[:7], g, 3, scale=scale), g, post["f_center"], post["f_halfwidth"], post["n_taps_bp"],
+                   post["n_taps_hilbert"], post["dyn_range_db"], mode="log")
+    sel = ref > -40.0
+    assert np.max(np.abs(gpu - ref)[sel]) <= 0.05
+
+
 @pytest.mark.parametrize("cfg,order", [("C2", 3), ("C4", 5), ("C3", 1), ("C5", 4)])
 def test_diagonal_kernel_self_check_named_geometries(pab, cfg, order):
     """pab_self_check on the geometries of the named configs (C5's with fp32 frames): no gather of the diagonal kernel
