@@ -704,6 +704,39 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
         bf.close()
 
 
+@pytest.mark.parametrize("tables", ["off", "single", "all"])
+def test_exact_integer_delays(pab, orc, tables):
+    """The degenerate case of the delay index: a geometry on which many delays are EXACT integers of samples (c / fs = 2^-15 m,
+    rows and z0 on multiples of it, columns on multiples of 4 samples, so every pixel under an element and every Pythagorean
+    (lateral, depth) pair has an integer idx).  floor() then sits on its discontinuity: whichever way the kernels' index rounds
+    (in-kernel fp64 with its rounding-constant floor and its tie rule, in-kernel fp32, or the fp64 tap table), the interpolated
+    sample must be the oracle's.  Single frames (diagonal kernel), 16-frame groups and a 5-frame call, orders 1, 3, 5."""
+    fs, c = float(2 ** 25), 1024.0
+    dx = 2.0 ** -13
+    g = synth.Geometry(16, 700, fs, c, 2 * dx, 33, 40, -16 * dx, dx, 2.0 ** -7, 2.0 ** -15).f32()
+    zs = (np.float64(g.z0) + np.arange(g.nz) * np.float64(g.dz)) * fs / c
+    assert np.all(zs == np.rint(zs))                                   # every row an integer number of samples deep
+    idx = np.sqrt(((g.pix_x()[None, :, None] - g.elem_x()[None, None, :]) * fs / c) ** 2 + zs[:, None, None] ** 2)
+    assert np.mean(idx == np.rint(idx)) > 0.02                         # thousands of exactly integer delays
+    rng = np.random.default_rng(5)
+    rf = rng.standard_normal((16, g.n_elem, g.n_samp)).astype(np.float32)      # white noise: adjacent samples unrelated
+    bf = pab.Beamformer(g, delay_cache=tables)
+    try:
+        assert bf.plan()["in_range"] == 1
+        for frames in (1, 5, 16):
+            for order in (1, 3, 5):
+                out = bf.beamform(torch.from_numpy(rf[:frames]).cuda(), order)
+                torch.cuda.synchronize()
+                gpu = out.cpu().numpy().astype(np.float64)
+                ref = orc.beamform(rf[:frames], g, order)
+                for f in range(frames):
+                    peak = np.max(np.abs(ref[f]))
+                    # DAS is linear in the samples: a wrong neighbour anywhere would show at 1e-2 of the peak
+                    assert np.max(np.abs(gpu[f] - ref[f])) <= (2e-6 if order == 1 else 5e-3) * peak, (frames, order, f)
+    finally:
+        bf.close()
+
+
 @pytest.mark.parametrize("tables", ["off", "all"])
 @pytest.mark.parametrize("dtype", ["float32", "int16"])
 def test_remainder_frames_take_the_diagonal_kernel(pab, orc, dtype, tables):
