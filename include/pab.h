@@ -84,7 +84,7 @@ typedef struct {
     int   in_range;              /* 1 when every (pixel, element) delay index lies inside the record and z0 is at
                                     least one sample deep: the kernels then skip the out-of-record masks (A6)     */
     int   diagonal;              /* single-frame diagonal kernel (translation-invariant geometry: pitch an exact integer
-                                    multiple q <= 8 of dx, in range): 1 once pab_set_delay_cache has built its tap tables;
+                                    multiple q <= 16 of dx, in range): 1 once pab_set_delay_cache has built its tap tables;
                                     2 once a call of 1..3 frames with the delay cache off has built the windows of its
                                     table-free form (taps computed in the kernel); else 0                             */
     double zs_per_row;           /* dz * fs / c : delay samples per pixel row                                      */
@@ -175,7 +175,7 @@ int pab_set_variant(pab_ctx* ctx, int variant);
  * Exceptions (one device synchronisation each, once per context; skipped while the stream is being captured): under
  * PAB_CACHE_ALL the first call of order 1 or 2 with >= 8 frames, at a row pitch in (1, 8/7] samples, builds a second tap
  * table; with the delay cache off and the automatic variant, the first call of 1..3 frames on a translation-invariant
- * in-range geometry (pitch_m an exact integer multiple q <= 8 of grid.dx, n_elem a multiple of 4) builds the windows of
+ * in-range geometry (pitch_m an exact integer multiple q <= 16 of grid.dx, n_elem a multiple of 4) builds the windows of
  * the single-frame diagonal kernel (a few hundred KB; no delay table: that kernel computes one delay per diagonal of
  * (column, element) pairs in the kernel, on the FP64 pipe, and is what such calls then run: pab_plan_info.diagonal = 2).
  * One context must not be used from two streams at once (shared scratch).  The CUDA device that was current at
@@ -246,7 +246,8 @@ long long pab_launch_count(const pab_ctx* ctx);
 int pab_set_profile(pab_ctx* ctx, int max_launches);
 int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset);
 
-/* pab_self_check -- diagnostic for the single-frame diagonal kernel (pab_plan_info.diagonal == 1; fp32 input): runs one
+/* pab_self_check -- diagnostic for the single-frame diagonal kernel (fp32 input; with the delay cache on: the form with its
+ * tap table, pab_plan_info.diagonal == 1; with it off and the automatic variant: the table-free form, == 2): runs one
  * frame through an instantiation that compares every shared-memory gather of its element loop with the staged window of
  * the channel quad it reads from, and returns the number of out-of-window accesses (0 for a correct build).  Stands in
  * for compute-sanitizer's memcheck, which is closed on the GPU pool this library was developed on.  order 1..5 selects

@@ -107,7 +107,7 @@ void free_all(pab_ctx* ctx) {
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
 }
 
-// Calls of 1..3 frames with the delay cache OFF on translation-invariant, in-range geometries (pitch = q dx exactly, q <= 8):
+// Calls of 1..3 frames with the delay cache OFF on translation-invariant, in-range geometries (pitch = q dx exactly, q <= 16):
 // the diagonal kernel in its table-free form (pab_diag.cuh, TAB = false: one tap per diagonal from delay_tap_f64, shared by
 // the 16 or 8 pairs of the diagonal).  It needs no delay table, only the window of every (tile, channel quad), a few
 // hundred KB built on the first such call (one device synchronisation, skipped while the stream is being captured).
@@ -118,7 +118,7 @@ bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
         if (cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
         ctx->diag_nt_tried = true;
         const long long q = llround((double)ctx->pitch / (double)ctx->grid.dx);
-        if (ctx->plan.in_range && ctx->plan.smem_bytes > 0 && q >= 1 && q <= 8 && (double)ctx->pitch == (double)q * (double)ctx->grid.dx &&
+        if (ctx->plan.in_range && ctx->plan.smem_bytes > 0 && q >= 1 && q <= 16 && (double)ctx->pitch == (double)q * (double)ctx->grid.dx &&
             xl_diag_configure(ctx->smem_optin) == cudaSuccess) {
             cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 4, 3, ctx->smem_optin, false,
                                           &ctx->diag_nt[0]);
@@ -381,8 +381,10 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
 
 int pab_self_check(pab_ctx* ctx, const float* rf_dev, int order, long long* violations) {
     if (!ctx || !rf_dev || !violations || order < 1 || order > 5) return PAB_ERR_INVALID;
-    const DiagSet& D = ctx->diag[order <= 3 ? 0 : 1];
-    if (ctx->cache_mode == PAB_CACHE_OFF || D.smem_bytes == 0 || ctx->dtype != PAB_F32) return PAB_ERR_INVALID;
+    // delay cache on: the kernel with its tap table; off: its table-free form (built here if no call has built it yet)
+    if (ctx->cache_mode == PAB_CACHE_OFF && (ctx->variant != PAB_VARIANT_AUTO || !ensure_diag_nt(ctx, order, 0))) return PAB_ERR_INVALID;
+    const DiagSet& D = ctx->cache_mode == PAB_CACHE_OFF ? ctx->diag_nt[order <= 3 ? 0 : 1] : ctx->diag[order <= 3 ? 0 : 1];
+    if (D.smem_bytes == 0 || ctx->dtype != PAB_F32) return PAB_ERR_INVALID;
     float* out = nullptr;
     int* d_viol = nullptr;
     int h = 0;

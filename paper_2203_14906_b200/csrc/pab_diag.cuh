@@ -33,11 +33,16 @@ namespace pab {
 struct DiagGeom {
     double fs, c, x0, dx, z0, dz;
     int N, S, nx, nz, q, P;
+    double ddx_max;         // largest |pixel column - element| (metres) of a real pair: max over table columns q P and nx - 1 + q (N - 1 + P)
 };
 // lateral offset (pixel column - element) of table column d: d = j - q i + q (N - 1 + P), x_j - x_i = x0 + j dx - (i - (N-1)/2) q dx
+// Table columns beyond those of the real pairs belong only to pairs that do not exist (pixel columns past nx in a ragged last
+// tile, the zero quads beside the array).  Their lateral offset is capped at the largest one a real pair has, so that every
+// tap lies inside the record like the real ones (the geometry is in range) and inside the windows, which are built from
+// this same expression; what such pairs read is never stored (columns past nx) or is zero (zero quads).
 __device__ __forceinline__ double diag_ddx(const DiagGeom& G, int d) {
     const double k = __dsub_rn((double)d, __dmul_rn((double)G.q, __dadd_rn(__ddiv_rn(__dsub_rn((double)G.N, 1.0), 2.0), (double)G.P)));
-    return __dadd_rn(G.x0, __dmul_rn(k, G.dx));
+    return fmin(fabs(__dadd_rn(G.x0, __dmul_rn(k, G.dx))), G.ddx_max);
 }
 __device__ __forceinline__ double diag_idx(const DiagGeom& G, int d, int m) {
     const double z = __dadd_rn(G.z0, __dmul_rn((double)m, G.dz));
@@ -167,6 +172,7 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
     const int f_lo = 4 * C.part_lo[part];
     // table-free: lateral offset (samples) of the next diagonal, stepped by -q xs_b per diagonal; depth of this lane's row
     double xs_next = 0.0, xs_step = 0.0, zs = 0.0;
+    int i0_cap = 0x7fffffff;
     uint2 tap_next;
     if constexpr (TAB) {
         tap_next = __ldg(D.taps + (t0 - (uint32_t)f_lo * tstep));
@@ -174,8 +180,12 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
         xs_step = -(double)C.q * D.xs_b;
         xs_next = fma((double)(j0 + C.q * (N - 1 + P + 4 * NPG) - C.q * f_lo), D.xs_b, D.xs_a);
         zs = fma((double)mc, D.zs_b, D.zs_a);
+        // diag_ddx's cap on the lateral offset, as one integer minimum per tap: no real pair of this row has a delay beyond
+        // that of the largest real offset (+1: the two evaluations may floor a borderline value differently; the windows
+        // of this form carry that sample of margin)
+        i0_cap = delay_tap_f64(D.xs2_max, zs).i0 + 1;
         const Tap t = delay_tap_f64(xs_next * xs_next, zs);
-        tap_next = make_uint2((unsigned)t.i0, __float_as_uint(t.wa));
+        tap_next = make_uint2((unsigned)min(t.i0, i0_cap), __float_as_uint(t.wa));
         xs_next += xs_step;
     }
     for (int egp = C.part_lo[part]; egp < C.part_lo[part + 1]; ++egp) {
@@ -195,7 +205,7 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
                 tap_next = __ldg(D.taps + (tg - (uint32_t)r * tstep));       // diagonal f + 1
             } else {
                 const Tap t = delay_tap_f64(xs_next * xs_next, zs);
-                tap_next = make_uint2((unsigned)t.i0, __float_as_uint(t.wa));
+                tap_next = make_uint2((unsigned)min(t.i0, i0_cap), __float_as_uint(t.wa));
                 xs_next += xs_step;
             }
             float4 lo0, lo1;                                                   // samples i0, i0 + 1 of quad eg + cg

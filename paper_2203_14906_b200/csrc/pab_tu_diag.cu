@@ -1,5 +1,6 @@
 // pab_tu_diag.cu -- translation unit: the single-frame "diagonal" beamforming kernel (pab_diag.cuh) and its tables.
 #include <algorithm>
+#include <cmath>
 #include <vector>
 #include "pab_diag.cuh"
 #include "pab_launch.h"
@@ -43,7 +44,7 @@ int split_parts(int G, int npg, int nq_real, int parts, int* lo) {
 template <int K, int NPG, typename T>
 void launch_diag_t(const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale, cudaStream_t st) {
     dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, F);
-    const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b};
+    const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b, D.xs2_max};
     if (D.taps)
         bf_diag_kernel<K, NPG, T><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
     else
@@ -70,16 +71,20 @@ cudaError_t diag_attr(int smem_optin) {
 cudaError_t xl_diag_check(int order, const DiagSet& D, const float* rf, float* out, int N, int S, int nx, int nz, int* d_viol,
                           cudaStream_t st) {
     dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, 1);
-    const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b};
+    const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b, D.xs2_max};
     const size_t smem = (size_t)D.smem_bytes + 2 * D.cfg.quads * 4 + 128;
     cudaError_t e;
-    if (order <= 3) {
-        if ((e = cudaFuncSetAttribute(bf_diag_kernel<3, 4, float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        bf_diag_kernel<3, 4, float, true><<<grid, D.cfg.wpp * D.cfg.parts * 32, smem, st>>>(rf, out, D.cfg, tabs, N, S, nx, nz, 1.0f, d_viol);
-    } else {
-        if ((e = cudaFuncSetAttribute(bf_diag_kernel<5, 2, float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        bf_diag_kernel<5, 2, float, true><<<grid, D.cfg.wpp * D.cfg.parts * 32, smem, st>>>(rf, out, D.cfg, tabs, N, S, nx, nz, 1.0f, d_viol);
-    }
+    const unsigned threads = D.cfg.wpp * D.cfg.parts * 32;
+    auto run = [&](auto kernel) -> cudaError_t {
+        cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        kernel<<<grid, threads, smem, st>>>(rf, out, D.cfg, tabs, N, S, nx, nz, 1.0f, d_viol);
+        return cudaSuccess;
+    };
+    // the set's own form: with its tap table, or table-free (taps computed in the kernel)
+    if (order <= 3) e = D.taps ? run(bf_diag_kernel<3, 4, float, true, true>) : run(bf_diag_kernel<3, 4, float, true, false>);
+    else e = D.taps ? run(bf_diag_kernel<5, 2, float, true, true>) : run(bf_diag_kernel<5, 2, float, true, false>);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
@@ -105,7 +110,7 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
                           bool with_taps, DiagSet* D) {
     *D = DiagSet();
     const int P = 4 * npg;
-    if (N % 4 != 0 || N < 4 || q < 1 || q > 8) return cudaSuccess;
+    if (N % 4 != 0 || N < 4 || q < 1 || q > 16) return cudaSuccess;
     // Blocking, measured at C2 and C4: 32-row tiles of one column block, 8 warps per CTA (two CTAs
     // per SM at 128 registers); 16-row tiles, 2..16 warps and 2..4 column blocks per tile were all slower.
     constexpr int kRows = 32, kBlocks = 1, kWarps = 8;
@@ -137,7 +142,12 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     cfg.parts = best_parts;
     split_parts(G, npg, N / 4, cfg.parts, cfg.part_lo);
 
-    const DiagGeom geo{fs, c, (double)g.x0, (double)g.dx, (double)g.z0, (double)g.dz, N, S, g.nx, g.nz, q, P};
+    // lateral offsets (metres) of the first and last table column a real pair uses: d = q P (pixel 0, element N - 1) and
+    // d = nx - 1 + q (N - 1 + P) (pixel nx - 1, element 0)
+    const double half = (N - 1) / 2.0 * q;
+    const double ddx_lo = (double)g.x0 - half * (double)g.dx, ddx_hi = (double)g.x0 + ((double)(g.nx - 1) + half) * (double)g.dx;
+    const double ddx_max = std::max(std::fabs(ddx_lo), std::fabs(ddx_hi));
+    const DiagGeom geo{fs, c, (double)g.x0, (double)g.dx, (double)g.z0, (double)g.dz, N, S, g.nx, g.nz, q, P, ddx_max};
     const size_t tiles = (size_t)cfg.tiles_x * cfg.tiles_z, nq = tiles * cfg.quads;
     int* d_len = nullptr;
     cudaError_t e;
@@ -171,6 +181,7 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     D->xs_a = ((double)g.x0 - (double)q * ((N - 1) / 2.0 + P) * (double)g.dx) * fs / c;
     D->zs_b = (double)g.dz * fs / c;
     D->zs_a = (double)g.z0 * fs / c;
+    D->xs2_max = (ddx_max * fs / c) * (ddx_max * fs / c);
     return cudaDeviceSynchronize();
 }
 

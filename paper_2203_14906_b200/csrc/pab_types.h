@@ -93,6 +93,7 @@ struct DiagTables {
     // table-free variant (taps computed in the kernel, delay_tap_f64): lateral offset in samples of table column d is
     // xs_a + d xs_b, depth in samples of row m is zs_a + m zs_b
     double xs_a, xs_b, zs_a, zs_b;
+    double xs2_max;         // square of the largest lateral offset (samples) of a real (pixel, element) pair
 };
 
 // one set of device tables of the diagonal kernel (P = 16 pixels per thread for orders 1..3, P = 8 for orders 4, 5)
@@ -103,7 +104,7 @@ struct DiagSet {
     int* qoff = nullptr;
     int npg = 0;            // pixel groups of 4 per thread
     int smem_bytes = 0;     // dynamic shared memory per CTA; 0: not built / does not fit
-    double xs_a = 0.0, xs_b = 0.0, zs_a = 0.0, zs_b = 0.0;       // see DiagTables (set for both variants)
+    double xs_a = 0.0, xs_b = 0.0, zs_a = 0.0, zs_b = 0.0, xs2_max = 0.0;       // see DiagTables (set for both variants)
 };
 
 // nearest-sample delays (pab_nearest.cuh)

@@ -662,11 +662,17 @@ def test_delay_cache_ragged_int16_and_batches(pab, orc):
 @pytest.mark.parametrize("tables", ["single", "off"])
 @pytest.mark.parametrize("q,n_elem,nx,nz,frames,dtype", [(1, 16, 37, 70, 1, "float32"), (2, 24, 45, 33, 3, "float32"),
                                                          (3, 8, 50, 129, 2, "int16"), (2, 4, 7, 5, 1, "float32"),
-                                                         (1, 64, 130, 95, 2, "int16"), (4, 12, 64, 64, 1, "float32")])
+                                                         (1, 64, 130, 95, 2, "int16"), (4, 12, 64, 64, 1, "float32"),
+                                                         (16, 16, 300, 70, 1, "float32"), (12, 8, 100, 40, 2, "int16"),
+                                                         (8, 16, 300, 70, 1, "float32")])
 def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, nz, frames, dtype, tables):
     """The single-frame diagonal kernel (pitch = q dx exactly: one tap per diagonal, channel-quad staging from the caller's
     frame) on ragged grids: nx, nz off the tile sizes, arrays of 1..16 channel quads, q = 1..4, 1..3 frames, int16 input
-    with a scale, every order 1..5 (16 pixels per thread for orders 1..3, 8 for orders 4, 5)."""
+    with a scale, every order 1..5 (16 pixels per thread for orders 1..3, 8 for orders 4, 5); q = 12 and 16: one diagonal
+    part of 12 / 16 warps.  The wide ragged grids (q = 8, 16 with nx = 300) are the regression cases of an out-of-window read:
+    the pixel columns past nx of their last tile lie so far out that their delays run past the record, and before table
+    columns were clamped to those of real pairs (diag_ddx) the kernel gathered 1502 / 58514 samples outside the staged windows
+    for them (never stored, so parity could not see it; pab_self_check did)."""
     rng = np.random.default_rng(100 + 7 * q + n_elem)
     fs, c, S = 40e6, 1540.0, 900
     dx = 2.0 ** -13                                              # 0.122 mm: q dx is a float32 for every small q
@@ -696,7 +702,7 @@ def test_diagonal_kernel_ragged_translation_invariant(pab, orc, q, n_elem, nx, n
                 assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
             if tables == "off":                # delay cache off: the table-free form of the kernel (taps on the FP64 pipe)
                 assert bf.plan()["diagonal"] == 2
-        if dtype == "float32" and tables == "single":      # every shared-memory gather inside the staged window of its quad
+        if dtype == "float32":               # every shared-memory gather inside the staged window of its quad (both forms)
             for order in (3, 5):
                 if order <= n_elem:
                     assert bf.self_check(torch.from_numpy(rf[:1]).cuda(), order) == 0
@@ -776,17 +782,21 @@ def test_remainder_frames_take_the_diagonal_kernel(pab, orc, dtype, tables):
     assert np.max(np.abs(gpu - ref)[sel]) <= 0.05
 
 
+@pytest.mark.parametrize("tables", ["single", "off"])
 @pytest.mark.parametrize("cfg,order", [("C2", 3), ("C4", 5), ("C3", 1), ("C5", 4)])
-def test_diagonal_kernel_self_check_named_geometries(pab, cfg, order):
-    """pab_self_check on the geometries of the named configs (C5's with fp32 frames): no gather of the diagonal kernel
-    leaves the staged window of its channel quad (the check compute-sanitizer would make; it is closed on this pool)."""
+def test_diagonal_kernel_self_check_named_geometries(pab, cfg, order, tables):
+    """pab_self_check on the geometries of the named configs (C5's with fp32 frames): no gather of the diagonal kernel, in
+    the form with its tap table or in the table-free form, leaves the staged window of its channel quad (the check
+    compute-sanitizer would make; it is closed on this pool)."""
     g = synth.geometry(cfg)
     rng = np.random.default_rng(3)
     rf = rng.standard_normal((1, g.n_elem, g.n_samp)).astype(np.float32)
-    bf = pab.Beamformer(g, delay_cache="single")
+    bf = pab.Beamformer(g, delay_cache=tables)
     try:
-        assert bf.plan()["diagonal"] == 1
+        if tables == "single":
+            assert bf.plan()["diagonal"] == 1
         assert bf.self_check(torch.from_numpy(rf).cuda(), order) == 0
+        assert bf.plan()["diagonal"] == (1 if tables == "single" else 2)
     finally:
         bf.close()
 
