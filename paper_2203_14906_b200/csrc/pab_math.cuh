@@ -373,12 +373,15 @@ __device__ __forceinline__ Tap delay_tap(float xs2, float c0, const float4 row, 
 
 // The same step for in-range geometries on the FP64 pipe (B200: 64 lanes/clk/SM beside the FP32 pipes, otherwise idle in
 // this library): idx = sqrt(xs^2 + zs^2) from one MUFU.RSQ64H seed and one Newton step in double (relative error ~1e-12),
-// floor and fraction by the 1.5 * 2^52 rounding constant (the integer is the low word of the sum: no conversion
-// instruction, which would queue on the XU pipe beside the roots), the fraction's 23 leading bits moved into a float in
-// [1, 2) by a funnel shift.  15 instructions of which 10 on the FP64 pipe, against 23 on the FP32 / ALU pipes above.
+// then floor and fraction by two rounding constants, with no conversion instruction (F2I / F2F would queue on the XU pipe
+// beside the roots): M = 1.5 * 2^52 has ulp 1, so t = (idx - 1/2) + M holds floor(idx) in its low word (ties fall either
+// way); M2 = 1.5 * 2^29 has ulp 2^-23, so u = idx + ((M + M2) - t) = fraction + M2 (the inner difference is exact) holds
+// round(fraction * 2^23) = 0 .. 2^23 in its low word, and 0x3f800000 + that is the float 1 + fraction, up to 2.0 when the
+// fraction rounds to 1 or a tie went down: weight 1 on the upper sample, the same value.  11 instructions per call, 10 of
+// them on the FP64 pipe, against 23 on the FP32 / ALU pipes above.
 //   xs2d  the lateral offset squared, in samples^2 (double; warp-uniform, from the producer)
 //   zs    z fs / c (double)
-// Returns floor(idx) and the fraction in [0, 1] (1 only when idx is an integer to the last bit and the tie rounded down).
+// Returns floor(idx) (or floor(idx) - 1 with fraction 1) and the fraction in [0, 1], good to 2^-24 samples.
 __device__ __forceinline__ Tap delay_tap_f64(double xs2d, double zs) {
     const double q = fma(zs, zs, xs2d);
     double r;
@@ -386,14 +389,13 @@ __device__ __forceinline__ Tap delay_tap_f64(double xs2d, double zs) {
     double d = q * r;
     const double e = fma(-d, d, q);
     d = fma(e * r, 0.5, d);                                        // sqrt(q) to ~1e-12 relative
-    const double kM = 6755399441055744.0;                          // 1.5 * 2^52: adding it rounds to an integer
-    const double t = (d - 0.5) + kM;                               // low word = floor(d) (ties fall either way: the interpolant is continuous)
-    const double f1 = d - (t - (kM + 1.0));                        // fraction + 1, in [1, 2]
-    const int lo = __double2loint(f1), hi = __double2hiint(f1);
-    const float a1 = __int_as_float((__funnelshift_l(lo, hi, 3) & 0x007fffff) | 0x3f800000);
+    const double kM = 6755399441055744.0;                          // 1.5 * 2^52
+    const double kMM2 = 6755400246362112.0;                        // 1.5 * 2^52 + 1.5 * 2^29, exact
+    const double t = (d - 0.5) + kM;
+    const double u = d + (kMM2 - t);
     Tap o;
     o.i0 = __double2loint(t);
-    o.wa = (hi >= 0x40000000) ? 1.0f : a1 - 1.0f;                  // f1 = 2 exactly (a tie rounded down): weight 1
+    o.wa = __int_as_float(0x3f800000 + __double2loint(u)) - 1.0f;
     o.wb = 0.0f;
     return o;
 }
