@@ -1,4 +1,5 @@
-// pab_diag.cuh -- the single-frame beamforming kernel for translation-invariant geometries (calls of 1..3 frames).
+// pab_diag.cuh -- the single-frame beamforming kernel for translation-invariant geometries (calls of 1..3 frames, and the
+// 1..3 frames a longer call leaves over after its whole quads).
 //
 // With one frame per thread nothing amortises the tap fetch, the address and the loop of a (pixel, element) pair: the
 // frame-group kernels share them over 16 frames.  When the pitch is an exact integer multiple q of the column spacing
@@ -20,6 +21,11 @@
 // diagonals (EP parts, balanced on the host), and the partial power sums meet in shared memory before the Newton
 // combination (step a6).  Per (tile, staged quad) the window start and its place in shared memory come from tables
 // built once per geometry in fp64 with the same expression as the taps, so table and window agree exactly.
+//
+// Two forms.  TAB = true (delay cache on): the tap of every (table column d, row) comes from a table built with that
+// expression.  TAB = false (delay cache off: the default): no tap table; the kernel computes the tap of a diagonal itself
+// on the FP64 pipe (delay_tap_f64, one per (thread, diagonal), one diagonal ahead of its use), and the windows carry one
+// sample of margin because that evaluation agrees with the table expression to ~1e-9 samples, not to the bit.
 #pragma once
 #include <cstdint>
 #include <type_traits>
