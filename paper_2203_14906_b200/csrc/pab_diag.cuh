@@ -161,7 +161,12 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
     // lane = (row of the tile, column phase inside the warp); phase ph = residue ph % q of column block ph / q
     const int part = warp / C.wpp, wph = warp % C.wpp;
     const int ph = wph * (32 / C.rows) + lane / C.rows;
-    const int m = by * C.rows + lane % C.rows;
+    // 28-row tiles (row pitches in (1, 8/7] samples): seven rows per quarter-warp keep the 128-bit gathers of a quarter on
+    // 8 distinct bank groups; the eighth lane repeats its neighbour's row (same addresses: a broadcast) and stores nothing
+    const bool r7 = C.tile_rows != C.rows;
+    const int trow = r7 ? (lane >> 3) * 7 + min(lane & 7, 6) : lane % C.rows;
+    const bool live = !r7 || (lane & 7) != 7;
+    const int m = by * C.tile_rows + trow;
     const int j0 = bx * C.cols + (ph % C.q) + (ph / C.q) * (P * C.q);
     const int mc = min(m, nz - 1);
     float2 pp[P / 2][K];
@@ -286,7 +291,7 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
             for (int k = 0; k < K; ++k) p[k] += src[k * 32];
         }
         const int j = j0 + C.q * c;
-        if (j < nx && m < nz) out[(size_t)frame * img + (size_t)m * nx + j] = combine<K>(p);
+        if (live && j < nx && m < nz) out[(size_t)frame * img + (size_t)m * nx + j] = combine<K>(p);
     }
 }
 

@@ -122,7 +122,10 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     cfg.wpp = cfg.cp / lj;
     cfg.cols = P * cfg.cp;
     cfg.tiles_x = (g.nx + cfg.cols - 1) / cfg.cols;
-    cfg.tiles_z = (g.nz + cfg.rows - 1) / cfg.rows;
+    // seven rows per quarter-warp where eight would span nine samples (pab_pipe.cuh, tile_row): conflict-free gathers
+    const double zs_per_row = (double)g.dz * fs / c;
+    cfg.tile_rows = (cfg.rows == 32 && zs_per_row > 1.0 && zs_per_row <= 8.0 / 7.0 + 1e-9) ? 28 : cfg.rows;
+    cfg.tiles_z = (g.nz + cfg.tile_rows - 1) / cfg.tile_rows;
     cfg.quads = N / 4 + 2;
     cfg.nd = cfg.tiles_x * cfg.cols + q * (N + P + 4);
     if ((long long)cfg.nd * g.nz >= (1LL << 27) || cfg.wpp > kDiagMaxWarps) return cudaSuccess;
@@ -156,7 +159,7 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     if ((e = cudaMalloc(&D->qoff, (nq + tiles) * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
     if ((e = cudaMalloc(&d_len, nq * sizeof(int))) != cudaSuccess) { xl_diag_free(D); return e; }
     if (with_taps) diag_taps_kernel<<<dim3((g.nz + 255) / 256, cfg.nd), 256>>>(geo, D->taps);
-    diag_window_kernel<<<dim3((unsigned)tiles, cfg.quads), 256>>>(geo, cfg.rows, cfg.cols, cfg.tiles_x, cfg.quads, with_taps ? 0 : 1, D->qw0, d_len);
+    diag_window_kernel<<<dim3((unsigned)tiles, cfg.quads), 256>>>(geo, cfg.tile_rows, cfg.cols, cfg.tiles_x, cfg.quads, with_taps ? 0 : 1, D->qw0, d_len);
     std::vector<int> len(nq), off(nq + tiles);
     e = cudaMemcpy(len.data(), d_len, nq * sizeof(int), cudaMemcpyDeviceToHost);
     cudaFree(d_len);

@@ -76,6 +76,8 @@ constexpr int kDiagMaxParts = 16;
 struct DiagCfg {
     int q;                  // pitch / dx
     int rows;               // rows per tile = rows along a warp's lanes: 16 or 32; a warp holds 32 / rows column phases
+    int tile_rows;          // rows of a tile in use: rows, or 28 (rows = 32: seven rows per quarter-warp, the eighth lane repeats its
+                            // neighbour's row; tile_row in pab_pipe.cuh has the reason)
     int cp;                 // column phases per tile: lcm(q, 32 / rows); phase ph = residue ph % q of column block ph / q
     int wpp;                // warps per diagonal part: cp / (32 / rows)
     int parts;              // EP: diagonal parts; warps per CTA = wpp * parts

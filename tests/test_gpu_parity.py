@@ -783,6 +783,37 @@ def test_remainder_frames_take_the_diagonal_kernel(pab, orc, dtype, tables):
 
 
 @pytest.mark.parametrize("tables", ["single", "off"])
+def test_diagonal_kernel_28_row_tiles(pab, orc, tables):
+    """Row pitches in (1, 8/7] samples (config C2's 1.14): the diagonal kernel takes tiles of 28 rows, seven per quarter-warp
+    with the eighth lane idle, so that the gathers of a quarter-warp never meet in a bank group.  A ragged grid (61 rows:
+    two whole tiles and 5 rows), 1 and 3 frames, orders 1..5, both forms of the kernel, and its bounds check."""
+    rng = np.random.default_rng(28)
+    fs, c, q, n_elem, nx, nz, S = 40e6, 1540.0, 2, 24, 45, 61, 900
+    dx = 2.0 ** -13
+    g = synth.Geometry(n_elem, S, fs, c, float(np.float32(q * np.float64(dx))), nx, nz, -(nx - 1) / 2 * dx + 0.3 * dx, dx, 2.1e-3,
+                       1.1 * c / fs).f32()
+    assert 1.0 < float(g.dz) * fs / c <= 8.0 / 7.0
+    base = [(rng.uniform(-1e-3, 1e-3), rng.uniform(2.5e-3, 4.5e-3), 1.0, 0.0) for _ in range(3)]
+    rf, _ = synth._frames(rng, g, base, 5e6, 3, 20.0, True)
+    bf = pab.Beamformer(g, delay_cache=tables)
+    try:
+        assert bf.plan()["in_range"] == 1
+        for frames in (1, 3):
+            for order in (1, 2, 3, 4, 5):
+                out = bf.beamform(torch.from_numpy(rf[:frames]).cuda(), order)
+                torch.cuda.synchronize()
+                gpu = out.cpu().numpy().astype(np.float64)
+                ref = orc.beamform(rf[:frames], g, order)
+                for f in range(frames):
+                    assert check_raw(gpu[f], ref[f], order) <= 2.5e-5
+        assert bf.plan()["diagonal"] == (1 if tables == "single" else 2)
+        for order in (3, 5):
+            assert bf.self_check(torch.from_numpy(rf[:1]).cuda(), order) == 0
+    finally:
+        bf.close()
+
+
+@pytest.mark.parametrize("tables", ["single", "off"])
 @pytest.mark.parametrize("cfg,order", [("C2", 3), ("C4", 5), ("C3", 1), ("C5", 4)])
 def test_diagonal_kernel_self_check_named_geometries(pab, cfg, order, tables):
     """pab_self_check on the geometries of the named configs (C5's with fp32 frames): no gather of the diagonal kernel, in
