@@ -133,7 +133,10 @@ int pab_set_weight(pab_ctx* ctx, int weight);
  * integer delay; reading A21): the delayed sample is the nearest RF sample, 0 outside the record.  The
  * signed k-th root is then taken once per RF sample while the frames are staged and the integer delays come from a
  * delay table in device memory (the paper's own arrangement), built here in fp64 with the oracle's
- * expression: n_elem * nx * nz uint16 entries.  Synchronises the device on the first call.
+ * expression: n_elem * nx * nz uint16 entries.  On translation-invariant in-range geometries (pitch_m an exact integer
+ * multiple q <= 16 of grid.dx, n_elem a multiple of 4) calls of 1..3 frames instead run the single-frame diagonal kernel on a
+ * compact table of the same fp64 decisions, one per (column - q * element, row), roots taken per item.  Synchronises the
+ * device on the first call.
  * Errors: PAB_ERR_INVALID (n_samp > 65534, or combined with PAB_WEIGHT_CF), PAB_ERR_ALLOC, PAB_ERR_CUDA. */
 int pab_set_interp(pab_ctx* ctx, int interp);
 

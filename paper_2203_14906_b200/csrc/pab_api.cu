@@ -44,6 +44,7 @@ struct pab_ctx {
     DiagSet diag[2];                     // single-frame diagonal kernel: [0] orders 1..3 (16 pixels per thread), [1] orders 4, 5 (8)
     DiagSet diag_nt[2];                  // the same for the table-free variant (delay cache off): windows only, taps in-kernel
     bool diag_nt_tried = false;
+    DiagSet diag_near[2];                // the same kernel for the nearest-sample path (row f4): tables of floor(idx + 1/2), fraction 0
     void* d_metric = nullptr;            // MetricAcc + double[1] + 2 x 4096 histogram bins (row f3), lazy
     unsigned short* d_near = nullptr;    // nearest-sample index table [N][nx][nz] (row f4), built by pab_set_interp
     pab_plan_info plan{};
@@ -94,6 +95,7 @@ void free_all(pab_ctx* ctx) {
     cudaFree(ctx->d_taps_bp); cudaFree(ctx->d_taps_h); cudaFree(ctx->d_max); cudaFree(ctx->d_near); cudaFree(ctx->d_metric); cudaFree(ctx->d_taps); cudaFree(ctx->d_w0s); cudaFree(ctx->d_compact); cudaFree(ctx->d_taps7); cudaFree(ctx->d_w0s7);
     xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]);
     xl_diag_free(&ctx->diag_nt[0]); xl_diag_free(&ctx->diag_nt[1]);
+    xl_diag_free(&ctx->diag_near[0]); xl_diag_free(&ctx->diag_near[1]);
     for (int b = 0; b < kHostSets; ++b) {
         cudaFree(ctx->d_in[b]); cudaFree(ctx->d_out[b]);
         if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
@@ -120,10 +122,10 @@ bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
         const long long q = llround((double)ctx->pitch / (double)ctx->grid.dx);
         if (ctx->plan.in_range && ctx->plan.smem_bytes > 0 && q >= 1 && q <= 16 && (double)ctx->pitch == (double)q * (double)ctx->grid.dx &&
             xl_diag_configure(ctx->smem_optin) == cudaSuccess) {
-            cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 4, 3, ctx->smem_optin, false,
+            cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 4, 3, ctx->smem_optin, 1,
                                           &ctx->diag_nt[0]);
             if (e == cudaSuccess)
-                e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 2, 5, ctx->smem_optin, false, &ctx->diag_nt[1]);
+                e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 2, 5, ctx->smem_optin, 1, &ctx->diag_nt[1]);
             if (e != cudaSuccess) {          // not fatal: the call keeps the one-frame-per-thread kernels
                 cudaGetLastError();
                 xl_diag_free(&ctx->diag_nt[0]); xl_diag_free(&ctx->diag_nt[1]);
@@ -368,8 +370,8 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
     if (mode != PAB_CACHE_OFF && ctx->d_compact && ctx->diag[0].smem_bytes == 0 && ctx->diag[1].smem_bytes == 0) {
         PAB_CUDA(ctx, xl_diag_configure(ctx->smem_optin));
         cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q,
-                                      4, 3, ctx->smem_optin, true, &ctx->diag[0]);
-        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, true, &ctx->diag[1]);
+                                      4, 3, ctx->smem_optin, 0, &ctx->diag[0]);
+        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, 0, &ctx->diag[1]);
         if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
         ctx->launches += 4;
     }
@@ -414,6 +416,24 @@ int pab_set_interp(pab_ctx* ctx, int interp) {
             ctx->launches++;
             cudaError_t e = cudaDeviceSynchronize();
             if (e != cudaSuccess) { cudaFree(ctx->d_near); ctx->d_near = nullptr; return cuda_fail(ctx, e, "nearest table"); }
+        }
+        // Calls of 1..3 frames on translation-invariant in-range geometries: the single-frame diagonal kernel (pab_diag.cuh)
+        // with a table of floor(idx + 1/2) and fraction 0, so that its interpolation returns rf[n] exactly and one integer
+        // delay serves the 16 (8) pairs of a diagonal; the decision is taken in fp64 by the same expression as the uint16
+        // table's.  Not fatal when the sets cannot be had: such calls keep the frame-group kernels.
+        if (ctx->diag_near[0].smem_bytes == 0 && ctx->diag_near[1].smem_bytes == 0) {
+            const long long q = llround((double)ctx->pitch / (double)ctx->grid.dx);
+            if (ctx->plan.in_range && ctx->plan.smem_bytes > 0 && q >= 1 && q <= 16 &&
+                (double)ctx->pitch == (double)q * (double)ctx->grid.dx && xl_diag_configure(ctx->smem_optin) == cudaSuccess) {
+                cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 4, 3, ctx->smem_optin, 2,
+                                              &ctx->diag_near[0]);
+                if (e == cudaSuccess)
+                    e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 2, 5, ctx->smem_optin, 2, &ctx->diag_near[1]);
+                if (e != cudaSuccess) { cudaGetLastError(); xl_diag_free(&ctx->diag_near[0]); xl_diag_free(&ctx->diag_near[1]); }
+                else ctx->launches += 4;
+            } else {
+                cudaGetLastError();
+            }
         }
     }
     ctx->interp = interp;

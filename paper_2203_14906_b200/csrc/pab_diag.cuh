@@ -40,6 +40,7 @@ struct DiagGeom {
     double fs, c, x0, dx, z0, dz;
     int N, S, nx, nz, q, P;
     double ddx_max;         // largest |pixel column - element| (metres) of a real pair: max over table columns q P and nx - 1 + q (N - 1 + P)
+    int nearest;            // 1: the table holds floor(idx + 1/2) with fraction 0 (row f4: integer delays, reading A21)
 };
 // lateral offset (pixel column - element) of table column d: d = j - q i + q (N - 1 + P), x_j - x_i = x0 + j dx - (i - (N-1)/2) q dx
 // Table columns beyond those of the real pairs belong only to pairs that do not exist (pixel columns past nx in a ragged last
@@ -61,6 +62,10 @@ __global__ void __launch_bounds__(256) diag_taps_kernel(const DiagGeom G, uint2*
     const int m = blockIdx.x * blockDim.x + threadIdx.x, d = blockIdx.y;
     if (m >= G.nz) return;
     const double idx = diag_idx(G, d, m);
+    if (G.nearest) {            // the integer decision of the nearest-sample path, taken here in fp64 like its uint16 table's
+        taps[(size_t)d * G.nz + m] = make_uint2((unsigned)(int)floor(__dadd_rn(idx, 0.5)), 0u);
+        return;
+    }
     const double fl = floor(idx);
     taps[(size_t)d * G.nz + m] = make_uint2((unsigned)(int)fl, __float_as_uint((float)(idx - fl)));
 }
@@ -84,7 +89,8 @@ __global__ void __launch_bounds__(256) diag_window_kernel(const DiagGeom G, int 
         const int col = t % cols, ch = (t / cols) % 4, top = t / (cols * 4);
         const int j = bx * cols + col, i = (sq - 1) * 4 + ch;
         const int d = j - G.q * i + G.q * (G.N - 1 + G.P);
-        const int fl = (int)floor(diag_idx(G, d, top ? r_hi : r_lo));
+        const double ix = diag_idx(G, d, top ? r_hi : r_lo);
+        const int fl = (int)floor(G.nearest ? __dadd_rn(ix, 0.5) : ix);
         lo = min(lo, fl); hi = max(hi, fl);
     }
     atomicMin(&s_min, lo);

@@ -28,7 +28,7 @@ void xl_build_delay_compact(const CacheGeom& G, int q, int nd, uint2* compact);
 // ---- pab_tu_diag.cu: single frames on translation-invariant geometries ----
 cudaError_t xl_diag_configure(int smem_optin);
 cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, int q, int npg, int max_order, int smem_limit,
-                          bool with_taps, DiagSet* D);
+                          int mode, DiagSet* D);      // mode 0: tap table, 1: table-free (windows only), 2: nearest-sample table
 void xl_diag_free(DiagSet* D);
 cudaError_t xl_diag_check(int order, const DiagSet& D, const float* rf, float* out, int N, int S, int nx, int nz, int* d_viol,
                           cudaStream_t st);

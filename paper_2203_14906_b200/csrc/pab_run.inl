@@ -34,7 +34,12 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
     const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
                             (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0);
 
-    if (ctx->interp == PAB_INTERP_NEAREST) {
+    if (ctx->interp == PAB_INTERP_NEAREST && F < 4 && use_staged && order <= 5 && ctx->diag_near[order <= 3 ? 0 : 1].smem_bytes > 0) {
+        // row f4, calls of 1..3 frames on translation-invariant geometries: the diagonal kernel on its table of integer delays
+        // (fraction 0: the interpolation returns rf[n] exactly), straight from the caller's frames; roots per item
+        Span sp(ctx, PAB_STAGE_BEAMFORM, st);
+        xl_diag(order, ctx->dtype, ctx->diag_near[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
+    } else if (ctx->interp == PAB_INTERP_NEAREST) {
         // row f4: rooted quad staging, then the table-driven gather kernel (always the quad layout)
         {
             Span sp(ctx, PAB_STAGE_INGEST, st);

@@ -105,9 +105,12 @@ void xl_diag_free(DiagSet* D) {
 // Build the tables of one set (npg = 4: orders 1..3, npg = 2: orders 4, 5).  Leaves D->smem_bytes = 0 when the geometry
 // does not qualify (N not a multiple of 4, too many warps, a tile that does not fit in shared memory); returns a CUDA
 // error only for failed calls.  Synchronises the device.
-// with_taps = false: the set of the table-free variant: windows only, one sample of margin on either side.
+// mode 0: tap table + windows; 1: the set of the table-free variant: windows only, one sample of margin on either side;
+// 2: the table of the nearest-sample path (row f4): floor(idx + 1/2) with fraction 0, so that the same kernel reads
+// s = rf[n] exactly.
 cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, int q, int npg, int max_order, int smem_limit,
-                          bool with_taps, DiagSet* D) {
+                          int mode, DiagSet* D) {
+    const bool with_taps = mode != 1;
     *D = DiagSet();
     const int P = 4 * npg;
     if (N % 4 != 0 || N < 4 || q < 1 || q > 16) return cudaSuccess;
@@ -150,7 +153,7 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     const double half = (N - 1) / 2.0 * q;
     const double ddx_lo = (double)g.x0 - half * (double)g.dx, ddx_hi = (double)g.x0 + ((double)(g.nx - 1) + half) * (double)g.dx;
     const double ddx_max = std::max(std::fabs(ddx_lo), std::fabs(ddx_hi));
-    const DiagGeom geo{fs, c, (double)g.x0, (double)g.dx, (double)g.z0, (double)g.dz, N, S, g.nx, g.nz, q, P, ddx_max};
+    const DiagGeom geo{fs, c, (double)g.x0, (double)g.dx, (double)g.z0, (double)g.dz, N, S, g.nx, g.nz, q, P, ddx_max, mode == 2 ? 1 : 0};
     const size_t tiles = (size_t)cfg.tiles_x * cfg.tiles_z, nq = tiles * cfg.quads;
     int* d_len = nullptr;
     cudaError_t e;

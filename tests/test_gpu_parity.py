@@ -463,6 +463,48 @@ def test_nearest_ragged_int16_and_scale(pab, orc, variant):
             check_raw(gpu[f], ref[f], order)
 
 
+@pytest.mark.parametrize("dtype", ["float32", "int16"])
+def test_nearest_single_frames_take_the_diagonal_kernel(pab, orc, dtype):
+    """Row f4 in calls of 1..3 frames on translation-invariant in-range geometries: the single-frame diagonal kernel on a table
+    of floor(idx + 1/2) with fraction 0 (one integer delay per diagonal of pairs; its interpolation then returns rf[n]
+    exactly).  Integer decisions bit for bit on a sample-index ramp (ragged grid, 28-row tiles, q = 2; and config C2),
+    orders 1..5 on noisy frames, fp32 and int16 with a scale."""
+    rng = np.random.default_rng(44)
+    fs, c, q, n_elem, nx, nz, S = 40e6, 1540.0, 2, 24, 45, 61, 900
+    dx = 2.0 ** -13
+    g = synth.Geometry(n_elem, S, fs, c, float(np.float32(q * np.float64(dx))), nx, nz, -(nx - 1) / 2 * dx + 0.3 * dx, dx, 2.1e-3,
+                       1.1 * c / fs).f32()
+    ramp = np.tile(np.arange(S, dtype=np.float32), (2, n_elem, 1))
+    scale = 1.0
+    base = [(rng.uniform(-1e-3, 1e-3), rng.uniform(2.5e-3, 4.5e-3), 1.0, 0.0) for _ in range(3)]
+    rf, _ = synth._frames(rng, g, base, 5e6, 3, 20.0, True)
+    if dtype == "int16":
+        ramp, rf, scale = ramp.astype(np.int16), np.rint(rf * 4000.0).astype(np.int16), 0.25
+    bf = pab.Beamformer(g, dtype=dtype, scale=scale, interp="nearest")
+    try:
+        assert bf.plan()["in_range"] == 1
+        n0 = bf.launch_count()
+        out = bf.beamform(torch.from_numpy(ramp).cuda(), 1)
+        torch.cuda.synchronize()
+        assert bf.launch_count() - n0 == 1                         # one kernel, no ingest pass: the diagonal kernel
+        assert np.array_equal(out.cpu().numpy().astype(np.float64), orc.beamform_ex(ramp, g, 1, interp="nearest", scale=scale))
+        for frames in (1, 3):
+            for order in (1, 2, 3, 4, 5):
+                out = bf.beamform(torch.from_numpy(rf[:frames]).cuda(), order)
+                torch.cuda.synchronize()
+                gpu = out.cpu().numpy().astype(np.float64)
+                ref = orc.beamform_ex(rf[:frames], g, order, interp="nearest", scale=scale)
+                for f in range(frames):
+                    assert check_raw(gpu[f], ref[f], order) <= 2e-5
+    finally:
+        bf.close()
+    if dtype == "float32":
+        w = synth.make_config("C2")
+        for order in (1, 2, 3):
+            gpu, launches = run_gpu(pab, w.geom, w.rf, order, interp="nearest")
+            assert check_raw(gpu[0], orc.beamform_ex(w.rf, w.geom, order, interp="nearest")[0], order) <= 2e-5
+
+
 def test_nearest_c2b_batch_and_post_chain(pab, orc):
     w = synth.make_config("C2b", n_frames=20)
     g = w.geom
