@@ -443,7 +443,8 @@ def run_sweep(args):
               ("C2b", 64, (1, 2, 3), False, "cache-all"), ("C4", 16, (4, 5), False, "cache-all"),
               ("C2b", 64, (3,), False, "cf-cache-all"), ("C4", 16, (5,), False, "cf-cache-all"),
               ("C2b", 64, (6, 8), False, "cache-all"),
-              ("C3", 256, (3,), True, "cache-all"), ("C5", 1024, (3,), True, "cache-all")]
+              ("C3", 256, (3,), True, "cache-all"), ("C5", 1024, (3,), True, "cache-all"),
+              ("C2", 1, (1, 2, 3), False, "nearest"), ("C4", 1, (4, 5), False, "nearest")]
     if args.case:                         # --case C2:1:cache-single[:3]  ->  one config / frame count / mode [/ order]
         want = args.case.split(":")
         cases = [c for c in cases if c[0] == want[0] and str(c[1]) == want[1] and c[4] == want[2]]
@@ -503,6 +504,8 @@ def run_sweep(args):
             fp = _FP32[order][0] + (0.0 if taps_from_table else _FP32[order][1] / batch) + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
             if interp == "nearest":
                 fp = {1: 1.0, 2: 3.0, 3: 4.0, 4: 5.0, 5: 7.0}[order]
+                if F < 4 and bf.plan()["diagonal"] == 1:      # single frames on the diagonal kernel: roots per item, not per RF sample
+                    xu = _XU[order][0]
             if diag_share:
                 fp = _FP32[order][0] + _FP32[order][1] / diag_share
             t_xu = items * F * xu / (SM_COUNT * XU_LANES_PER_CLK_SM * f_hz) * 1e3

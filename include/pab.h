@@ -84,7 +84,8 @@ typedef struct {
     int   in_range;              /* 1 when every (pixel, element) delay index lies inside the record and z0 is at
                                     least one sample deep: the kernels then skip the out-of-record masks (A6)     */
     int   diagonal;              /* single-frame diagonal kernel (translation-invariant geometry: pitch an exact integer
-                                    multiple q <= 16 of dx, in range): 1 once pab_set_delay_cache has built its tap tables;
+                                    multiple q <= 16 of dx, in range): 1 once pab_set_delay_cache (or pab_set_interp, for the
+                                    nearest-sample path) has built its tap tables;
                                     2 once a call of 1..3 frames with the delay cache off has built the windows of its
                                     table-free form (taps computed in the kernel); else 0                             */
     double zs_per_row;           /* dz * fs / c : delay samples per pixel row                                      */

@@ -437,6 +437,8 @@ int pab_set_interp(pab_ctx* ctx, int interp) {
         }
     }
     ctx->interp = interp;
+    if (interp == PAB_INTERP_NEAREST && (ctx->diag_near[0].smem_bytes > 0 || ctx->diag_near[1].smem_bytes > 0) && ctx->plan.diagonal == 0)
+        ctx->plan.diagonal = 1;
     return PAB_OK;
 }
 
