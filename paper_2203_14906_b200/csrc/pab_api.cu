@@ -114,6 +114,14 @@ void free_all(pab_ctx* ctx) {
 // the 16 or 8 pairs of the diagonal).  It needs no delay table, only the window of every (tile, channel quad), a few
 // hundred KB built on the first such call (one device synchronisation, skipped while the stream is being captured).
 // Returns whether the set of this order is there.
+// pab_plan_info.diagonal: which form of the single-frame diagonal kernel the context's current settings would run
+void refresh_diagonal_flag(pab_ctx* ctx) {
+    auto has = [](const DiagSet (&d)[2]) { return d[0].smem_bytes > 0 || d[1].smem_bytes > 0; };
+    if (ctx->interp == PAB_INTERP_NEAREST) ctx->plan.diagonal = has(ctx->diag_near) ? 1 : 0;
+    else if (ctx->cache_mode != PAB_CACHE_OFF) ctx->plan.diagonal = has(ctx->diag) ? 1 : 0;
+    else ctx->plan.diagonal = has(ctx->diag_nt) ? 2 : 0;
+}
+
 bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
     if (!ctx->diag_nt_tried) {
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -131,7 +139,7 @@ bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
                 xl_diag_free(&ctx->diag_nt[0]); xl_diag_free(&ctx->diag_nt[1]);
             } else {
                 ctx->launches += 2;
-                if (ctx->plan.diagonal == 0 && (ctx->diag_nt[0].smem_bytes > 0 || ctx->diag_nt[1].smem_bytes > 0)) ctx->plan.diagonal = 2;
+                refresh_diagonal_flag(ctx);
             }
         } else {
             cudaGetLastError();
@@ -375,9 +383,8 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
         if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
         ctx->launches += 4;
     }
-    ctx->plan.diagonal = (mode != PAB_CACHE_OFF && (ctx->diag[0].smem_bytes > 0 || ctx->diag[1].smem_bytes > 0)) ? 1
-                         : (ctx->diag_nt[0].smem_bytes > 0 || ctx->diag_nt[1].smem_bytes > 0) ? 2 : 0;
     ctx->cache_mode = mode;
+    refresh_diagonal_flag(ctx);
     return PAB_OK;
 }
 
@@ -437,8 +444,7 @@ int pab_set_interp(pab_ctx* ctx, int interp) {
         }
     }
     ctx->interp = interp;
-    if (interp == PAB_INTERP_NEAREST && (ctx->diag_near[0].smem_bytes > 0 || ctx->diag_near[1].smem_bytes > 0) && ctx->plan.diagonal == 0)
-        ctx->plan.diagonal = 1;
+    refresh_diagonal_flag(ctx);
     return PAB_OK;
 }
 
