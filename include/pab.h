@@ -251,7 +251,8 @@ int pab_set_profile(pab_ctx* ctx, int max_launches);
 int pab_get_profile(pab_ctx* ctx, int stage, double* total_ms, long long* n_launches, int reset);
 
 /* pab_self_check -- diagnostic for the single-frame diagonal kernel (fp32 input; with the delay cache on: the form with its
- * tap table, pab_plan_info.diagonal == 1; with it off and the automatic variant: the table-free form, == 2): runs one
+ * tap table, pab_plan_info.diagonal == 1; with it off and the automatic variant: the table-free form, == 2; under
+ * PAB_INTERP_NEAREST: the form on its table of integer delays): runs one
  * frame through an instantiation that compares every shared-memory gather of its element loop with the staged window of
  * the channel quad it reads from, and returns the number of out-of-window accesses (0 for a correct build).  Stands in
  * for compute-sanitizer's memcheck, which is closed on the GPU pool this library was developed on.  order 1..5 selects

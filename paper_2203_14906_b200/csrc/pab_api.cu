@@ -391,8 +391,10 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
 int pab_self_check(pab_ctx* ctx, const float* rf_dev, int order, long long* violations) {
     if (!ctx || !rf_dev || !violations || order < 1 || order > 5) return PAB_ERR_INVALID;
     // delay cache on: the kernel with its tap table; off: its table-free form (built here if no call has built it yet)
-    if (ctx->cache_mode == PAB_CACHE_OFF && (ctx->variant != PAB_VARIANT_AUTO || !ensure_diag_nt(ctx, order, 0))) return PAB_ERR_INVALID;
-    const DiagSet& D = ctx->cache_mode == PAB_CACHE_OFF ? ctx->diag_nt[order <= 3 ? 0 : 1] : ctx->diag[order <= 3 ? 0 : 1];
+    const bool near = ctx->interp == PAB_INTERP_NEAREST;        // the nearest-sample path: the kernel on its table of integer delays
+    if (!near && ctx->cache_mode == PAB_CACHE_OFF && (ctx->variant != PAB_VARIANT_AUTO || !ensure_diag_nt(ctx, order, 0))) return PAB_ERR_INVALID;
+    const DiagSet& D = near ? ctx->diag_near[order <= 3 ? 0 : 1]
+                            : ctx->cache_mode == PAB_CACHE_OFF ? ctx->diag_nt[order <= 3 ? 0 : 1] : ctx->diag[order <= 3 ? 0 : 1];
     if (D.smem_bytes == 0 || ctx->dtype != PAB_F32) return PAB_ERR_INVALID;
     float* out = nullptr;
     int* d_viol = nullptr;

@@ -496,6 +496,10 @@ def test_nearest_single_frames_take_the_diagonal_kernel(pab, orc, dtype):
                 ref = orc.beamform_ex(rf[:frames], g, order, interp="nearest", scale=scale)
                 for f in range(frames):
                     assert check_raw(gpu[f], ref[f], order) <= 2e-5
+        if dtype == "float32":                 # no gather outside the staged windows (built from the rounded indices)
+            assert bf.plan()["diagonal"] == 1
+            for order in (3, 5):
+                assert bf.self_check(torch.from_numpy(rf[:1]).cuda(), order) == 0
     finally:
         bf.close()
     if dtype == "float32":
