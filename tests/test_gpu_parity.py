@@ -666,6 +666,46 @@ def test_beamform_is_cuda_graph_capturable(pab, orc):
         bf.close()
 
 
+def test_single_frame_default_path_under_graph_capture(pab, orc):
+    """The table-free diagonal kernel builds its windows on the first 1..3-frame call (a device synchronisation), which must not
+    happen inside a stream capture: a context whose FIRST such call is captured keeps the one-frame-per-thread kernel for
+    it (and stays correct), builds the windows on its next eager call, and a capture made after that replays the diagonal
+    kernel."""
+    rng = np.random.default_rng(91)
+    dx = 2.0 ** -13
+    g = synth.Geometry(16, 900, 40e6, 1540.0, 2 * dx, 37, 70, -18 * dx, dx, 2.1e-3, 0.09e-3).f32()
+    base = [(rng.uniform(-1e-3, 1e-3), rng.uniform(3e-3, 8e-3), 1.0, 0.0) for _ in range(3)]
+    rf_np, _ = synth._frames(rng, g, base, 5e6, 1, 20.0, True)
+    ref = orc.beamform(rf_np, g, 3)[0]
+    bf = pab.Beamformer(g)
+    try:
+        rf = torch.from_numpy(rf_np).cuda()
+        out = torch.empty((1, g.nz, g.nx), device="cuda")
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            bf.beamform(rf, 3, out=out, stream=s)            # first call of the context: captured, no set-up allowed
+        assert bf.plan()["diagonal"] == 0
+        out.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        check_raw(out.cpu().numpy().astype(np.float64)[0], ref, 3)
+        eager = bf.beamform(rf, 3)                           # eager call: builds the windows, runs the diagonal kernel
+        torch.cuda.synchronize()
+        assert bf.plan()["diagonal"] == 2
+        check_raw(eager.cpu().numpy().astype(np.float64)[0], ref, 3)
+        graph2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph2, stream=s):
+            bf.beamform(rf, 3, out=out, stream=s)
+        out.zero_()
+        graph2.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager)
+    finally:
+        bf.close()
+
+
 # ---- cached interpolation taps (pab_set_delay_cache): the paper's delay table where it wins ----
 @pytest.mark.parametrize("order", [1, 2, 3, 4, 5])
 def test_delay_cache_single_frames_c2(pab, orc, order):
