@@ -122,7 +122,7 @@ void refresh_diagonal_flag(pab_ctx* ctx) {
     else ctx->plan.diagonal = has(ctx->diag_nt) ? 2 : 0;
 }
 
-bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
+bool ensure_diag_nt(pab_ctx* ctx, int set, cudaStream_t st) {        // set 0: 16 pixels per thread (orders 1..3), 1: 8 pixels
     if (!ctx->diag_nt_tried) {
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
         if (cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
@@ -133,7 +133,7 @@ bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
             cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 4, 3, ctx->smem_optin, 1,
                                           &ctx->diag_nt[0]);
             if (e == cudaSuccess)
-                e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 2, 5, ctx->smem_optin, 1, &ctx->diag_nt[1]);
+                e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, (int)q, 2, 6, ctx->smem_optin, 1, &ctx->diag_nt[1]);
             if (e != cudaSuccess) {          // not fatal: the call keeps the one-frame-per-thread kernels
                 cudaGetLastError();
                 xl_diag_free(&ctx->diag_nt[0]); xl_diag_free(&ctx->diag_nt[1]);
@@ -145,7 +145,7 @@ bool ensure_diag_nt(pab_ctx* ctx, int order, cudaStream_t st) {
             cudaGetLastError();
         }
     }
-    return ctx->diag_nt[order <= 3 ? 0 : 1].smem_bytes > 0;
+    return ctx->diag_nt[set].smem_bytes > 0;
 }
 
 // Orders 1 and 2 in frame groups are bound by the shared-memory data pipe, and at row pitches in (1, 8/7] samples 64-row
@@ -379,7 +379,7 @@ int pab_set_delay_cache(pab_ctx* ctx, int mode) {
         PAB_CUDA(ctx, xl_diag_configure(ctx->smem_optin));
         cudaError_t e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q,
                                       4, 3, ctx->smem_optin, 0, &ctx->diag[0]);
-        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 5, ctx->smem_optin, 0, &ctx->diag[1]);
+        if (e == cudaSuccess) e = xl_diag_build(ctx->N, ctx->S, (double)ctx->fs, (double)ctx->c, ctx->grid, ctx->cache_q, 2, 6, ctx->smem_optin, 0, &ctx->diag[1]);
         if (e != cudaSuccess) { xl_diag_free(&ctx->diag[0]); xl_diag_free(&ctx->diag[1]); return cuda_fail(ctx, e, "diagonal tables"); }
         ctx->launches += 4;
     }
@@ -392,7 +392,7 @@ int pab_self_check(pab_ctx* ctx, const float* rf_dev, int order, long long* viol
     if (!ctx || !rf_dev || !violations || order < 1 || order > 5) return PAB_ERR_INVALID;
     // delay cache on: the kernel with its tap table; off: its table-free form (built here if no call has built it yet)
     const bool near = ctx->interp == PAB_INTERP_NEAREST;        // the nearest-sample path: the kernel on its table of integer delays
-    if (!near && ctx->cache_mode == PAB_CACHE_OFF && (ctx->variant != PAB_VARIANT_AUTO || !ensure_diag_nt(ctx, order, 0))) return PAB_ERR_INVALID;
+    if (!near && ctx->cache_mode == PAB_CACHE_OFF && (ctx->variant != PAB_VARIANT_AUTO || !ensure_diag_nt(ctx, order <= 3 ? 0 : 1, 0))) return PAB_ERR_INVALID;
     const DiagSet& D = near ? ctx->diag_near[order <= 3 ? 0 : 1]
                             : ctx->cache_mode == PAB_CACHE_OFF ? ctx->diag_nt[order <= 3 ? 0 : 1] : ctx->diag[order <= 3 ? 0 : 1];
     if (D.smem_bytes == 0 || ctx->dtype != PAB_F32) return PAB_ERR_INVALID;

@@ -115,11 +115,14 @@ template <typename T> __device__ __forceinline__ float diag_ld(const T* p) { ret
 // the most intricate of the library).
 // TAB = false: no tap table; the tap of a diagonal comes from delay_tap_f64 (FP64 pipe), computed one diagonal ahead the
 // way the table variant prefetches it: 13 instructions per (thread, diagonal), shared by the thread's P pairs.
-template <int K, int NPG, typename T, bool CHK = false, bool TAB = true>
+// W = 1: coherence-factor weighting (row f1): the accumulator row of a pixel grows by sum s^2 (and sum s for even K), and
+// the epilogue multiplies e_k by (sum s)^2 / (N sum s^2) (combine_w); 8 pixels per thread for every order.
+template <int K, int NPG, typename T, bool CHK = false, bool TAB = true, int W = 0>
 __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T* __restrict__ rf, float* __restrict__ out,
                                                                           const DiagCfg C, const DiagTables D, int N, int S,
                                                                           int nx, int nz, float scale, int* __restrict__ viol = nullptr) {
     constexpr int P = 4 * NPG;
+    constexpr int A = kAcc<K, W>;                    // accumulators per pixel
     extern __shared__ __align__(128) unsigned char dg_smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_warps = blockDim.x >> 5;
@@ -175,11 +178,11 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
     const int m = by * C.tile_rows + trow;
     const int j0 = bx * C.cols + (ph % C.q) + (ph / C.q) * (P * C.q);
     const int mc = min(m, nz - 1);
-    float2 pp[P / 2][K];
+    float2 pp[P / 2][A];
 #pragma unroll
     for (int f = 0; f < P / 2; ++f)
 #pragma unroll
-        for (int k = 0; k < K; ++k) pp[f][k] = make_float2(0.0f, 0.0f);
+        for (int k = 0; k < A; ++k) pp[f][k] = make_float2(0.0f, 0.0f);
     const int n_quads_real = C.quads - 2;
     // Tap of diagonal e = 4 eg + r: table column d = j0 - q e + q (N - 1 + P), i.e. entry t0 - f * tstep for the flat
     // diagonal index f = 4 egp + r (egp = eg + NPG >= 0).  The table is wide enough for every f a part can touch, one
@@ -253,7 +256,7 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
                     float2 v;
                     if constexpr ((r & 1) == 0) v = interp2(a, x0, x1);            // an aligned register pair: packed
                     else v = make_float2(fmaf(a, x1.x - x0.x, x0.x), fmaf(a, x1.y - x0.y, x0.y));
-                    accumulate2<K>(v, pp[2 * cg + h]);
+                    accumulate2_w<K, W>(v, pp[2 * cg + h]);
                 }
                 if constexpr (r != 0) { lo0 = hi0; lo1 = hi1; have = true; }
             }
@@ -273,31 +276,32 @@ __global__ void __launch_bounds__(kDiagMaxWarps * 32, 1) bf_diag_kernel(const T*
 
     // ---- partial power sums of the parts meet in shared memory (the staging area is dead now) ----
     __syncthreads();
-    float* red = reinterpret_cast<float*>(dg_smem + head_bytes);       // [part][warp of the part][P][K][32]
+    float* red = reinterpret_cast<float*>(dg_smem + head_bytes);       // [part][warp of the part][P][A][32]
     {
-        float* mine = red + (size_t)((part * C.wpp + wph) * P * K) * 32 + lane;
+        float* mine = red + (size_t)((part * C.wpp + wph) * P * A) * 32 + lane;
 #pragma unroll
         for (int f = 0; f < P / 2; ++f)
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
-                mine[((2 * f) * K + k) * 32] = pp[f][k].x;
-                mine[((2 * f + 1) * K + k) * 32] = pp[f][k].y;
+            for (int k = 0; k < A; ++k) {
+                mine[((2 * f) * A + k) * 32] = pp[f][k].x;
+                mine[((2 * f + 1) * A + k) * 32] = pp[f][k].y;
             }
     }
     __syncthreads();
     // ---- a6: pixel c of this lane's column phase is finished by part c % parts ----
     const size_t img = (size_t)nz * nx;
+    const float inv_n = 1.0f / (float)N;
     for (int c = part; c < P; c += C.parts) {
-        float p[K];
+        float p[A];
 #pragma unroll
-        for (int k = 0; k < K; ++k) p[k] = 0.0f;
+        for (int k = 0; k < A; ++k) p[k] = 0.0f;
         for (int pt = 0; pt < C.parts; ++pt) {
-            const float* src = red + (size_t)(((pt * C.wpp + wph) * P + c) * K) * 32 + lane;
+            const float* src = red + (size_t)(((pt * C.wpp + wph) * P + c) * A) * 32 + lane;
 #pragma unroll
-            for (int k = 0; k < K; ++k) p[k] += src[k * 32];
+            for (int k = 0; k < A; ++k) p[k] += src[k * 32];
         }
         const int j = j0 + C.q * c;
-        if (live && j < nx && m < nz) out[(size_t)frame * img + (size_t)m * nx + j] = combine<K>(p);
+        if (live && j < nx && m < nz) out[(size_t)frame * img + (size_t)m * nx + j] = combine_w<K, W>(p, inv_n);
     }
 }
 

@@ -32,8 +32,8 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
 void xl_diag_free(DiagSet* D);
 cudaError_t xl_diag_check(int order, const DiagSet& D, const float* rf, float* out, int N, int S, int nx, int nz, int* d_viol,
                           cudaStream_t st);
-void xl_diag(int order, int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
-             cudaStream_t st);
+void xl_diag(int order, int dtype, int weight, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz,
+             float scale, cudaStream_t st);
 
 // ---- pab_tu_nearest.cu: row f4 ----
 cudaError_t xl_nearest_configure(int smem_optin);

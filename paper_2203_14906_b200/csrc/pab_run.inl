@@ -34,11 +34,14 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
     const bool use_staged = ctx->variant == PAB_VARIANT_STAGED ||
                             (ctx->variant == PAB_VARIANT_AUTO && ctx->plan.smem_bytes > 0);
 
+    // table set of the single-frame diagonal kernel: 16 pixels per thread for orders 1..3, 8 for orders 4, 5 and for every order
+    // under coherence-factor weighting (more accumulators per pixel)
+    const int dset = (order <= 3 && weight == 0) ? 0 : 1;
     if (ctx->interp == PAB_INTERP_NEAREST && F < 4 && use_staged && order <= 5 && ctx->diag_near[order <= 3 ? 0 : 1].smem_bytes > 0) {
         // row f4, calls of 1..3 frames on translation-invariant geometries: the diagonal kernel on its table of integer delays
         // (fraction 0: the interpolation returns rf[n] exactly), straight from the caller's frames; roots per item
         Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-        xl_diag(order, ctx->dtype, ctx->diag_near[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
+        xl_diag(order, ctx->dtype, 0, ctx->diag_near[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
     } else if (ctx->interp == PAB_INTERP_NEAREST) {
         // row f4: rooted quad staging, then the table-driven gather kernel (always the quad layout)
         {
@@ -63,16 +66,15 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
             q0 += groups * g;
             nq -= groups * g;
         }
-    } else if (F < 4 && ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
-               ctx->diag[order <= 3 ? 0 : 1].smem_bytes > 0) {
+    } else if (F < 4 && ctx->cache_mode != PAB_CACHE_OFF && use_staged && order <= 5 && ctx->diag[dset].smem_bytes > 0) {
         // translation-invariant geometry: the diagonal kernel, straight from the caller's frames (no ingest pass)
         Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-        xl_diag(order, ctx->dtype, ctx->diag[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
-    } else if (F < 4 && ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && weight == 0 && order <= 5 &&
-               ensure_diag_nt(ctx, order, st)) {
+        xl_diag(order, ctx->dtype, weight, ctx->diag[dset], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
+    } else if (F < 4 && ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && order <= 5 &&
+               ensure_diag_nt(ctx, dset, st)) {
         // the same kernel without any delay table: the tap of a diagonal is computed in the kernel (FP64 pipe)
         Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-        xl_diag(order, ctx->dtype, ctx->diag_nt[order <= 3 ? 0 : 1], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
+        xl_diag(order, ctx->dtype, weight, ctx->diag_nt[dset], rf, P.out, F, N, S, nx, nz, ctx->scale, st);
     } else if (F < 4) {
         const bool cached = ctx->cache_mode != PAB_CACHE_OFF && use_staged && weight == 0 && order <= 5 &&
                             xl_cached_fits(ctx->plan, 0, ctx->d_compact != nullptr, ctx->smem_optin);
@@ -105,13 +107,13 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         if (rem != 0 && weight == 0 && order <= 5) {
             if (ctx->cache_mode != PAB_CACHE_OFF && use_staged && ctx->diag[order <= 3 ? 0 : 1].smem_bytes > 0)
                 dg = &ctx->diag[order <= 3 ? 0 : 1];
-            else if (ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && ensure_diag_nt(ctx, order, st))
+            else if (ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && ensure_diag_nt(ctx, order <= 3 ? 0 : 1, st))
                 dg = &ctx->diag_nt[order <= 3 ? 0 : 1];
         }
         if (dg) {
             const int Fq = F - rem;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            xl_diag(order, ctx->dtype, *dg, (const char*)rf + (size_t)Fq * N * (size_t)S * elem_size(ctx->dtype),
+            xl_diag(order, ctx->dtype, 0, *dg, (const char*)rf + (size_t)Fq * N * (size_t)S * elem_size(ctx->dtype),
                     P.out + (size_t)Fq * nz * (size_t)nx, rem, N, S, nx, nz, ctx->scale, st);
             F = Fq;                      // the frame groups below see whole quads only; the post chain still sees every frame
         }

@@ -41,28 +41,28 @@ int split_parts(int G, int npg, int nq_real, int parts, int* lo) {
     return best_cap;
 }
 
-template <int K, int NPG, typename T>
+template <int K, int NPG, typename T, int W>
 void launch_diag_t(const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale, cudaStream_t st) {
     dim3 grid(D.cfg.tiles_x * D.cfg.tiles_z, F);
     const DiagTables tabs{D.taps, D.qw0, D.qoff, D.xs_a, D.xs_b, D.zs_a, D.zs_b, D.xs2_max};
     if (D.taps)
-        bf_diag_kernel<K, NPG, T><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
+        bf_diag_kernel<K, NPG, T, false, true, W><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
     else
-        bf_diag_kernel<K, NPG, T, false, false><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
+        bf_diag_kernel<K, NPG, T, false, false, W><<<grid, D.cfg.wpp * D.cfg.parts * 32, D.smem_bytes, st>>>((const T*)rf, out, D.cfg, tabs, N, S, nx, nz, scale);
 }
-template <int K, int NPG>
+template <int K, int NPG, int W = 0>
 void launch_diag_k(int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
                    cudaStream_t st) {
-    if (dtype == PAB_I16) launch_diag_t<K, NPG, int16_t>(D, rf, out, F, N, S, nx, nz, scale, st);
-    else launch_diag_t<K, NPG, float>(D, rf, out, F, N, S, nx, nz, scale, st);
+    if (dtype == PAB_I16) launch_diag_t<K, NPG, int16_t, W>(D, rf, out, F, N, S, nx, nz, scale, st);
+    else launch_diag_t<K, NPG, float, W>(D, rf, out, F, N, S, nx, nz, scale, st);
 }
-template <int K, int NPG>
+template <int K, int NPG, int W = 0>
 cudaError_t diag_attr(int smem_optin) {
-    cudaError_t e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float, false, true, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
-    return cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if ((e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t, false, true, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(bf_diag_kernel<K, NPG, float, false, false, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(bf_diag_kernel<K, NPG, int16_t, false, false, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 
 }  // namespace
@@ -94,7 +94,13 @@ cudaError_t xl_diag_configure(int smem_optin) {
     if ((e = diag_attr<2, 4>(smem_optin)) != cudaSuccess) return e;
     if ((e = diag_attr<3, 4>(smem_optin)) != cudaSuccess) return e;
     if ((e = diag_attr<4, 2>(smem_optin)) != cudaSuccess) return e;
-    return diag_attr<5, 2>(smem_optin);
+    if ((e = diag_attr<5, 2>(smem_optin)) != cudaSuccess) return e;
+    // coherence-factor weighting: 8 pixels per thread at every order
+    if ((e = diag_attr<1, 2, 1>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<2, 2, 1>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<3, 2, 1>(smem_optin)) != cudaSuccess) return e;
+    if ((e = diag_attr<4, 2, 1>(smem_optin)) != cudaSuccess) return e;
+    return diag_attr<5, 2, 1>(smem_optin);
 }
 
 void xl_diag_free(DiagSet* D) {
@@ -191,8 +197,19 @@ cudaError_t xl_diag_build(int N, int S, double fs, double c, const pab_grid& g, 
     return cudaDeviceSynchronize();
 }
 
-void xl_diag(int order, int dtype, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz, float scale,
-             cudaStream_t st) {
+// weight = 1 (coherence factor): D must be the 8-pixel set (npg = 2), whatever the order
+void xl_diag(int order, int dtype, int weight, const DiagSet& D, const void* rf, float* out, int F, int N, int S, int nx, int nz,
+             float scale, cudaStream_t st) {
+    if (weight != 0) {
+        switch (order) {
+        case 1: launch_diag_k<1, 2, 1>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+        case 2: launch_diag_k<2, 2, 1>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+        case 3: launch_diag_k<3, 2, 1>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+        case 4: launch_diag_k<4, 2, 1>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+        default: launch_diag_k<5, 2, 1>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
+        }
+        return;
+    }
     switch (order) {
     case 1: launch_diag_k<1, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;
     case 2: launch_diag_k<2, 4>(dtype, D, rf, out, F, N, S, nx, nz, scale, st); break;

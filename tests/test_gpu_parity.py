@@ -666,6 +666,44 @@ def test_beamform_is_cuda_graph_capturable(pab, orc):
         bf.close()
 
 
+@pytest.mark.parametrize("tables", ["off", "single"])
+def test_cf_weighting_single_frames_take_the_diagonal_kernel(pab, orc, tables):
+    """Row f1 in calls of 1..3 frames on translation-invariant in-range geometries: the diagonal kernel with the two (three
+    for even orders) extra sums of the coherence factor per pixel, 8 pixels per thread at every order; both forms of the
+    kernel, orders 1..5, fp32 and int16, a ragged 61-row grid (28-row tiles), an all-zero frame (exact 0), and config C2."""
+    rng = np.random.default_rng(66)
+    fs, c, q, n_elem, nx, nz, S = 40e6, 1540.0, 2, 24, 45, 61, 900
+    dx = 2.0 ** -13
+    g = synth.Geometry(n_elem, S, fs, c, float(np.float32(q * np.float64(dx))), nx, nz, -(nx - 1) / 2 * dx + 0.3 * dx, dx, 2.1e-3,
+                       1.1 * c / fs).f32()
+    base = [(rng.uniform(-1e-3, 1e-3), rng.uniform(2.5e-3, 4.5e-3), 1.0, 0.0) for _ in range(3)]
+    rf, _ = synth._frames(rng, g, base, 5e6, 3, 20.0, True)
+    rf[1] = 0.0
+    for dtype, data, scale in (("float32", rf, 1.0), ("int16", np.rint(rf * 4000.0).astype(np.int16), 0.25)):
+        bf = pab.Beamformer(g, dtype=dtype, scale=scale, weight="cf", delay_cache=tables)
+        try:
+            for frames in (1, 3):
+                for order in (1, 2, 3, 4, 5):
+                    n0 = bf.launch_count()
+                    out = bf.beamform(torch.from_numpy(data[:frames]).cuda(), order)
+                    torch.cuda.synchronize()
+                    if not (tables == "off" and frames == 1 and order == 1):
+                        assert bf.launch_count() - n0 == 1            # one kernel, no ingest pass: the diagonal kernel
+                    gpu = out.cpu().numpy().astype(np.float64)
+                    ref = orc.beamform_ex(data[:frames], g, order, weight="cf", scale=scale)
+                    for f in range(frames):
+                        if f == 1:
+                            assert np.all(gpu[f] == 0.0) and np.all(ref[f] == 0.0)
+                        else:
+                            check_raw(gpu[f], ref[f], order)
+            assert bf.plan()["diagonal"] == (2 if tables == "off" else 1)
+        finally:
+            bf.close()
+    w = synth.make_config("C2")
+    gpu, _ = run_gpu(pab, w.geom, w.rf, 3, weight="cf", delay_cache=tables)
+    check_raw(gpu[0], orc.beamform_ex(w.rf, w.geom, 3, weight="cf")[0], 3)
+
+
 def test_single_frame_default_path_under_graph_capture(pab, orc):
     """The table-free diagonal kernel builds its windows on the first 1..3-frame call (a device synchronisation), which must not
     happen inside a stream capture: a context whose FIRST such call is captured keeps the one-frame-per-thread kernel for
