@@ -444,7 +444,8 @@ def run_sweep(args):
               ("C2b", 64, (3,), False, "cf-cache-all"), ("C4", 16, (5,), False, "cf-cache-all"),
               ("C2b", 64, (6, 8), False, "cache-all"),
               ("C3", 256, (3,), True, "cache-all"), ("C5", 1024, (3,), True, "cache-all"),
-              ("C2", 1, (1, 2, 3), False, "nearest"), ("C4", 1, (4, 5), False, "nearest")]
+              ("C2", 1, (1, 2, 3), False, "nearest"), ("C4", 1, (4, 5), False, "nearest"),
+              ("C2", 1, (3,), False, "cf"), ("C4", 1, (5,), False, "cf")]
     if args.case:                         # --case C2:1:cache-single[:3]  ->  one config / frame count / mode [/ order]
         want = args.case.split(":")
         cases = [c for c in cases if c[0] == want[0] and str(c[1]) == want[1] and c[4] == want[2]]
@@ -495,10 +496,10 @@ def run_sweep(args):
             if cache != "off" and (F < 4 or cache == "all"):
                 xu = _XU[order][0]            # taps come from the table: no delay square root in the kernel
             diag_share = 0
-            if cache == "off" and F < 4 and weight == "none" and interp == "linear" and bf.plan()["diagonal"] == 2:
+            if cache == "off" and F < 4 and interp == "linear" and bf.plan()["diagonal"] == 2:
                 # table-free diagonal kernel: one delay (one MUFU, 3 FP32-equivalent slots) per diagonal, shared by the
-                # 16 (orders 1..3) or 8 (orders 4, 5) pairs of the diagonal a thread owns
-                diag_share = 16 if order <= 3 else 8
+                # 16 (orders 1..3) or 8 (orders 4, 5, and every order under CF weighting) pairs of the diagonal a thread owns
+                diag_share = 16 if (order <= 3 and weight == "none") else 8
                 xu = _XU[order][0] + _XU[order][1] / diag_share
             taps_from_table = cache != "off" and (F < 4 or cache == "all")       # no delay arithmetic in the kernel at all
             fp = _FP32[order][0] + (0.0 if taps_from_table else _FP32[order][1] / batch) + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
@@ -507,7 +508,7 @@ def run_sweep(args):
                 if F < 4 and bf.plan()["diagonal"] == 1:      # single frames on the diagonal kernel: roots per item, not per RF sample
                     xu = _XU[order][0]
             if diag_share:
-                fp = _FP32[order][0] + _FP32[order][1] / diag_share
+                fp = _FP32[order][0] + _FP32[order][1] / diag_share + ((1.0 if order % 2 else 2.0) if weight == "cf" else 0.0)
             t_xu = items * F * xu / (SM_COUNT * XU_LANES_PER_CLK_SM * f_hz) * 1e3
             t_fp = items * F * fp / (SM_COUNT * FP32_LANES_PER_CLK_SM * f_hz) * 1e3
             in_b = g.n_elem * g.n_samp * (2 if dtype == "int16" else 4)
