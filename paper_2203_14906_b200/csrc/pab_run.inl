@@ -104,16 +104,14 @@ int run_batch(pab_ctx* ctx, const void* rf, int F, int order, float* out, cudaSt
         // buffer (measured at C2b order 3: 5 frames 181 -> 138 us, 9 frames 287 -> 215 us).
         const int rem = F & 3;
         const DiagSet* dg = nullptr;
-        if (rem != 0 && weight == 0 && order <= 5) {
-            if (ctx->cache_mode != PAB_CACHE_OFF && use_staged && ctx->diag[order <= 3 ? 0 : 1].smem_bytes > 0)
-                dg = &ctx->diag[order <= 3 ? 0 : 1];
-            else if (ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && ensure_diag_nt(ctx, order <= 3 ? 0 : 1, st))
-                dg = &ctx->diag_nt[order <= 3 ? 0 : 1];
+        if (rem != 0 && order <= 5) {
+            if (ctx->cache_mode != PAB_CACHE_OFF && use_staged && ctx->diag[dset].smem_bytes > 0) dg = &ctx->diag[dset];
+            else if (ctx->cache_mode == PAB_CACHE_OFF && ctx->variant == PAB_VARIANT_AUTO && ensure_diag_nt(ctx, dset, st)) dg = &ctx->diag_nt[dset];
         }
         if (dg) {
             const int Fq = F - rem;
             Span sp(ctx, PAB_STAGE_BEAMFORM, st);
-            xl_diag(order, ctx->dtype, 0, *dg, (const char*)rf + (size_t)Fq * N * (size_t)S * elem_size(ctx->dtype),
+            xl_diag(order, ctx->dtype, weight, *dg, (const char*)rf + (size_t)Fq * N * (size_t)S * elem_size(ctx->dtype),
                     P.out + (size_t)Fq * nz * (size_t)nx, rem, N, S, nx, nz, ctx->scale, st);
             F = Fq;                      // the frame groups below see whole quads only; the post chain still sees every frame
         }

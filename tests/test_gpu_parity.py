@@ -898,6 +898,11 @@ def test_remainder_frames_take_the_diagonal_kernel(pab, orc, dtype, tables):
                     check_raw(gpu[f], ref[f], order)
     finally:
         bf.close()
+    for frames, order in ((5, 3), (9, 2), (22, 5)):                 # the same with coherence-factor weighting
+        gpu, _ = run_gpu(pab, g, rf[:frames], order, dtype=dtype, scale=scale, weight="cf", delay_cache=tables)
+        ref = orc.beamform_ex(rf[:frames], g, order, weight="cf", scale=scale)
+        for f in range(frames):
+            check_raw(gpu[f], ref[f], order)
     post = dict(mode="log", f_center=10e6, f_halfwidth=2.5e6, n_taps_bp=64, n_taps_hilbert=63, dyn_range_db=60.0)
     gpu, _ = run_gpu(pab, g, rf[:7], 3, dtype=dtype, scale=scale, post=post, delay_cache=tables)
     ref = orc.post(orc.beamform(rf[:7], g, 3, scale=scale), g, post["f_center"], post["f_halfwidth"], post["n_taps_bp"],
